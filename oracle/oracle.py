@@ -1,0 +1,273 @@
+"""ctypes front end of ``sparrow_oracle.c`` (argument marshalling only; all arithmetic is in C).
+
+TEST INFRASTRUCTURE: see the package docstring.  bf16 tensors are numpy ``uint16`` arrays of raw
+bit patterns; everything the oracle returns is fp64 / integer numpy.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from dataclasses import dataclass, field
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "sparrow_oracle.c")
+_LIB = os.path.join(_HERE, "libsparrow_oracle.so")
+_lib = None
+
+KIND = {"dense": 0, "fixed": 1, "clamp_frac": 2, "linear_frac": 3, "table": 4}
+
+
+class _CSchedule(C.Structure):
+    _fields_ = [
+        ("kind", C.c_int32),
+        ("sink_tokens", C.c_int32),
+        ("local_tokens", C.c_int32),
+        ("fixed_tokens", C.c_int64),
+        ("floor_tokens", C.c_int64),
+        ("f0_ppm", C.c_int64),
+        ("f1_ppm", C.c_int64),
+        ("L0", C.c_int64),
+        ("L1", C.c_int64),
+        ("table_pages", C.POINTER(C.c_int32)),
+        ("table_len", C.c_int32),
+        ("bin_tokens", C.c_int32),
+    ]
+
+
+@dataclass
+class Schedule:
+    """B(L) description, oracle side (R3).  Fractions are parts per million."""
+
+    kind: str = "dense"
+    sink_tokens: int = 0
+    local_tokens: int = 0
+    fixed_tokens: int = 0
+    floor_tokens: int = 0
+    f0_ppm: int = 0
+    f1_ppm: int = 0
+    L0: int = 0
+    L1: int = 1
+    table_pages: Sequence[int] = field(default_factory=tuple)
+    bin_tokens: int = 2048
+
+    @classmethod
+    def from_spec(cls, spec: dict) -> "Schedule":
+        """Build from the plain-data schedule dict of the workload generator."""
+        return cls(**spec)
+
+    def _c(self):
+        tbl = np.ascontiguousarray(np.asarray(self.table_pages, dtype=np.int32))
+        s = _CSchedule(
+            KIND[self.kind], self.sink_tokens, self.local_tokens, self.fixed_tokens, self.floor_tokens,
+            self.f0_ppm, self.f1_ppm, self.L0, self.L1,
+            tbl.ctypes.data_as(C.POINTER(C.c_int32)), len(tbl), self.bin_tokens,
+        )
+        s._keep = tbl
+        return s
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (-O2, OpenMP).  Building the checker is not using it."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(
+            ["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared", "-o", _LIB, _SRC, "-lm"]
+        )
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = C.CDLL(_LIB)
+        _lib.oracle_budget_tokens.restype = C.c_int64
+        _lib.oracle_k_pages.restype = C.c_int64
+        _lib.oracle_forced_pages.restype = C.c_int64
+        _lib.oracle_select_unit.restype = C.c_int64
+        _lib.oracle_sparse_step.restype = C.c_int
+        _lib.oracle_num_threads.restype = C.c_int
+    return _lib
+
+
+def _p(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def _u16(a) -> np.ndarray:
+    a = np.ascontiguousarray(a)
+    assert a.dtype == np.uint16, "bf16 tensors are passed as uint16 bit patterns"
+    return a
+
+
+def _i32(a) -> np.ndarray:
+    return np.ascontiguousarray(np.asarray(a, dtype=np.int32))
+
+
+def _i64(x):
+    return C.c_int64(int(x))
+
+
+def num_threads() -> int:
+    return int(_load().oracle_num_threads())
+
+
+def budget_tokens(sched: Schedule, L: int, page_size: int = 16) -> int:
+    s = sched._c()
+    return int(_load().oracle_budget_tokens(C.byref(s), _i64(L), _i64(page_size)))
+
+
+def k_pages(sched: Schedule, L: int, page_size: int = 16) -> int:
+    s = sched._c()
+    return int(_load().oracle_k_pages(C.byref(s), _i64(L), _i64(page_size)))
+
+
+def forced_pages(L: int, S: int, W: int, page_size: int = 16) -> np.ndarray:
+    n_pages = -(-L // page_size)
+    f = np.zeros(max(n_pages, 1), dtype=np.uint8)
+    _load().oracle_forced_pages(_i64(L), _i64(S), _i64(W), _i64(page_size), _p(f))
+    return f[:n_pages].astype(bool)
+
+
+def summarize(k_cache, page_ids, n_valid=None) -> np.ndarray:
+    """O1.  k_cache [n_phys][Hkv][P][D] uint16 -> [n_update][Hkv][2][D] float64 (min, max)."""
+    k_cache = _u16(k_cache)
+    _, Hkv, P, D = k_cache.shape
+    page_ids = _i32(page_ids)
+    nv = None if n_valid is None else _i32(n_valid)
+    out = np.empty((len(page_ids), Hkv, 2, D), dtype=np.float64)
+    _load().oracle_summarize(_p(k_cache), _p(page_ids), _p(nv), _i64(len(page_ids)), _i64(Hkv), _i64(P), _i64(D), _p(out))
+    return out
+
+
+def scores_unit(q_seq, k_cache, pt_row, L: int, g: int) -> np.ndarray:
+    """O5 for one (sequence, kv-head): scores of all n_pages(L) logical pages."""
+    q_seq, k_cache, pt_row = _u16(q_seq), _u16(k_cache), _i32(pt_row)
+    Hq, D = q_seq.shape
+    _, Hkv, P, _ = k_cache.shape
+    n_pages = -(-L // P)
+    s = np.empty(n_pages, dtype=np.float64)
+    _load().oracle_scores_unit(_p(q_seq), _p(k_cache), _p(pt_row), _i64(L), _i64(g), _i64(Hq), _i64(Hkv), _i64(P), _i64(D), _p(s))
+    return s
+
+
+def select_unit(scores, forced, K_pages: int):
+    """O4, O6, O7 for one (sequence, kv-head).  Returns (ascending page list, tau)."""
+    scores = np.ascontiguousarray(scores, dtype=np.float64)
+    forced = np.ascontiguousarray(np.asarray(forced, dtype=np.uint8))
+    n_pages = len(forced)
+    sel = np.empty(max(n_pages, 1), dtype=np.int32)
+    tau = C.c_double()
+    m = _load().oracle_select_unit(_p(scores), _p(forced), _i64(n_pages), _i64(K_pages), _p(sel), C.byref(tau))
+    return sel[:m].copy(), float(tau.value)
+
+
+def attention_unit(q_seq, k_cache, v_cache, pt_row, L: int, pages, g: int, sm_scale: float, want_probs: bool = False):
+    """O8 for one (sequence, kv-head).  Returns (out [r][D], lse [r][, probs [r][n_sel*P]])."""
+    q_seq, k_cache, v_cache, pt_row, pages = _u16(q_seq), _u16(k_cache), _u16(v_cache), _i32(pt_row), _i32(pages)
+    Hq, D = q_seq.shape
+    _, Hkv, P, _ = k_cache.shape
+    r = Hq // Hkv
+    out = np.empty((r, D), dtype=np.float64)
+    lse = np.empty(r, dtype=np.float64)
+    probs = np.zeros((r, max(len(pages) * P, 1)), dtype=np.float64) if want_probs else None
+    _load().oracle_attention_unit(
+        _p(q_seq), _p(k_cache), _p(v_cache), _p(pt_row), _i64(L), _p(pages), _i64(len(pages)), _i64(g),
+        _i64(Hq), _i64(Hkv), _i64(P), _i64(D), C.c_double(sm_scale), _p(out), _p(lse), _p(probs))
+    if want_probs:
+        return out, lse, probs[:, : len(pages) * P]
+    return out, lse
+
+
+def attention_partial_unit(q_seq, k_cache, v_cache, pt_row, L: int, pages, g: int, sm_scale: float):
+    """a6 partial state (m [r], l [r], o [r][D]) of one chunk of pages."""
+    q_seq, k_cache, v_cache, pt_row, pages = _u16(q_seq), _u16(k_cache), _u16(v_cache), _i32(pt_row), _i32(pages)
+    Hq, D = q_seq.shape
+    _, Hkv, P, _ = k_cache.shape
+    r = Hq // Hkv
+    m = np.empty(r, dtype=np.float64)
+    l = np.empty(r, dtype=np.float64)
+    o = np.empty((r, D), dtype=np.float64)
+    _load().oracle_attention_partial_unit(
+        _p(q_seq), _p(k_cache), _p(v_cache), _p(pt_row), _i64(L), _p(pages), _i64(len(pages)), _i64(g),
+        _i64(Hq), _i64(Hkv), _i64(P), _i64(D), C.c_double(sm_scale), _p(m), _p(l), _p(o))
+    return m, l, o
+
+
+def lse_merge(m_i, l_i, o_i):
+    """a7 for one query head: partials m_i [n], l_i [n], o_i [n][D] -> (out [D], lse)."""
+    m_i = np.ascontiguousarray(m_i, dtype=np.float64)
+    l_i = np.ascontiguousarray(l_i, dtype=np.float64)
+    o_i = np.ascontiguousarray(o_i, dtype=np.float64)
+    n, D = o_i.shape
+    out = np.empty(D, dtype=np.float64)
+    lse = C.c_double()
+    _load().oracle_lse_merge(_p(m_i), _p(l_i), _p(o_i), _i64(n), _i64(D), _p(out), C.byref(lse))
+    return out, float(lse.value)
+
+
+def sparse_step(q, k_cache, v_cache, page_table, seq_lens, sched: Schedule, sm_scale: float,
+                max_sel: Optional[int] = None, do_attention: bool = True) -> dict:
+    """O1..O8 for a batch.  Returns a dict with every intermediate the checker needs."""
+    q, k_cache, v_cache = _u16(q), _u16(k_cache), _u16(v_cache)
+    page_table, seq_lens = _i32(page_table), _i32(seq_lens)
+    n, Hq, D = q.shape
+    _, Hkv, P, _ = k_cache.shape
+    max_pages = page_table.shape[1]
+    if max_sel is None:
+        max_sel = max_pages
+    res = dict(
+        budget_tokens=np.zeros(n, dtype=np.int64),
+        k_pages=np.zeros(n, dtype=np.int64),
+        sel_count=np.zeros(n, dtype=np.int64),
+        forced=np.zeros((n, max_pages), dtype=np.uint8),
+        scores=np.zeros((n, Hkv, max_pages), dtype=np.float64),
+        tau=np.zeros((n, Hkv), dtype=np.float64),
+        sel=np.zeros((n, Hkv, max_sel), dtype=np.int32),
+        out=np.zeros((n, Hq, D), dtype=np.float64),
+        lse=np.zeros((n, Hq), dtype=np.float64),
+    )
+    s = sched._c()
+    rc = _load().oracle_sparse_step(
+        _p(q), _p(k_cache), _p(v_cache), _p(page_table), _p(seq_lens), C.byref(s),
+        _i64(n), _i64(Hq), _i64(Hkv), _i64(P), _i64(D), _i64(max_pages), _i64(max_sel),
+        C.c_double(sm_scale), C.c_int(1 if do_attention else 0),
+        _p(res["budget_tokens"]), _p(res["k_pages"]), _p(res["sel_count"]), _p(res["forced"]),
+        _p(res["scores"]), _p(res["tau"]), _p(res["sel"]), _p(res["out"]), _p(res["lse"]))
+    if rc != 0:
+        raise ValueError("oracle_sparse_step: max_sel too small for the schedule")
+    return res
+
+
+def attention_on_sets(q, k_cache, v_cache, page_table, seq_lens, sel, sel_count, sm_scale: float):
+    """O8 on caller-supplied page lists sel [n][Hkv][max_sel] (R11).  Returns (out, lse)."""
+    q, k_cache, v_cache = _u16(q), _u16(k_cache), _u16(v_cache)
+    page_table, seq_lens, sel = _i32(page_table), _i32(seq_lens), _i32(sel)
+    sel_count = np.ascontiguousarray(np.asarray(sel_count, dtype=np.int64))
+    n, Hq, D = q.shape
+    _, Hkv, P, _ = k_cache.shape
+    out = np.zeros((n, Hq, D), dtype=np.float64)
+    lse = np.zeros((n, Hq), dtype=np.float64)
+    _load().oracle_attention_on_sets(
+        _p(q), _p(k_cache), _p(v_cache), _p(page_table), _p(seq_lens), _p(sel), _p(sel_count),
+        _i64(n), _i64(Hq), _i64(Hkv), _i64(P), _i64(D), _i64(page_table.shape[1]), _i64(sel.shape[2]),
+        C.c_double(sm_scale), _p(out), _p(lse))
+    return out, lse
+
+
+def dense_step(q, k_cache, v_cache, page_table, seq_lens, sm_scale: float):
+    """a8: dense attention over all pages.  Returns (out [n][Hq][D], lse [n][Hq])."""
+    q, k_cache, v_cache = _u16(q), _u16(k_cache), _u16(v_cache)
+    page_table, seq_lens = _i32(page_table), _i32(seq_lens)
+    n, Hq, D = q.shape
+    _, Hkv, P, _ = k_cache.shape
+    out = np.zeros((n, Hq, D), dtype=np.float64)
+    lse = np.zeros((n, Hq), dtype=np.float64)
+    _load().oracle_dense_step(
+        _p(q), _p(k_cache), _p(v_cache), _p(page_table), _p(seq_lens),
+        _i64(n), _i64(Hq), _i64(Hkv), _i64(P), _i64(D), _i64(page_table.shape[1]), C.c_double(sm_scale),
+        _p(out), _p(lse))
+    return out, lse

@@ -1,0 +1,210 @@
+"""Seeded synthetic workloads shaped like the paper's Qwen3 rollouts (BASELINE.json configs 1-5).
+
+This module serves BOTH the CUDA path and the CPU oracle and therefore holds none of the method's
+arithmetic: it draws lengths, page tables, q, K and V, plants pages (reading R19) and
+describes the schedule as plain data.  B(L), forced pages, scores, top-k and attention are each
+written twice elsewhere (oracle/ and csrc/), never here.
+
+The paper measures on AIME24 prompts x8 with a 32K cutoff and Polaris rollouts;
+those items and the Qwen3 weights are not available, so these inputs take only their *shapes*
+(Qwen3 GQA head counts, page 16, contexts up to ~40K tokens) and stand in for them.
+"""
+from __future__ import annotations
+
+import math
+from dataclasses import dataclass, field
+from typing import Dict, List, Optional
+
+import numpy as np
+import torch
+
+PAGE = 16
+HEAD_DIM = 128
+
+
+def _sched(kind, S, W, **kw) -> dict:
+    d = dict(kind=kind, sink_tokens=S, local_tokens=W, fixed_tokens=0, floor_tokens=0,
+             f0_ppm=0, f1_ppm=0, L0=0, L1=1, table_pages=(), bin_tokens=2048)
+    d.update(kw)
+    return d
+
+
+# Plain-data descriptions of BASELINE.json's configs.
+CONFIGS: Dict[str, dict] = {
+    "cfg1": dict(n_seq=2, Hq=4, Hkv=2, lengths=("list", [1024, 1500]), plant=False,
+                 schedule=_sched("fixed", 16, 64, fixed_tokens=256)),
+    "cfg1_dense": dict(n_seq=2, Hq=4, Hkv=2, lengths=("list", [1024, 1500]), plant=False,
+                       schedule=_sched("fixed", 16, 64, fixed_tokens=4096)),
+    "cfg2": dict(n_seq=64, Hq=16, Hkv=8, lengths=("uniform", 4096, 16384), plant=True,
+                 schedule=_sched("clamp_frac", 64, 512, f0_ppm=125000, floor_tokens=2048)),
+    "cfg3": dict(n_seq=128, Hq=32, Hkv=8, lengths=("uniform", 8192, 32768), plant=True,
+                 schedule=_sched("linear_frac", 64, 512, f0_ppm=250000, f1_ppm=62500, L0=8192, L1=32768,
+                                 floor_tokens=2048)),
+    # one layer pool of config 4 (36 layers = 36 calls over rotating pools, layers 0-1 dense)
+    "cfg4": dict(n_seq=256, Hq=32, Hkv=8, lengths=("lognormal", 12288, 0.7, 1024, 32768), plant=True,
+                 schedule=_sched("linear_frac", 64, 512, f0_ppm=250000, f1_ppm=62500, L0=8192, L1=32768,
+                                 floor_tokens=2048), n_layers=36, dense_layers=2),
+    "cfg5": dict(n_seq=32, Hq=40, Hkv=8, lengths=("uniform", 24576, 40960), plant=True,
+                 schedule=_sched("clamp_frac", 64, 512, f0_ppm=50000, floor_tokens=1024)),
+}
+
+
+@dataclass
+class Workload:
+    name: str
+    n_seq: int
+    Hq: int
+    Hkv: int
+    schedule: dict
+    seq_lens: torch.Tensor        # int32 [n]            (device)
+    page_table: torch.Tensor      # int32 [n][max_pages] (device), logical -> physical, padding = 0
+    q: torch.Tensor               # bf16  [n][Hq][128]
+    k_cache: torch.Tensor         # bf16  [n_phys][Hkv][16][128]
+    v_cache: torch.Tensor         # bf16  [n_phys][Hkv][16][128]
+    sm_scale: float
+    planted: Optional[List[List[np.ndarray]]] = None   # [seq][kv-head] -> planted logical pages
+    seed: int = 0
+    meta: dict = field(default_factory=dict)
+
+    @property
+    def max_pages(self) -> int:
+        return int(self.page_table.shape[1])
+
+    @property
+    def n_phys(self) -> int:
+        return int(self.k_cache.shape[0])
+
+    def host(self) -> dict:
+        """Exact bit patterns as numpy (bf16 -> uint16) for the oracle."""
+        def bits(t):
+            return t.detach().contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
+        return dict(q=bits(self.q), k_cache=bits(self.k_cache), v_cache=bits(self.v_cache),
+                    page_table=self.page_table.cpu().numpy().astype(np.int32),
+                    seq_lens=self.seq_lens.cpu().numpy().astype(np.int32))
+
+
+def draw_lengths(spec, n_seq: int, gen: torch.Generator) -> List[int]:
+    kind = spec[0]
+    if kind == "list":
+        assert len(spec[1]) == n_seq
+        return [int(x) for x in spec[1]]
+    if kind == "uniform":
+        lo, hi = spec[1], spec[2]
+        return torch.randint(lo, hi + 1, (n_seq,), generator=gen).tolist()
+    if kind == "lognormal":           # R20: median, sigma in ln-space, rejection-sampled into [lo, hi]
+        med, sig, lo, hi = spec[1:]
+        out: List[int] = []
+        while len(out) < n_seq:
+            x = med * torch.exp(sig * torch.randn(4 * n_seq, generator=gen, dtype=torch.float64))
+            out.extend(int(v) for v in x.tolist() if lo <= v <= hi)
+        return out[:n_seq]
+    raise ValueError(kind)
+
+
+def make_workload(name: str = "custom", *, n_seq: int, Hq: int, Hkv: int, lengths, schedule: dict,
+                  plant: bool = False, seed: int = 0, device="cpu", spare_pages: int = 3,
+                  poison_tail: bool = False, plant_scale: float = 3.0, plant_frac: float = 0.05,
+                  chunk_pages: int = 8192, **_ignored) -> Workload:
+    """Draw one batch.  Lengths, page tables and planted pages come from a CPU generator (so they do
+    not depend on the device); q/K/V values come from a generator on ``device``."""
+    dev = torch.device(device)
+    cg = torch.Generator(device="cpu").manual_seed(seed)
+    dg = torch.Generator(device=dev).manual_seed(seed + 7919)
+    D, P = HEAD_DIM, PAGE
+    r = Hq // Hkv
+    assert Hq == r * Hkv
+
+    lens = draw_lengths(lengths, n_seq, cg)
+    n_pages = [-(-L // P) for L in lens]
+    max_pages = max(n_pages)
+    n_phys = sum(n_pages) + spare_pages
+    perm = torch.randperm(n_phys, generator=cg)          # scattered physical placement
+    page_table = torch.zeros((n_seq, max_pages), dtype=torch.int32)
+    owner = torch.full((n_phys,), -1, dtype=torch.int64)
+    o = 0
+    for i, npg in enumerate(n_pages):
+        ids = perm[o:o + npg]
+        page_table[i, :npg] = ids.to(torch.int32)
+        owner[ids] = i
+        o += npg
+
+    q = torch.randn((n_seq, Hq, D), generator=dg, device=dev, dtype=torch.float32).to(torch.bfloat16)
+
+    planted = None
+    plant_mask = None
+    if plant:
+        planted = []
+        plant_mask = torch.zeros((n_phys, Hkv), dtype=torch.bool)
+        for i, npg in enumerate(n_pages):
+            per_head = []
+            n_pl = int(round(plant_frac * npg))
+            for g in range(Hkv):
+                lp = torch.randperm(npg, generator=cg)[:n_pl]
+                plant_mask[page_table[i, lp].long(), g] = True
+                per_head.append(np.sort(lp.numpy()))
+            planted.append(per_head)
+        # R19: offset = plant_scale * unit(sum of the group's query heads), added in fp32 before rounding
+        gq = q.float().view(n_seq, Hkv, r, D).sum(2)
+        U = plant_scale * gq / gq.norm(dim=-1, keepdim=True).clamp_min(1e-20)          # [n][Hkv][D]
+        plant_mask = plant_mask.to(dev)
+        owner_d = owner.to(dev)
+
+    k_cache = torch.empty((n_phys, Hkv, P, D), dtype=torch.bfloat16, device=dev)
+    v_cache = torch.empty((n_phys, Hkv, P, D), dtype=torch.bfloat16, device=dev)
+    for a in range(0, n_phys, chunk_pages):
+        b = min(a + chunk_pages, n_phys)
+        kf = torch.randn((b - a, Hkv, P, D), generator=dg, device=dev, dtype=torch.float32)
+        if plant:
+            own = owner_d[a:b].clamp_min(0)
+            off = U[own] * plant_mask[a:b].unsqueeze(-1)                                 # [c][Hkv][D]
+            kf += off.unsqueeze(2)
+        k_cache[a:b] = kf.to(torch.bfloat16)
+        v_cache[a:b] = torch.randn((b - a, Hkv, P, D), generator=dg, device=dev, dtype=torch.float32).to(torch.bfloat16)
+
+    if poison_tail:   # slots beyond the cached length must never influence any result
+        for i, L in enumerate(lens):
+            tail = L % P
+            if tail:
+                ph = int(page_table[i, n_pages[i] - 1])
+                k_cache[ph, :, tail:, :] = 1.0e4
+                v_cache[ph, :, tail:, :] = -1.0e4
+
+    return Workload(
+        name=name, n_seq=n_seq, Hq=Hq, Hkv=Hkv, schedule=dict(schedule),
+        seq_lens=torch.tensor(lens, dtype=torch.int32, device=dev),
+        page_table=page_table.to(dev), q=q, k_cache=k_cache, v_cache=v_cache,
+        sm_scale=1.0 / math.sqrt(D), planted=planted, seed=seed,
+        meta=dict(lengths=lengths, n_pages_total=sum(n_pages), plant=plant),
+    )
+
+
+def make_config(name: str, *, seed: Optional[int] = None, device="cpu", **overrides) -> Workload:
+    """One of BASELINE.json's configs ('cfg1', 'cfg1_dense', 'cfg2', ... 'cfg5')."""
+    spec = dict(CONFIGS[name])
+    spec.update(overrides)
+    if seed is None:
+        seed = 1000 * int("".join(ch for ch in name if ch.isdigit()) or 0)
+    return make_workload(name, seed=seed, device=device, **spec)
+
+
+def full_page_updates(wl: Workload):
+    """(page_ids, n_valid) of every page the batch owns: the post-prefill bulk summarize call."""
+    lens = wl.seq_lens.cpu().tolist()
+    pt = wl.page_table.cpu()
+    ids, nv = [], []
+    for i, L in enumerate(lens):
+        npg = -(-L // PAGE)
+        ids.append(pt[i, :npg])
+        v = torch.full((npg,), PAGE, dtype=torch.int32)
+        if L % PAGE:
+            v[-1] = L % PAGE
+        nv.append(v)
+    return torch.cat(ids).to(torch.int32), torch.cat(nv)
+
+
+def just_filled_updates(wl: Workload):
+    """(page_ids, n_valid) of pages that became full at this decode step (L % 16 == 0)."""
+    lens = wl.seq_lens.cpu().tolist()
+    pt = wl.page_table.cpu()
+    ids = [int(pt[i, L // PAGE - 1]) for i, L in enumerate(lens) if L % PAGE == 0 and L > 0]
+    return torch.tensor(ids, dtype=torch.int32), torch.full((len(ids),), PAGE, dtype=torch.int32)

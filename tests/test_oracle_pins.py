@@ -1,0 +1,352 @@
+"""Pins for the fp64 CPU oracle (``-m "not gpu"``).
+
+Each test checks ``oracle/`` against something other than itself: values worked by hand from the
+definitions (tests/golden/), numpy brute force on tiny inputs written from the token-level
+definitions, closed forms, invariants and special cases (SURVEY.md section 8(c) "what pins each part").
+A plausible mistake in the oracle (dropped term, wrong sign/index, transposed operand, off-by-one in a
+page boundary) fails at least one of them.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2606_08446_b200 import workloads as W
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+P, D = 16, 128
+
+
+def f64(bits):
+    """bf16 bit patterns -> float64 (exact)."""
+    return (np.asarray(bits, dtype=np.uint16).astype(np.uint32) << 16).view(np.float32).astype(np.float64)
+
+
+def bf16_bits(x):
+    return torch.as_tensor(np.asarray(x, dtype=np.float32)).to(torch.bfloat16).view(torch.int16).numpy().view(np.uint16)
+
+
+def tiny(n_seq=2, Hq=4, Hkv=2, lens=(70, 33), seed=0, sched=None, plant=False, **kw):
+    sched = sched or W._sched("fixed", 16, 16, fixed_tokens=48)
+    wl = W.make_workload(n_seq=n_seq, Hq=Hq, Hkv=Hkv, lengths=("list", list(lens)), schedule=sched,
+                         plant=plant, seed=seed, **kw)
+    return wl, wl.host()
+
+
+# --------------------------------------------------------------- O2-O4 budget / forced ----
+def _golden_rows():
+    rows = []
+    with open(os.path.join(GOLD, "budget_values.txt")) as f:
+        for line in f:
+            line = line.strip()
+            if not line or line.startswith("#"):
+                continue
+            c, *v = line.split()
+            rows.append((c, *map(int, v)))
+    return rows
+
+
+@pytest.mark.parametrize("row", _golden_rows(), ids=lambda r: f"{r[0]}-L{r[1]}")
+def test_budget_and_forced_match_hand_worked_values(row):
+    cfg, L, n_pages, B, K, n_forced, k, n_cand = row
+    sched = oracle.Schedule.from_spec(W.CONFIGS[cfg]["schedule"])
+    assert -(-L // P) == n_pages
+    assert oracle.budget_tokens(sched, L) == B
+    assert oracle.k_pages(sched, L) == K
+    forced = oracle.forced_pages(L, sched.sink_tokens, sched.local_tokens)
+    assert forced.sum() == n_forced
+    assert max(0, K - n_forced) == k
+    assert n_pages - n_forced == n_cand
+
+
+def test_cfg1_forced_sets_by_hand():
+    # L=1024 -> F = {0} U {60..63}; L=1500 -> F = {0} U {89..93}
+    assert np.flatnonzero(oracle.forced_pages(1024, 16, 64)).tolist() == [0, 60, 61, 62, 63]
+    assert np.flatnonzero(oracle.forced_pages(1500, 16, 64)).tolist() == [0, 89, 90, 91, 92, 93]
+
+
+def test_table4_budget_identity():
+    # PAPER.md:428-434 (Table 4, first row garbled "166-4" = "16-64"): all four configs are budget 1024
+    for page, num in ((16, 64), (32, 32), (64, 16), (128, 8)):
+        s = oracle.Schedule(kind="table", table_pages=[num], bin_tokens=2048)
+        assert oracle.budget_tokens(s, 40000, page_size=page) == 1024
+        assert oracle.k_pages(s, 40000, page_size=page) == num
+
+
+def test_table_schedule_uses_2k_length_bins():
+    # tokens grouped by position with 2K bin size; budget is a page count per bin
+    s = oracle.Schedule(kind="table", table_pages=[10, 20, 30], bin_tokens=2048)
+    assert oracle.k_pages(s, 2048) == 10 and oracle.k_pages(s, 2049) == 20
+    assert oracle.k_pages(s, 4096) == 20 and oracle.k_pages(s, 4097) == 30
+    assert oracle.k_pages(s, 99999) == 30            # beyond the table: last bin
+    assert oracle.k_pages(s, 100) == 7               # B clamps to L: ceil(100/16) pages = dense
+
+
+@pytest.mark.parametrize("seed", range(3))
+def test_forced_pages_token_level_bruteforce(seed):
+    rng = np.random.default_rng(seed)
+    for _ in range(200):
+        L = int(rng.integers(1, 700)); S = int(rng.integers(0, 80)); Wn = int(rng.integers(0, 200))
+        n_pages = -(-L // P)
+        want = np.zeros(n_pages, bool)
+        for t in range(L):                       # token-level definition
+            if t < S or t >= L - Wn:
+                want[t // P] = True
+        want[n_pages - 1] = True                 # the page of the current token is always kept
+        got = oracle.forced_pages(L, S, Wn)
+        assert np.array_equal(got, want), (L, S, Wn)
+
+
+def test_budget_clamps_and_dense_boundary():
+    # dense while the context fits the budget  =>  K_pages == n_pages iff B >= L (R13)
+    for cfg in ("cfg2", "cfg3", "cfg5"):
+        s = oracle.Schedule.from_spec(W.CONFIGS[cfg]["schedule"])
+        for L in (1, 15, 16, 17, 1000, 2047, 2048, 2049, 5000):
+            B = oracle.budget_tokens(s, L)
+            assert B == min(L, max(B, s.floor_tokens)) and B <= L
+            if L <= s.floor_tokens:
+                assert oracle.k_pages(s, L) == -(-L // P)
+    s = oracle.Schedule(kind="dense")
+    assert oracle.k_pages(s, 1500) == 94
+
+
+# ------------------------------------------------------------------------ O1 summaries ----
+def test_summaries_bruteforce_and_bounds():
+    wl, h = tiny(lens=(70, 33), seed=3)
+    ids, nv = W.full_page_updates(wl)
+    got = oracle.summarize(h["k_cache"], ids.numpy(), nv.numpy())
+    K = f64(h["k_cache"])
+    for u, (pid, v) in enumerate(zip(ids.tolist(), nv.tolist())):
+        tile = K[pid][:, :v, :]                                   # [Hkv][valid][D]
+        assert np.array_equal(got[u, :, 0], tile.min(axis=1))
+        assert np.array_equal(got[u, :, 1], tile.max(axis=1))
+        assert (got[u, :, 0][:, None, :] <= tile).all() and (tile <= got[u, :, 1][:, None, :]).all()
+    # partial page really ignores the tail: n_valid=1 gives min == max == the first key
+    one = oracle.summarize(h["k_cache"], ids.numpy()[:1], np.array([1], np.int32))
+    assert np.array_equal(one[0, :, 0], K[ids[0]][:, 0, :]) and np.array_equal(one[0, :, 0], one[0, :, 1])
+
+
+# --------------------------------------------------------------------------- O5 scores ----
+def test_scores_numpy_bruteforce_and_closed_form_R5():
+    wl, h = tiny(lens=(100, 64), seed=5)
+    K, q = f64(h["k_cache"]), f64(h["q"])
+    r = wl.Hq // wl.Hkv
+    for i, L in enumerate(h["seq_lens"].tolist()):
+        n_pages = -(-L // P)
+        for g in range(wl.Hkv):
+            s = oracle.scores_unit(h["q"][i], h["k_cache"], h["page_table"][i], L, g)
+            for p in range(n_pages):
+                valid = min(P, L - P * p)
+                tile = K[h["page_table"][i, p], g, :valid]          # [valid][D]
+                mn, mx = tile.min(0), tile.max(0)
+                qs = q[i, g * r:(g + 1) * r]                        # [r][D]
+                want = np.maximum(qs * mn, qs * mx).sum()
+                assert s[p] == pytest.approx(want, rel=1e-13, abs=1e-12)
+                # R5 closed form: sum_d (Q+ mx + Q- mn)
+                qp, qm = np.clip(qs, 0, None).sum(0), np.clip(qs, None, 0).sum(0)
+                assert s[p] == pytest.approx((qp * mx + qm * mn).sum(), rel=1e-12, abs=1e-11)
+                # Quest upper bound: per head >= max_t q.k_t ; group sum >= max_t sum_h q_h.k_t
+                dots = tile @ qs.T                                   # [valid][r]
+                assert s[p] >= dots.sum(1).max() - 1e-9
+                assert np.maximum(qs * mn, qs * mx).sum(1).min() >= -1e300   # finite
+                for j in range(r):
+                    assert np.maximum(qs[j] * mn, qs[j] * mx).sum() >= dots[:, j].max() - 1e-9
+
+
+def test_score_of_page_with_identical_keys_is_exact_dot():
+    wl, h = tiny(lens=(64,), n_seq=1, seed=7)
+    kc = h["k_cache"].copy()
+    ph = h["page_table"][0, 2]
+    kc[ph, :, :, :] = kc[ph, :, :1, :]                               # all 16 keys of page 2 identical
+    K, q = f64(kc), f64(h["q"])
+    for g in range(wl.Hkv):
+        s = oracle.scores_unit(h["q"][0], kc, h["page_table"][0], 64, g)
+        want = sum(q[0, hq] @ K[ph, g, 0] for hq in range(g * 2, g * 2 + 2))
+        assert s[2] == pytest.approx(want, rel=1e-13)
+
+
+# ---------------------------------------------------------------------------- O6 top-k ----
+def test_topk_bruteforce_lexsort_and_properties():
+    rng = np.random.default_rng(11)
+    for trial in range(200):
+        n_pages = int(rng.integers(1, 60))
+        s = rng.standard_normal(n_pages)
+        if trial % 3 == 0:
+            s = np.round(s)                                           # many exact ties
+        forced = rng.random(n_pages) < 0.2
+        forced[-1] = True
+        K = int(rng.integers(0, n_pages + 3))
+        sel, tau = oracle.select_unit(s, forced, K)
+        if K >= n_pages:
+            assert sel.tolist() == list(range(n_pages))
+            continue
+        cand = np.flatnonzero(~forced)
+        k = min(max(0, K - forced.sum()), len(cand))
+        order = cand[np.lexsort((cand, -s[cand]))]                    # score desc, then page asc
+        want = np.sort(np.concatenate([np.flatnonzero(forced), order[:k]]))
+        assert sel.tolist() == want.tolist()
+        assert len(set(sel.tolist())) == len(sel) and (np.diff(sel) > 0).all()
+        if k > 0:
+            assert tau == s[order[k - 1]]
+            assert (s[order[:k]] >= tau).all() and (s[order[k:]] <= tau).all()
+
+
+def test_topk_zero_query_ties_go_to_lowest_pages():
+    # q = 0 => every score is 0 => T = the k lowest-index candidates (pins the R10 tie-break)
+    wl, h = tiny(lens=(40 * P,), n_seq=1, seed=1, sched=W._sched("fixed", 16, 32, fixed_tokens=10 * P))
+    h["q"][:] = 0
+    res = oracle.sparse_step(h["q"], h["k_cache"], h["v_cache"], h["page_table"], h["seq_lens"],
+                             oracle.Schedule.from_spec(wl.schedule), wl.sm_scale)
+    # forced = {0} U {38, 39}; k = 10 - 3 = 7 -> candidates 1..7
+    assert res["sel"][0, 0, :10].tolist() == [0, 1, 2, 3, 4, 5, 6, 7, 38, 39]
+    assert (res["scores"][0, :, :40] == 0).all()
+
+
+def test_topk_recovers_planted_pages():
+    # strong planting (R19 alternative, oracle self-test only): top-k must contain every planted candidate
+    sched = W._sched("fixed", 16, 32, fixed_tokens=24 * P)
+    wl = W.make_workload(n_seq=2, Hq=4, Hkv=2, lengths=("list", [100 * P, 77 * P + 5]), schedule=sched,
+                         plant=True, plant_scale=40.0, plant_frac=0.08, seed=21)
+    h = wl.host()
+    res = oracle.sparse_step(h["q"], h["k_cache"], h["v_cache"], h["page_table"], h["seq_lens"],
+                             oracle.Schedule.from_spec(sched), wl.sm_scale, do_attention=False)
+    for i in range(2):
+        cnt = int(res["sel_count"][i])
+        assert cnt == 24
+        for g in range(2):
+            sel = set(res["sel"][i, g, :cnt].tolist())
+            assert len(wl.planted[i][g]) >= 6
+            assert set(wl.planted[i][g].tolist()) <= sel
+            assert (res["sel"][i, g, cnt:] == -1).all()
+
+
+# ------------------------------------------------------------------------ O8 attention ----
+def _numpy_attention(h, i, g, pages, L, Hq, Hkv, scale):
+    """Independent brute force: gather tokens, mask by position, plain softmax."""
+    K, V, q = f64(h["k_cache"]), f64(h["v_cache"]), f64(h["q"])
+    r = Hq // Hkv
+    pt = h["page_table"][i]
+    ks = np.concatenate([K[pt[p], g] for p in pages], 0)
+    vs = np.concatenate([V[pt[p], g] for p in pages], 0)
+    pos = np.concatenate([np.arange(p * P, p * P + P) for p in pages])
+    keep = pos < L
+    ks, vs = ks[keep], vs[keep]
+    out, lse = [], []
+    for hq in range(g * r, (g + 1) * r):
+        z = (ks @ q[i, hq]) * scale
+        w = np.exp(z - z.max())
+        out.append((w / w.sum()) @ vs)
+        lse.append(z.max() + np.log(w.sum()))
+    return np.array(out), np.array(lse)
+
+
+@pytest.mark.parametrize("lens", [(70, 33), (16, 17), (1, 48), (255, 256)])
+def test_dense_attention_matches_numpy_softmax(lens):
+    wl, h = tiny(lens=lens, seed=sum(lens), poison_tail=True)
+    out, lse = oracle.dense_step(h["q"], h["k_cache"], h["v_cache"], h["page_table"], h["seq_lens"], wl.sm_scale)
+    for i, L in enumerate(lens):
+        for g in range(wl.Hkv):
+            wo, wl_ = _numpy_attention(h, i, g, list(range(-(-L // P))), L, wl.Hq, wl.Hkv, wl.sm_scale)
+            np.testing.assert_allclose(out[i, g * 2:(g + 1) * 2], wo, rtol=1e-11, atol=1e-13)
+            np.testing.assert_allclose(lse[i, g * 2:(g + 1) * 2], wl_, rtol=1e-12)
+
+
+def test_softmax_rows_sum_to_one_and_one_hot_v_gives_page_mass():
+    wl, h = tiny(lens=(90,), n_seq=1, seed=9)
+    pages = [0, 2, 5]
+    out, lse, probs = oracle.attention_unit(h["q"][0], h["k_cache"], h["v_cache"], h["page_table"][0], 90,
+                                            pages, 1, wl.sm_scale, want_probs=True)
+    np.testing.assert_allclose(probs.sum(1), 1.0, rtol=1e-13)
+    assert (probs[:, 2 * P + 10:] == 0).all()            # page 5 holds tokens 80..89 only
+    # V = one-hot(page index) in channel c  =>  out[:, c] = attention mass on that page
+    vc = np.zeros_like(h["v_cache"])
+    one = bf16_bits([1.0])[0]
+    for c, p in enumerate(pages):
+        vc[h["page_table"][0, p], :, :, c] = one
+    out2, _ = oracle.attention_unit(h["q"][0], h["k_cache"], vc, h["page_table"][0], 90, pages, 1, wl.sm_scale)
+    for c in range(3):
+        np.testing.assert_allclose(out2[:, c], probs[:, c * P:(c + 1) * P].sum(1), rtol=1e-12)
+
+
+def test_zero_query_gives_mean_of_v_and_log_count():
+    wl, h = tiny(lens=(75,), n_seq=1, seed=2)
+    h["q"][:] = 0
+    out, lse = oracle.dense_step(h["q"], h["k_cache"], h["v_cache"], h["page_table"], h["seq_lens"], wl.sm_scale)
+    V = f64(h["v_cache"])
+    for g in range(wl.Hkv):
+        toks = np.concatenate([V[h["page_table"][0, p], g] for p in range(5)], 0)[:75]
+        np.testing.assert_allclose(out[0, 2 * g], toks.mean(0), rtol=1e-12, atol=1e-14)
+    np.testing.assert_allclose(lse, math.log(75), rtol=1e-13)
+
+
+def test_chunked_partials_merged_by_lse_equal_single_pass():
+    wl, h = tiny(lens=(16 * 9 + 1,), n_seq=1, seed=4)
+    L = 16 * 9 + 1
+    pages = [0, 1, 3, 4, 6, 9]
+    args = (h["q"][0], h["k_cache"], h["v_cache"], h["page_table"][0], L)
+    for g in range(wl.Hkv):
+        full_out, full_lse = oracle.attention_unit(*args, pages, g, wl.sm_scale)
+        # chunks incl. an empty one and one whose only page has a single valid token (page 9)
+        chunks = [[0, 1], [], [3, 4, 6], [9]]
+        parts = [oracle.attention_partial_unit(*args, c, g, wl.sm_scale) for c in chunks]
+        assert parts[1][1].tolist() == [0.0, 0.0] and np.isneginf(parts[1][0]).all()
+        for j in range(2):
+            o, lse = oracle.lse_merge([p[0][j] for p in parts], [p[1][j] for p in parts],
+                                      np.stack([p[2][j] for p in parts]))
+            assert np.isfinite(o).all()
+            np.testing.assert_allclose(o, full_out[j], rtol=1e-12, atol=1e-14)
+            assert lse == pytest.approx(full_lse[j], rel=1e-13)
+    # all-empty merge: no NaN
+    o, lse = oracle.lse_merge([-np.inf], [0.0], np.zeros((1, D)))
+    assert (o == 0).all() and lse == -np.inf
+
+
+# --------------------------------------------------------------------------- end to end ----
+def test_sparse_equals_dense_when_budget_covers_context():
+    # PAPER.md:494-496 (L_dense): sparse == dense whenever L <= B   (BASELINE.json config 1, B >= L run)
+    wl = W.make_config("cfg1_dense")
+    h = wl.host()
+    sched = oracle.Schedule.from_spec(wl.schedule)
+    res = oracle.sparse_step(h["q"], h["k_cache"], h["v_cache"], h["page_table"], h["seq_lens"], sched, wl.sm_scale)
+    out, lse = oracle.dense_step(h["q"], h["k_cache"], h["v_cache"], h["page_table"], h["seq_lens"], wl.sm_scale)
+    assert res["sel_count"].tolist() == [64, 94]
+    assert np.array_equal(res["out"], out) and np.array_equal(res["lse"], lse)
+    assert np.isnan(res["tau"]).all()
+
+
+def test_cfg1_sparse_structure_and_attention_on_sets():
+    wl = W.make_config("cfg1")
+    h = wl.host()
+    sched = oracle.Schedule.from_spec(wl.schedule)
+    res = oracle.sparse_step(h["q"], h["k_cache"], h["v_cache"], h["page_table"], h["seq_lens"], sched, wl.sm_scale)
+    assert res["sel_count"].tolist() == [16, 16] and res["k_pages"].tolist() == [16, 16]
+    for i, F in enumerate(([0, 60, 61, 62, 63], [0, 89, 90, 91, 92, 93])):
+        for g in range(2):
+            sel = res["sel"][i, g, :16]
+            assert set(F) <= set(sel.tolist()) and (np.diff(sel) > 0).all()
+            # every selected candidate scores >= tau >= every unselected candidate
+            n_pages = -(-int(h["seq_lens"][i]) // P)
+            s = res["scores"][i, g, :n_pages]
+            cand_in = [p for p in sel if p not in F]
+            cand_out = [p for p in range(n_pages) if p not in set(sel.tolist())]
+            assert min(s[cand_in]) == res["tau"][i, g] and max(s[cand_out]) <= res["tau"][i, g]
+            wo, wlse = _numpy_attention(h, i, g, sel.tolist(), int(h["seq_lens"][i]), 4, 2, wl.sm_scale)
+            np.testing.assert_allclose(res["out"][i, 2 * g:2 * g + 2], wo, rtol=1e-11, atol=1e-13)
+            np.testing.assert_allclose(res["lse"][i, 2 * g:2 * g + 2], wlse, rtol=1e-12)
+    o2, l2 = oracle.attention_on_sets(h["q"], h["k_cache"], h["v_cache"], h["page_table"], h["seq_lens"],
+                                      res["sel"], res["sel_count"], wl.sm_scale)
+    assert np.array_equal(o2, res["out"]) and np.array_equal(l2, res["lse"])
+    # sparse differs from dense (it is an approximation), but not wildly: same sign of lse gap
+    _, lse_d = oracle.dense_step(h["q"], h["k_cache"], h["v_cache"], h["page_table"], h["seq_lens"], wl.sm_scale)
+    assert (res["lse"] < lse_d).all()           # attending a strict subset of tokens lowers the log-sum-exp
+
+
+def test_oracle_rejects_undersized_max_sel():
+    wl = W.make_config("cfg1")
+    h = wl.host()
+    with pytest.raises(ValueError):
+        oracle.sparse_step(h["q"], h["k_cache"], h["v_cache"], h["page_table"], h["seq_lens"],
+                           oracle.Schedule.from_spec(wl.schedule), wl.sm_scale, max_sel=8)
