@@ -1,0 +1,160 @@
+/*
+ * sparrow.h -- C ABI of the B200-native sparse decode attention of Sparrow's sparse rollout
+ * (arxiv/paper_2606_08446).  One shared library, libsparrow_b200.so, hand-written CUDA for sm_100a.
+ *
+ * What the calls compute (paper passages; readings R1..R20):
+ *   per decode step and layer:  page "landmark" scores  ->  Top-k pages under the KV budget
+ *   B = pagesize x num_pages  ->  attention over the B selected tokens            (Eq. 3)
+ *   the budget grows with sequence length (dynamic sparsity schedule, 2K-token bins)
+ *   attention is dense while the context still fits the budget
+ *   page size 16
+ * The paper leaves the selector's details open; BASELINE.json north_star fixes them: page summaries are
+ * per-channel key min/max, the score is the upper bound of q.k against the summary summed over the GQA
+ * group, sink and local-window pages are always kept, the top-k remaining pages fill B(L).
+ *
+ * Conventions (all entry points)
+ *   - Every pointer is a DEVICE pointer owned by the caller unless the parameter is documented "host".
+ *     The library never allocates, frees or synchronises on the device-pointer entry points; work is
+ *     enqueued on `stream` (a cudaStream_t passed as void*, NULL = the legacy default stream) and the
+ *     calls can be captured in a CUDA graph.  Device pointers must be 16-byte aligned.
+ *   - bf16 tensors are raw 16-bit patterns.  Layouts (row-major, innermost last):
+ *       k_cache, v_cache  [n_phys_pages][n_kv_heads][page_size=16][head_dim=128]   bf16  ("HND" pages)
+ *       summaries         [n_phys_pages][n_kv_heads][2][128]                       bf16  ([0]=min, [1]=max)
+ *       q, out            [n_seq][n_q_heads][128]                                  bf16
+ *       lse               [n_seq][n_q_heads]                                       fp32  (natural log)
+ *       page_table        [n_seq][max_pages_per_seq]                               int32 logical -> physical
+ *       seq_lens          [n_seq]                                                  int32 L = cached length
+ *                                                      INCLUDING the current token (R6); L >= 1
+ *       sel_pages         [n_seq][n_kv_heads][max_sel]                             int32 logical pages,
+ *                                                      ascending, forced pages included
+ *       sel_count         [n_seq]                                                  int32 (same for all kv heads)
+ *     Query head h uses kv head h / r, r = n_q_heads / n_kv_heads (GQA; K/V are read once per group).
+ *   - Return value: SPARROW_OK (0) or a negative sparrow_status; nothing throws, aborts or falls back to
+ *     the CPU.  Supported: head_dim = 128, page_size = 16, 1 <= r <= 8, bf16; anything else returns
+ *     SPARROW_ERR_UNSUPPORTED.
+ */
+#ifndef SPARROW_H_
+#define SPARROW_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum sparrow_status {
+    SPARROW_OK = 0,
+    SPARROW_ERR_INVALID_ARG = -1,        /* null / negative / misaligned argument */
+    SPARROW_ERR_UNSUPPORTED = -2,        /* shape outside the supported set (see above) */
+    SPARROW_ERR_WORKSPACE_TOO_SMALL = -3,
+    SPARROW_ERR_CUDA = -4                /* launch or runtime failure; text via sparrow_strerror */
+} sparrow_status;
+
+typedef struct sparrow_shape {
+    int32_t n_seq;               /* sequences in the batch (n) */
+    int32_t n_q_heads;           /* Hq */
+    int32_t n_kv_heads;          /* Hkv */
+    int32_t head_dim;            /* D, must be 128 */
+    int32_t page_size;           /* P, must be 16 */
+    int32_t max_pages_per_seq;   /* row stride of page_table */
+    int64_t n_phys_pages;        /* pages in the K/V pools */
+} sparrow_shape_t;
+
+/* Dynamic sparsity schedule B(L) in EXACT integer arithmetic (R3), so that host, device and any checker
+ * agree bit for bit.  Fractions are parts per million.  After the kind-specific value B is clamped to
+ * at least floor_tokens (kinds 2, 3) and at most L.  K_pages = min(ceil(B/16), ceil(L/16)) (R4); a
+ * sequence with K_pages >= n_pages is dense. */
+enum {
+    SPARROW_SCHED_DENSE = 0,        /* B = L */
+    SPARROW_SCHED_FIXED = 1,        /* B = fixed_tokens */
+    SPARROW_SCHED_CLAMP_FRAC = 2,   /* B = max(floor(L*f0_ppm/1e6), floor_tokens) */
+    SPARROW_SCHED_LINEAR_FRAC = 3,  /* keep fraction falls linearly from f0_ppm at L0 to f1_ppm at L1 (clamped outside) */
+    SPARROW_SCHED_TABLE = 4         /* the paper's native form: pages per length bin, bin b = (L-1)/bin_tokens
+                                       (2K bins); B = table_pages[b] * 16 */
+};
+#define SPARROW_MAX_TABLE_BINS 64
+
+typedef struct sparrow_schedule {
+    int32_t kind;
+    int32_t sink_tokens;          /* S: pages [0, ceil(S/16)) are always kept (R8) */
+    int32_t local_tokens;         /* W: every page overlapping the last W tokens is always kept (R7);
+                                     the last page is kept even when W = 0 (R9) */
+    int64_t fixed_tokens;
+    int64_t floor_tokens;
+    int64_t f0_ppm, f1_ppm;
+    int64_t L0, L1;
+    const int32_t *table_pages;   /* HOST pointer, table_len <= SPARROW_MAX_TABLE_BINS entries; copied by value */
+    int32_t table_len;
+    int32_t bin_tokens;
+} sparrow_schedule_t;
+
+/* ---- a1: page summaries (north_star (a); "landmark") -------------------------------
+ * For u < n_update: page = page_ids ? page_ids[u] : u; valid = n_valid ? n_valid[u] : 16.
+ * summaries[page][g][0][d] = min over t < valid of k_cache[page][g][t][d], [1] = max.  Results are exact
+ * (a min/max of bf16 values).  Runs on page fill (a few pages per step) or in bulk after prefill. */
+int sparrow_summarize(const void *k_cache, void *summaries, const int32_t *page_ids, const int32_t *n_valid,
+                      int64_t n_update, const sparrow_shape_t *shape, void *stream);
+
+/* ---- a2..a5: budget, forced pages, fused page scoring + per-(sequence, kv-head) top-k ------------
+ * For every sequence: B(L) from `sched`; forced pages F (sink, local window, last page); candidates =
+ * the other pages, scored  s[p] = sum_{h in group} sum_d max(q[h][d]*min[p][d], q[h][d]*max[p][d])  in
+ * fp32; the k = max(0, K_pages - |F|) best candidates (ties: lower page index, R10) join F.  Output:
+ * sel_pages ascending, sel_count[i] = n_pages if dense else max(K_pages, |F|).  `max_sel` must be
+ * >= sparrow_max_sel_pages(sched, longest L) (precondition; the kernel clamps instead of overflowing).
+ * scores_dbg: optional fp32 [n_seq][n_kv_heads][max_pages_per_seq]; candidate scores are written there
+ * (other entries untouched).  workspace: sparrow_select_workspace_bytes(shape) bytes, ZERO-INITIALISED
+ * once by the caller; the kernel restores the zeros it uses, so it can be reused call after call. */
+int sparrow_select(const void *q, const void *summaries, const int32_t *page_table, const int32_t *seq_lens,
+                   const sparrow_schedule_t *sched, int32_t *sel_pages, int32_t max_sel, int32_t *sel_count,
+                   float *scores_dbg, void *workspace, size_t workspace_bytes,
+                   const sparrow_shape_t *shape, void *stream);
+
+/* ---- a6 + a7: split-K flash-decode over the selected pages, log-sum-exp merge ---------------------
+ * out[i][h] = softmax_t(sm_scale * q[i][h].K_t) V_t over tokens t < L of the pages sel_pages[i][h/r][0..sel_count[i]),
+ * gathered through page_table; fp32 accumulation, bf16 output; lse (optional, may be NULL) = ln sum exp.
+ * workspace: sparrow_decode_workspace_bytes(shape, max_sel) bytes, contents irrelevant. */
+int sparrow_sparse_decode(const void *q, const void *k_cache, const void *v_cache, const int32_t *page_table,
+                          const int32_t *seq_lens, const int32_t *sel_pages, int32_t max_sel,
+                          const int32_t *sel_count, void *out, float *lse, float sm_scale,
+                          void *workspace, size_t workspace_bytes, const sparrow_shape_t *shape, void *stream);
+
+/* ---- a8: dense decode = the same kernels with B(L) = L (all ceil(L/16) pages) ---
+ * workspace: sparrow_decode_workspace_bytes(shape, 0) bytes. */
+int sparrow_dense_decode(const void *q, const void *k_cache, const void *v_cache, const int32_t *page_table,
+                         const int32_t *seq_lens, void *out, float *lse, float sm_scale,
+                         void *workspace, size_t workspace_bytes, const sparrow_shape_t *shape, void *stream);
+
+/* ---- whole step through HOST buffers (the end-to-end measurement path) ----------------------------
+ * Copies this step's inputs from host memory (q_host [n][Hq][128] bf16, seq_lens_host [n] int32; pinned
+ * memory makes the copies asynchronous), runs summarize (n_update pages, page_ids/n_valid are HOST arrays,
+ * n_update may be 0) -> select -> sparse decode (or the dense path when sched->kind == DENSE) on `stream`,
+ * copies out back to out_host [n][Hq][128] bf16 and WAITS for the stream.  The K/V pools, summaries and
+ * page_table are the resident cache state and stay device pointers.  `scratch` is a device buffer of at
+ * least sparrow_step_scratch_bytes(shape, max_sel) bytes, zero-initialised once by the caller. */
+int sparrow_step_host(const void *q_host, const int32_t *seq_lens_host,
+                      const int32_t *page_ids_host, const int32_t *n_valid_host, int64_t n_update,
+                      const void *k_cache, const void *v_cache, void *summaries, const int32_t *page_table,
+                      const sparrow_schedule_t *sched, int32_t max_sel, float sm_scale,
+                      void *out_host, void *scratch, size_t scratch_bytes,
+                      const sparrow_shape_t *shape, void *stream);
+
+/* ---- host helpers (no device work; callable without a GPU) ---------------------------------------- */
+size_t sparrow_select_workspace_bytes(const sparrow_shape_t *shape);
+size_t sparrow_decode_workspace_bytes(const sparrow_shape_t *shape, int32_t max_sel /* 0 = dense */);
+size_t sparrow_step_scratch_bytes(const sparrow_shape_t *shape, int32_t max_sel);
+/* B(L) in tokens, K_pages, number of forced pages, and the bound on sel_count over all L <= max_len. */
+int64_t sparrow_budget_tokens(const sparrow_schedule_t *sched, int64_t L);
+int32_t sparrow_k_pages(const sparrow_schedule_t *sched, int64_t L);
+int32_t sparrow_forced_count(const sparrow_schedule_t *sched, int64_t L);
+int32_t sparrow_sel_count(const sparrow_schedule_t *sched, int64_t L);
+int32_t sparrow_max_sel_pages(const sparrow_schedule_t *sched, int64_t max_len);
+const char *sparrow_strerror(int status);   /* static string; for SPARROW_ERR_CUDA includes the last CUDA error text */
+int sparrow_version(void);
+/* Kernels launched by the most recent entry-point call on this thread (for gpu_launches accounting). */
+int sparrow_last_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPARROW_H_ */

@@ -1,0 +1,196 @@
+"""Thin ctypes binding of libsparrow_b200.so: same names as include/sparrow.h, argument marshalling only.
+
+Every step of the path runs in the CUDA kernels.  torch is used for device memory and streams.  There is no
+CPU fallback: if the shared library is missing this module raises at import, and a non-zero status raises
+``SparrowError``.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libsparrow_b200.so")
+if not os.path.exists(LIB_PATH):
+    raise ImportError(
+        f"{LIB_PATH} is missing: build it with `python -m paper_2606_08446_b200.build` "
+        "(or __graft_entry__.build()); there is no fallback path")
+_lib = C.CDLL(LIB_PATH)
+
+SCHED_KIND = {"dense": 0, "fixed": 1, "clamp_frac": 2, "linear_frac": 3, "table": 4}
+
+
+class SparrowError(RuntimeError):
+    pass
+
+
+class sparrow_shape_t(C.Structure):
+    _fields_ = [("n_seq", C.c_int32), ("n_q_heads", C.c_int32), ("n_kv_heads", C.c_int32), ("head_dim", C.c_int32),
+                ("page_size", C.c_int32), ("max_pages_per_seq", C.c_int32), ("n_phys_pages", C.c_int64)]
+
+
+class sparrow_schedule_t(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("sink_tokens", C.c_int32), ("local_tokens", C.c_int32),
+                ("fixed_tokens", C.c_int64), ("floor_tokens", C.c_int64), ("f0_ppm", C.c_int64), ("f1_ppm", C.c_int64),
+                ("L0", C.c_int64), ("L1", C.c_int64), ("table_pages", C.POINTER(C.c_int32)),
+                ("table_len", C.c_int32), ("bin_tokens", C.c_int32)]
+
+
+def make_shape(n_seq, n_q_heads, n_kv_heads, max_pages_per_seq, n_phys_pages, head_dim=128, page_size=16):
+    return sparrow_shape_t(n_seq, n_q_heads, n_kv_heads, head_dim, page_size, max_pages_per_seq, n_phys_pages)
+
+
+def make_schedule(spec: dict) -> sparrow_schedule_t:
+    """From the plain-data schedule dict of ``workloads`` (kind, sink_tokens, ... table_pages, bin_tokens)."""
+    tbl = (C.c_int32 * max(1, len(spec.get("table_pages", ()))))(*spec.get("table_pages", ()))
+    s = sparrow_schedule_t(SCHED_KIND[spec["kind"]], spec.get("sink_tokens", 0), spec.get("local_tokens", 0),
+                           spec.get("fixed_tokens", 0), spec.get("floor_tokens", 0), spec.get("f0_ppm", 0),
+                           spec.get("f1_ppm", 0), spec.get("L0", 0), spec.get("L1", 1),
+                           C.cast(tbl, C.POINTER(C.c_int32)), len(spec.get("table_pages", ())), spec.get("bin_tokens", 2048))
+    s._keep = tbl
+    return s
+
+
+_vp, _i32, _i64, _sz, _f = C.c_void_p, C.c_int32, C.c_int64, C.c_size_t, C.c_float
+_SHP, _SCH = C.POINTER(sparrow_shape_t), C.POINTER(sparrow_schedule_t)
+_SIGS = {
+    "sparrow_summarize": (C.c_int, [_vp, _vp, _vp, _vp, _i64, _SHP, _vp]),
+    "sparrow_select": (C.c_int, [_vp, _vp, _vp, _vp, _SCH, _vp, _i32, _vp, _vp, _vp, _sz, _SHP, _vp]),
+    "sparrow_sparse_decode": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _i32, _vp, _vp, _vp, _f, _vp, _sz, _SHP, _vp]),
+    "sparrow_dense_decode": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _f, _vp, _sz, _SHP, _vp]),
+    "sparrow_step_host": (C.c_int, [_vp, _vp, _vp, _vp, _i64, _vp, _vp, _vp, _vp, _SCH, _i32, _f, _vp, _vp, _sz, _SHP, _vp]),
+    "sparrow_select_workspace_bytes": (_sz, [_SHP]),
+    "sparrow_decode_workspace_bytes": (_sz, [_SHP, _i32]),
+    "sparrow_step_scratch_bytes": (_sz, [_SHP, _i32]),
+    "sparrow_budget_tokens": (_i64, [_SCH, _i64]),
+    "sparrow_k_pages": (_i32, [_SCH, _i64]),
+    "sparrow_forced_count": (_i32, [_SCH, _i64]),
+    "sparrow_sel_count": (_i32, [_SCH, _i64]),
+    "sparrow_max_sel_pages": (_i32, [_SCH, _i64]),
+    "sparrow_strerror": (C.c_char_p, [C.c_int]),
+    "sparrow_version": (C.c_int, []),
+    "sparrow_last_launch_count": (C.c_int, []),
+}
+for _name, (_res, _args) in _SIGS.items():
+    _fn = getattr(_lib, _name)          # AttributeError here = the library does not export a declared symbol
+    _fn.restype, _fn.argtypes = _res, _args
+EXPORTS = tuple(_SIGS)
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        raise SparrowError(f"{what}: {_lib.sparrow_strerror(rc).decode()} (status {rc})")
+
+
+def _ptr(t: Optional[torch.Tensor], *, cuda: bool = True):
+    if t is None:
+        return None
+    assert t.is_contiguous(), "tensors must be contiguous"
+    if cuda:
+        assert t.is_cuda, "device pointer expected"
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream(stream):
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(stream.cuda_stream)
+
+
+def _by(x):
+    return C.byref(x)
+
+
+def sparrow_version() -> int:
+    return _lib.sparrow_version()
+
+
+def sparrow_last_launch_count() -> int:
+    return _lib.sparrow_last_launch_count()
+
+
+def sparrow_strerror(rc: int) -> str:
+    return _lib.sparrow_strerror(rc).decode()
+
+
+def sparrow_select_workspace_bytes(shape) -> int:
+    return _lib.sparrow_select_workspace_bytes(_by(shape))
+
+
+def sparrow_decode_workspace_bytes(shape, max_sel: int) -> int:
+    return _lib.sparrow_decode_workspace_bytes(_by(shape), max_sel)
+
+
+def sparrow_step_scratch_bytes(shape, max_sel: int) -> int:
+    return _lib.sparrow_step_scratch_bytes(_by(shape), max_sel)
+
+
+def sparrow_budget_tokens(sched, L: int) -> int:
+    return _lib.sparrow_budget_tokens(_by(sched), L)
+
+
+def sparrow_k_pages(sched, L: int) -> int:
+    return _lib.sparrow_k_pages(_by(sched), L)
+
+
+def sparrow_forced_count(sched, L: int) -> int:
+    return _lib.sparrow_forced_count(_by(sched), L)
+
+
+def sparrow_sel_count(sched, L: int) -> int:
+    return _lib.sparrow_sel_count(_by(sched), L)
+
+
+def sparrow_max_sel_pages(sched, max_len: int) -> int:
+    return _lib.sparrow_max_sel_pages(_by(sched), max_len)
+
+
+def sparrow_summarize(k_cache, summaries, page_ids, n_valid, n_update: int, shape, stream=None, *, check=True):
+    rc = _lib.sparrow_summarize(_ptr(k_cache), _ptr(summaries), _ptr(page_ids), _ptr(n_valid), n_update, _by(shape), _stream(stream))
+    if check:
+        _check(rc, "sparrow_summarize")
+    return rc
+
+
+def sparrow_select(q, summaries, page_table, seq_lens, sched, sel_pages, max_sel: int, sel_count, scores_dbg,
+                   workspace, shape, stream=None, *, check=True):
+    rc = _lib.sparrow_select(_ptr(q), _ptr(summaries), _ptr(page_table), _ptr(seq_lens), _by(sched), _ptr(sel_pages), max_sel,
+                             _ptr(sel_count), _ptr(scores_dbg), _ptr(workspace),
+                             0 if workspace is None else workspace.numel() * workspace.element_size(), _by(shape), _stream(stream))
+    if check:
+        _check(rc, "sparrow_select")
+    return rc
+
+
+def sparrow_sparse_decode(q, k_cache, v_cache, page_table, seq_lens, sel_pages, max_sel: int, sel_count, out, lse,
+                          sm_scale: float, workspace, shape, stream=None, *, check=True):
+    rc = _lib.sparrow_sparse_decode(_ptr(q), _ptr(k_cache), _ptr(v_cache), _ptr(page_table), _ptr(seq_lens), _ptr(sel_pages),
+                                    max_sel, _ptr(sel_count), _ptr(out), _ptr(lse), sm_scale, _ptr(workspace),
+                                    0 if workspace is None else workspace.numel() * workspace.element_size(), _by(shape), _stream(stream))
+    if check:
+        _check(rc, "sparrow_sparse_decode")
+    return rc
+
+
+def sparrow_dense_decode(q, k_cache, v_cache, page_table, seq_lens, out, lse, sm_scale: float, workspace, shape,
+                         stream=None, *, check=True):
+    rc = _lib.sparrow_dense_decode(_ptr(q), _ptr(k_cache), _ptr(v_cache), _ptr(page_table), _ptr(seq_lens), _ptr(out), _ptr(lse),
+                                   sm_scale, _ptr(workspace),
+                                   0 if workspace is None else workspace.numel() * workspace.element_size(), _by(shape), _stream(stream))
+    if check:
+        _check(rc, "sparrow_dense_decode")
+    return rc
+
+
+def sparrow_step_host(q_host, seq_lens_host, page_ids_host, n_valid_host, n_update: int, k_cache, v_cache, summaries,
+                      page_table, sched, max_sel: int, sm_scale: float, out_host, scratch, shape, stream=None, *, check=True):
+    rc = _lib.sparrow_step_host(_ptr(q_host, cuda=False), _ptr(seq_lens_host, cuda=False), _ptr(page_ids_host, cuda=False),
+                                _ptr(n_valid_host, cuda=False), n_update, _ptr(k_cache), _ptr(v_cache), _ptr(summaries),
+                                _ptr(page_table), _by(sched), max_sel, sm_scale, _ptr(out_host, cuda=False), _ptr(scratch),
+                                scratch.numel() * scratch.element_size(), _by(shape), _stream(stream))
+    if check:
+        _check(rc, "sparrow_step_host")
+    return rc

@@ -1,0 +1,399 @@
+// api.cu -- the C ABI of libsparrow_b200 (include/sparrow.h): argument validation, launch geometry, workspaces.
+// Every step of the path runs in the kernels of summarize.cuh / select.cuh / decode.cuh; there is no CPU fallback.
+#include <stdio.h>
+#include <string.h>
+
+#include "common.cuh"
+#include "decode.cuh"
+#include "select.cuh"
+#include "summarize.cuh"
+
+using namespace sparrow;
+
+namespace {
+
+thread_local int g_launches = 0;
+thread_local char g_errbuf[256] = "";
+constexpr int kNumSmsB200 = 148;
+
+int cuda_fail(cudaError_t e, const char *where)
+{
+    snprintf(g_errbuf, sizeof(g_errbuf), "CUDA error in %s: %s", where, cudaGetErrorString(e));
+    return SPARROW_ERR_CUDA;
+}
+#define SPARROW_CHECK_LAUNCH(where)                         \
+    do {                                                    \
+        cudaError_t e__ = cudaGetLastError();               \
+        if (e__ != cudaSuccess) return cuda_fail(e__, where); \
+        ++g_launches;                                       \
+    } while (0)
+
+bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+int check_shape(const sparrow_shape_t *s)
+{
+    if (!s) return SPARROW_ERR_INVALID_ARG;
+    if (s->n_seq < 0 || s->n_q_heads <= 0 || s->n_kv_heads <= 0 || s->max_pages_per_seq <= 0 || s->n_phys_pages < 0)
+        return SPARROW_ERR_INVALID_ARG;
+    if (s->head_dim != kDim || s->page_size != kPage) return SPARROW_ERR_UNSUPPORTED;
+    if (s->n_q_heads % s->n_kv_heads != 0) return SPARROW_ERR_UNSUPPORTED;
+    const int r = s->n_q_heads / s->n_kv_heads;
+    if (r < 1 || r > kMaxGroup) return SPARROW_ERR_UNSUPPORTED;
+    if (s->n_kv_heads > 65535 || s->n_seq > 65535) return SPARROW_ERR_UNSUPPORTED;     // grid.y / grid.z
+    return SPARROW_OK;
+}
+
+int to_dev_sched(const sparrow_schedule_t *in, SchedDev *out)
+{
+    if (!in) return SPARROW_ERR_INVALID_ARG;
+    if (in->kind < SPARROW_SCHED_DENSE || in->kind > SPARROW_SCHED_TABLE) return SPARROW_ERR_INVALID_ARG;
+    if (in->sink_tokens < 0 || in->local_tokens < 0) return SPARROW_ERR_INVALID_ARG;
+    memset(out, 0, sizeof(*out));
+    out->kind = in->kind;
+    out->sink_tokens = in->sink_tokens;
+    out->local_tokens = in->local_tokens;
+    out->fixed_tokens = in->fixed_tokens;
+    out->floor_tokens = in->floor_tokens;
+    out->f0_ppm = in->f0_ppm;
+    out->f1_ppm = in->f1_ppm;
+    out->L0 = in->L0;
+    out->L1 = in->L1;
+    out->bin_tokens = in->bin_tokens;
+    if (in->kind == SPARROW_SCHED_FIXED && in->fixed_tokens < 0) return SPARROW_ERR_INVALID_ARG;
+    if (in->kind == SPARROW_SCHED_CLAMP_FRAC && (in->f0_ppm < 0 || in->floor_tokens < 0)) return SPARROW_ERR_INVALID_ARG;
+    if (in->kind == SPARROW_SCHED_LINEAR_FRAC &&
+        (in->L1 <= in->L0 || in->f0_ppm < 0 || in->f1_ppm < 0 || in->floor_tokens < 0))
+        return SPARROW_ERR_INVALID_ARG;
+    if (in->kind == SPARROW_SCHED_TABLE) {
+        if (!in->table_pages || in->table_len <= 0 || in->table_len > SPARROW_MAX_TABLE_BINS || in->bin_tokens <= 0)
+            return SPARROW_ERR_INVALID_ARG;
+        out->table_len = in->table_len;
+        for (int i = 0; i < in->table_len; ++i) {
+            if (in->table_pages[i] < 0) return SPARROW_ERR_INVALID_ARG;
+            out->table[i] = in->table_pages[i];
+        }
+    }
+    return SPARROW_OK;
+}
+
+// Pages of the list that one CTA (= one split) handles.  Larger chunks amortise the per-CTA prologue and the
+// partial write; smaller ones give enough CTAs to fill 148 SMs x 2 resident CTAs for several waves.
+int pick_chunk_pages(int64_t n_units, int max_cnt)
+{
+    const int64_t want = 4 * 2 * kNumSmsB200;
+    for (int c = kMaxChunkPages; c > kDecWarps; c >>= 1) {
+        const int64_t items = n_units * ((max_cnt + c - 1) / c);
+        if (items >= want) return c;
+    }
+    return kDecWarps;
+}
+
+struct DecodeGeom {
+    int max_cnt, chunk, n_splits;
+    size_t bytes_o, bytes_ml;
+};
+DecodeGeom decode_geom(const sparrow_shape_t *s, int max_sel)
+{
+    DecodeGeom gm;
+    gm.max_cnt = max_sel > 0 ? (max_sel < s->max_pages_per_seq ? max_sel : s->max_pages_per_seq) : s->max_pages_per_seq;
+    const int64_t units = (int64_t)s->n_seq * s->n_kv_heads;
+    gm.chunk = pick_chunk_pages(units, gm.max_cnt);
+    gm.n_splits = (gm.max_cnt + gm.chunk - 1) / gm.chunk;
+    const size_t rows = (size_t)units * gm.n_splits * (s->n_q_heads / s->n_kv_heads);
+    gm.bytes_o = (rows * kDim * sizeof(float) + 255) & ~(size_t)255;
+    gm.bytes_ml = (rows * 2 * sizeof(float) + 255) & ~(size_t)255;
+    return gm;
+}
+
+size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+template <bool kDense>
+int launch_decode(const void *q, const void *k_cache, const void *v_cache, const int32_t *page_table,
+                  const int32_t *seq_lens, const int32_t *sel_pages, int32_t max_sel, const int32_t *sel_count,
+                  void *out, float *lse, float sm_scale, void *workspace, size_t workspace_bytes,
+                  const sparrow_shape_t *s, cudaStream_t st)
+{
+    const DecodeGeom gm = decode_geom(s, kDense ? 0 : max_sel);
+    if (workspace_bytes < gm.bytes_o + gm.bytes_ml) return SPARROW_ERR_WORKSPACE_TOO_SMALL;
+    if (s->n_seq == 0) return SPARROW_OK;
+    float *ws_o = reinterpret_cast<float *>(workspace);
+    float *ws_ml = reinterpret_cast<float *>(reinterpret_cast<uint8_t *>(workspace) + gm.bytes_o);
+
+    static bool attr_done[2] = {false, false};
+    if (!attr_done[kDense]) {
+        cudaError_t e = cudaFuncSetAttribute(decode_kernel<kDense>, cudaFuncAttributeMaxDynamicSharedMemorySize, kDecSmemBytes);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(decode_kernel)");
+        attr_done[kDense] = true;
+    }
+    const float scale_log2 = sm_scale * 1.4426950408889634f;
+    dim3 grid(gm.n_splits, s->n_kv_heads, s->n_seq);
+    decode_kernel<kDense><<<grid, kDecThreads, kDecSmemBytes, st>>>(
+        (const uint16_t *)q, (const uint16_t *)k_cache, (const uint16_t *)v_cache, page_table, seq_lens, sel_pages,
+        max_sel, sel_count, ws_o, ws_ml, gm.chunk, gm.n_splits, scale_log2, s->n_q_heads, s->n_kv_heads,
+        s->max_pages_per_seq);
+    SPARROW_CHECK_LAUNCH("decode_kernel");
+    dim3 mgrid(s->n_q_heads, s->n_seq);
+    merge_kernel<kDense><<<mgrid, kDim, 0, st>>>(ws_o, ws_ml, seq_lens, sel_count, max_sel, (uint16_t *)out, lse,
+                                                  gm.chunk, gm.n_splits, s->n_q_heads, s->n_kv_heads);
+    SPARROW_CHECK_LAUNCH("merge_kernel");
+    return SPARROW_OK;
+}
+
+int summarize_impl(const void *k_cache, void *summaries, const int32_t *page_ids, const int32_t *n_valid,
+                   int64_t n_update, const sparrow_shape_t *s, cudaStream_t st)
+{
+    if (n_update == 0) return SPARROW_OK;
+    const int64_t tiles = n_update * s->n_kv_heads;
+    const int64_t blocks = (tiles + kSumWarps - 1) / kSumWarps;
+    if (blocks > 0x7fffffffLL) return SPARROW_ERR_UNSUPPORTED;
+    summarize_kernel<<<(unsigned)blocks, kSumWarps * 32, 0, st>>>((const uint16_t *)k_cache, (uint16_t *)summaries,
+                                                                 page_ids, n_valid, n_update, s->n_kv_heads);
+    SPARROW_CHECK_LAUNCH("summarize_kernel");
+    return SPARROW_OK;
+}
+
+int select_impl(const void *q, const void *summaries, const int32_t *page_table, const int32_t *seq_lens,
+                const SchedDev &sd, int32_t *sel_pages, int32_t max_sel, int32_t *sel_count, float *scores_dbg,
+                void *workspace, size_t workspace_bytes, const sparrow_shape_t *s, cudaStream_t st)
+{
+    if (workspace_bytes < sparrow_select_workspace_bytes(s)) return SPARROW_ERR_WORKSPACE_TOO_SMALL;
+    if (s->max_pages_per_seq > kSelMaxPages) return SPARROW_ERR_UNSUPPORTED;
+    if (s->n_seq == 0) return SPARROW_OK;
+    int32_t *counters = reinterpret_cast<int32_t *>(workspace);
+    float *scores_ws = reinterpret_cast<float *>(reinterpret_cast<uint8_t *>(workspace) +
+                                                 align256((size_t)s->n_seq * s->n_kv_heads * sizeof(int32_t)));
+    const size_t dyn = (size_t)s->max_pages_per_seq * sizeof(uint32_t);
+    static size_t dyn_set = 0;
+    if (dyn > 48 * 1024 && dyn > dyn_set) {
+        cudaError_t e = cudaFuncSetAttribute(select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(select_kernel)");
+        dyn_set = dyn;
+    }
+    dim3 grid((s->max_pages_per_seq + kSelChunk - 1) / kSelChunk, s->n_kv_heads, s->n_seq);
+    select_kernel<<<grid, kSelThreads, dyn, st>>>((const uint16_t *)q, (const uint16_t *)summaries, page_table, seq_lens,
+                                                  sd, sel_pages, max_sel, sel_count, scores_ws, counters, scores_dbg,
+                                                  s->n_q_heads, s->n_kv_heads, s->max_pages_per_seq);
+    SPARROW_CHECK_LAUNCH("select_kernel");
+    return SPARROW_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int sparrow_version(void) { return 100; }
+int sparrow_last_launch_count(void) { return g_launches; }
+
+const char *sparrow_strerror(int status)
+{
+    switch (status) {
+    case SPARROW_OK: return "ok";
+    case SPARROW_ERR_INVALID_ARG: return "invalid argument (null, negative or misaligned)";
+    case SPARROW_ERR_UNSUPPORTED: return "unsupported shape (need head_dim 128, page_size 16, 1 <= Hq/Hkv <= 8, bf16)";
+    case SPARROW_ERR_WORKSPACE_TOO_SMALL: return "workspace too small";
+    case SPARROW_ERR_CUDA: return g_errbuf[0] ? g_errbuf : "CUDA error";
+    default: return "unknown status";
+    }
+}
+
+size_t sparrow_select_workspace_bytes(const sparrow_shape_t *s)
+{
+    if (check_shape(s) != SPARROW_OK) return 0;
+    const size_t units = (size_t)s->n_seq * s->n_kv_heads;
+    return align256(units * sizeof(int32_t)) + align256(units * s->max_pages_per_seq * sizeof(float));
+}
+
+size_t sparrow_decode_workspace_bytes(const sparrow_shape_t *s, int32_t max_sel)
+{
+    if (check_shape(s) != SPARROW_OK) return 0;
+    const DecodeGeom gm = decode_geom(s, max_sel);
+    return gm.bytes_o + gm.bytes_ml;
+}
+
+int64_t sparrow_budget_tokens(const sparrow_schedule_t *sched, int64_t L)
+{
+    SchedDev sd;
+    if (to_dev_sched(sched, &sd) != SPARROW_OK || L < 0) return -1;
+    return budget_tokens(sd, L);
+}
+int32_t sparrow_k_pages(const sparrow_schedule_t *sched, int64_t L)
+{
+    SchedDev sd;
+    if (to_dev_sched(sched, &sd) != SPARROW_OK || L < 1) return -1;
+    return make_plan(sd, L).k_pages;
+}
+int32_t sparrow_forced_count(const sparrow_schedule_t *sched, int64_t L)
+{
+    SchedDev sd;
+    if (to_dev_sched(sched, &sd) != SPARROW_OK || L < 1) return -1;
+    return make_plan(sd, L).n_forced;
+}
+int32_t sparrow_sel_count(const sparrow_schedule_t *sched, int64_t L)
+{
+    SchedDev sd;
+    if (to_dev_sched(sched, &sd) != SPARROW_OK || L < 1) return -1;
+    return make_plan(sd, L).count;
+}
+int32_t sparrow_max_sel_pages(const sparrow_schedule_t *sched, int64_t max_len)
+{
+    SchedDev sd;
+    if (to_dev_sched(sched, &sd) != SPARROW_OK || max_len < 1) return -1;
+    int32_t best = 0;      // B(L) need not be monotone (R15): scan every length (host only, ~1e5 evaluations at most)
+    for (int64_t L = 1; L <= max_len; ++L) {
+        const int32_t c = make_plan(sd, L).count;
+        if (c > best) best = c;
+    }
+    return best;
+}
+
+int sparrow_summarize(const void *k_cache, void *summaries, const int32_t *page_ids, const int32_t *n_valid,
+                      int64_t n_update, const sparrow_shape_t *shape, void *stream)
+{
+    g_launches = 0;
+    int rc = check_shape(shape);
+    if (rc) return rc;
+    if (n_update < 0 || (!page_ids && n_update > shape->n_phys_pages)) return SPARROW_ERR_INVALID_ARG;
+    if (n_update == 0) return SPARROW_OK;
+    if (!k_cache || !summaries || !aligned16(k_cache) || !aligned16(summaries)) return SPARROW_ERR_INVALID_ARG;
+    return summarize_impl(k_cache, summaries, page_ids, n_valid, n_update, shape, (cudaStream_t)stream);
+}
+
+int sparrow_select(const void *q, const void *summaries, const int32_t *page_table, const int32_t *seq_lens,
+                   const sparrow_schedule_t *sched, int32_t *sel_pages, int32_t max_sel, int32_t *sel_count,
+                   float *scores_dbg, void *workspace, size_t workspace_bytes, const sparrow_shape_t *shape, void *stream)
+{
+    g_launches = 0;
+    int rc = check_shape(shape);
+    if (rc) return rc;
+    SchedDev sd;
+    rc = to_dev_sched(sched, &sd);
+    if (rc) return rc;
+    if (!q || !summaries || !page_table || !seq_lens || !sel_pages || !sel_count || !workspace || max_sel <= 0)
+        return SPARROW_ERR_INVALID_ARG;
+    if (!aligned16(q) || !aligned16(summaries) || !aligned16(workspace)) return SPARROW_ERR_INVALID_ARG;
+    return select_impl(q, summaries, page_table, seq_lens, sd, sel_pages, max_sel, sel_count, scores_dbg, workspace,
+                       workspace_bytes, shape, (cudaStream_t)stream);
+}
+
+int sparrow_sparse_decode(const void *q, const void *k_cache, const void *v_cache, const int32_t *page_table,
+                          const int32_t *seq_lens, const int32_t *sel_pages, int32_t max_sel, const int32_t *sel_count,
+                          void *out, float *lse, float sm_scale, void *workspace, size_t workspace_bytes,
+                          const sparrow_shape_t *shape, void *stream)
+{
+    g_launches = 0;
+    int rc = check_shape(shape);
+    if (rc) return rc;
+    if (!q || !k_cache || !v_cache || !page_table || !seq_lens || !sel_pages || !sel_count || !out || !workspace || max_sel <= 0)
+        return SPARROW_ERR_INVALID_ARG;
+    if (!aligned16(q) || !aligned16(k_cache) || !aligned16(v_cache) || !aligned16(out) || !aligned16(workspace))
+        return SPARROW_ERR_INVALID_ARG;
+    return launch_decode<false>(q, k_cache, v_cache, page_table, seq_lens, sel_pages, max_sel, sel_count, out, lse,
+                                sm_scale, workspace, workspace_bytes, shape, (cudaStream_t)stream);
+}
+
+int sparrow_dense_decode(const void *q, const void *k_cache, const void *v_cache, const int32_t *page_table,
+                         const int32_t *seq_lens, void *out, float *lse, float sm_scale, void *workspace,
+                         size_t workspace_bytes, const sparrow_shape_t *shape, void *stream)
+{
+    g_launches = 0;
+    int rc = check_shape(shape);
+    if (rc) return rc;
+    if (!q || !k_cache || !v_cache || !page_table || !seq_lens || !out || !workspace) return SPARROW_ERR_INVALID_ARG;
+    if (!aligned16(q) || !aligned16(k_cache) || !aligned16(v_cache) || !aligned16(out) || !aligned16(workspace))
+        return SPARROW_ERR_INVALID_ARG;
+    return launch_decode<true>(q, k_cache, v_cache, page_table, seq_lens, nullptr, 0, nullptr, out, lse, sm_scale,
+                               workspace, workspace_bytes, shape, (cudaStream_t)stream);
+}
+
+// Device scratch of the host-buffer step, carved in this order (each 256-byte aligned):
+//   q | seq_lens | page_ids | n_valid | sel_pages | sel_count | out | select workspace | decode workspace
+namespace {
+struct StepCarve {
+    size_t q, lens, ids, nval, sel, cnt, out, sel_ws, dec_ws, total;
+    size_t sel_ws_bytes, dec_ws_bytes;
+};
+constexpr int64_t kStepMaxUpdates = 4096;     // pages that can fill in one step (<= n_seq in practice)
+StepCarve step_carve(const sparrow_shape_t *s, int32_t max_sel)
+{
+    StepCarve c;
+    size_t o = 0;
+    const size_t n = (size_t)s->n_seq;
+    c.q = o; o += align256(n * s->n_q_heads * kDim * 2);
+    c.lens = o; o += align256(n * 4);
+    c.ids = o; o += align256(kStepMaxUpdates * 4);
+    c.nval = o; o += align256(kStepMaxUpdates * 4);
+    c.sel = o; o += align256(n * s->n_kv_heads * (size_t)(max_sel > 0 ? max_sel : 1) * 4);
+    c.cnt = o; o += align256(n * 4);
+    c.out = o; o += align256(n * s->n_q_heads * kDim * 2);
+    c.sel_ws_bytes = sparrow_select_workspace_bytes(s);
+    c.sel_ws = o; o += c.sel_ws_bytes;
+    const size_t d1 = sparrow_decode_workspace_bytes(s, max_sel), d0 = sparrow_decode_workspace_bytes(s, 0);
+    c.dec_ws_bytes = d1 > d0 ? d1 : d0;
+    c.dec_ws = o; o += c.dec_ws_bytes;
+    c.total = o;
+    return c;
+}
+}  // namespace
+
+size_t sparrow_step_scratch_bytes(const sparrow_shape_t *s, int32_t max_sel)
+{
+    if (check_shape(s) != SPARROW_OK) return 0;
+    return step_carve(s, max_sel).total;
+}
+
+int sparrow_step_host(const void *q_host, const int32_t *seq_lens_host, const int32_t *page_ids_host,
+                      const int32_t *n_valid_host, int64_t n_update, const void *k_cache, const void *v_cache,
+                      void *summaries, const int32_t *page_table, const sparrow_schedule_t *sched, int32_t max_sel,
+                      float sm_scale, void *out_host, void *scratch, size_t scratch_bytes, const sparrow_shape_t *s,
+                      void *stream)
+{
+    g_launches = 0;
+    int rc = check_shape(s);
+    if (rc) return rc;
+    SchedDev sd;
+    rc = to_dev_sched(sched, &sd);
+    if (rc) return rc;
+    if (!q_host || !seq_lens_host || !k_cache || !v_cache || !summaries || !page_table || !out_host || !scratch || max_sel <= 0)
+        return SPARROW_ERR_INVALID_ARG;
+    if (n_update < 0 || n_update > kStepMaxUpdates || (n_update > 0 && !page_ids_host)) return SPARROW_ERR_INVALID_ARG;
+    if (!aligned16(k_cache) || !aligned16(v_cache) || !aligned16(summaries) || !aligned16(scratch)) return SPARROW_ERR_INVALID_ARG;
+    const StepCarve c = step_carve(s, max_sel);
+    if (scratch_bytes < c.total) return SPARROW_ERR_WORKSPACE_TOO_SMALL;
+    cudaStream_t st = (cudaStream_t)stream;
+    uint8_t *base = reinterpret_cast<uint8_t *>(scratch);
+    const size_t qbytes = (size_t)s->n_seq * s->n_q_heads * kDim * 2;
+    cudaError_t e;
+    if ((e = cudaMemcpyAsync(base + c.q, q_host, qbytes, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(e, "H2D q");
+    if ((e = cudaMemcpyAsync(base + c.lens, seq_lens_host, (size_t)s->n_seq * 4, cudaMemcpyHostToDevice, st)) != cudaSuccess)
+        return cuda_fail(e, "H2D seq_lens");
+    const int32_t *lens_d = reinterpret_cast<const int32_t *>(base + c.lens);
+    if (n_update > 0) {
+        if ((e = cudaMemcpyAsync(base + c.ids, page_ids_host, (size_t)n_update * 4, cudaMemcpyHostToDevice, st)) != cudaSuccess)
+            return cuda_fail(e, "H2D page_ids");
+        const int32_t *nv_d = nullptr;
+        if (n_valid_host) {
+            if ((e = cudaMemcpyAsync(base + c.nval, n_valid_host, (size_t)n_update * 4, cudaMemcpyHostToDevice, st)) != cudaSuccess)
+                return cuda_fail(e, "H2D n_valid");
+            nv_d = reinterpret_cast<const int32_t *>(base + c.nval);
+        }
+        rc = summarize_impl(k_cache, summaries, reinterpret_cast<const int32_t *>(base + c.ids), nv_d, n_update, s, st);
+        if (rc) return rc;
+    }
+    if (sd.kind == SPARROW_SCHED_DENSE) {
+        rc = launch_decode<true>(base + c.q, k_cache, v_cache, page_table, lens_d, nullptr, 0, nullptr, base + c.out, nullptr,
+                                 sm_scale, base + c.dec_ws, c.dec_ws_bytes, s, st);
+    } else {
+        rc = select_impl(base + c.q, summaries, page_table, lens_d, sd, reinterpret_cast<int32_t *>(base + c.sel), max_sel,
+                         reinterpret_cast<int32_t *>(base + c.cnt), nullptr, base + c.sel_ws, c.sel_ws_bytes, s, st);
+        if (rc) return rc;
+        rc = launch_decode<false>(base + c.q, k_cache, v_cache, page_table, lens_d, reinterpret_cast<int32_t *>(base + c.sel),
+                                  max_sel, reinterpret_cast<int32_t *>(base + c.cnt), base + c.out, nullptr, sm_scale,
+                                  base + c.dec_ws, c.dec_ws_bytes, s, st);
+    }
+    if (rc) return rc;
+    if ((e = cudaMemcpyAsync(out_host, base + c.out, qbytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e, "D2H out");
+    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e, "stream sync");
+    return SPARROW_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,112 @@
+// common.cuh -- shared device/host helpers of libsparrow_b200 (sm_100a only).
+// Schedule arithmetic (a2, a3 of SURVEY.md 8(a); readings R2-R9, R13 of DESIGN.md) is written here once for the
+// library (host helpers and kernels both use it); the CPU oracle has its own, independent statement.
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/sparrow.h"
+
+namespace sparrow {
+
+constexpr int kPage = 16;          // tokens per page
+constexpr int kDim = 128;          // head dim
+constexpr int kTileElems = kPage * kDim;        // one (page, kv-head) K or V tile: 2048 bf16 = 4 KiB
+constexpr int kTileBytes = kTileElems * 2;
+constexpr int kSumElems = 2 * kDim;             // one (page, kv-head) summary: min[128] + max[128] = 512 B
+
+// Schedule passed to kernels by value (no device memory, graph-capturable).
+struct SchedDev {
+    int32_t kind, sink_tokens, local_tokens, table_len, bin_tokens;
+    int64_t fixed_tokens, floor_tokens, f0_ppm, f1_ppm, L0, L1;
+    int32_t table[SPARROW_MAX_TABLE_BINS];
+};
+
+__host__ __device__ inline int64_t ceil_div64(int64_t a, int64_t b) { return (a + b - 1) / b; }
+
+// a2: B(L) in tokens, exact integers (R3).
+__host__ __device__ inline int64_t budget_tokens(const SchedDev &s, int64_t L)
+{
+    int64_t B;
+    switch (s.kind) {
+    case SPARROW_SCHED_DENSE: B = L; break;
+    case SPARROW_SCHED_FIXED: B = s.fixed_tokens; break;
+    case SPARROW_SCHED_CLAMP_FRAC:
+        B = (int64_t)(((__int128)L * s.f0_ppm) / 1000000);
+        if (B < s.floor_tokens) B = s.floor_tokens;
+        break;
+    case SPARROW_SCHED_LINEAR_FRAC: {
+        int64_t Lc = L < s.L0 ? s.L0 : (L > s.L1 ? s.L1 : L);
+        int64_t span = s.L1 - s.L0;
+        __int128 num = (__int128)s.f0_ppm * span - (__int128)(s.f0_ppm - s.f1_ppm) * (Lc - s.L0);
+        __int128 den = (__int128)1000000 * span;
+        B = (int64_t)(((__int128)L * num) / den);
+        if (B < s.floor_tokens) B = s.floor_tokens;
+        break;
+    }
+    default: {  // TABLE: pages per length bin, B = pagesize x num_pages
+        int64_t b = (L - 1) / s.bin_tokens;
+        if (b < 0) b = 0;
+        if (b >= s.table_len) b = s.table_len - 1;
+        B = (int64_t)s.table[b] * kPage;
+        break;
+    }
+    }
+    return B > L ? L : B;
+}
+
+// Everything the selector needs to know about one sequence (a2 + a3).
+struct SeqPlan {
+    int32_t L, n_pages, k_pages;
+    int32_t n_sink;      // sink pages are [0, n_sink)
+    int32_t tail0;       // local-window pages + last page are [tail0, n_pages)
+    int32_t n_forced;    // |F|
+    int32_t k;           // candidates to pick = max(0, K_pages - |F|)   (R2)
+    int32_t count;       // pages attended = n_pages if dense else max(K_pages, |F|)
+    bool dense;          // K_pages >= n_pages (R13)
+    __host__ __device__ bool forced(int p) const { return p < n_sink || p >= tail0; }
+};
+
+__host__ __device__ inline SeqPlan make_plan(const SchedDev &s, int64_t L)
+{
+    SeqPlan pl;
+    pl.L = (int32_t)L;
+    pl.n_pages = (int32_t)ceil_div64(L, kPage);
+    int64_t kp = ceil_div64(budget_tokens(s, L), kPage);                 // R4: ceil
+    pl.k_pages = (int32_t)(kp < pl.n_pages ? kp : pl.n_pages);
+    int32_t ns = (int32_t)ceil_div64(s.sink_tokens, kPage);              // R8
+    pl.n_sink = ns < pl.n_pages ? ns : pl.n_pages;
+    int32_t t0 = pl.n_pages - 1;                                         // last page always kept (R9)
+    if (s.local_tokens > 0) {
+        int64_t lo = L - s.local_tokens;
+        if (lo < 0) lo = 0;
+        int32_t fl = (int32_t)(lo / kPage);                              // R7: every page overlapping the window
+        if (fl < t0) t0 = fl;
+    }
+    if (t0 < 0) t0 = 0;
+    pl.tail0 = t0;
+    int32_t tail_from = t0 > pl.n_sink ? t0 : pl.n_sink;
+    pl.n_forced = pl.n_sink + (pl.n_pages - tail_from);
+    pl.dense = pl.k_pages >= pl.n_pages;
+    int32_t k = pl.k_pages - pl.n_forced;
+    pl.k = k > 0 ? k : 0;
+    pl.count = pl.dense ? pl.n_pages : (pl.k_pages > pl.n_forced ? pl.k_pages : pl.n_forced);
+    return pl;
+}
+
+// ---------------------------------------------------------------- small device helpers ----
+__device__ __forceinline__ float bf16_lo(uint32_t x) { return __uint_as_float(x << 16); }
+__device__ __forceinline__ float bf16_hi(uint32_t x) { return __uint_as_float(x & 0xffff0000u); }
+
+__device__ __forceinline__ uint4 ldg_stream16(const void *p)
+{
+    uint4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+    return r;
+}
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+}  // namespace sparrow

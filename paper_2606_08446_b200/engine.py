@@ -1,0 +1,80 @@
+"""Buffer owner + call sequencer for one batch: summarize -> select -> sparse decode (or dense decode).
+
+This is plumbing only: it allocates device buffers with torch and calls the C ABI through ``binding``;
+every step of the path runs in the CUDA kernels.  Importing it without the built library fails loudly.
+"""
+from __future__ import annotations
+
+from typing import Optional
+
+import torch
+
+from . import binding as B
+from .workloads import PAGE, Workload, full_page_updates
+
+
+class SparrowEngine:
+    def __init__(self, wl: Workload, schedule: Optional[dict] = None, want_scores: bool = False):
+        assert wl.q.is_cuda, "the engine needs the workload on a CUDA device (no CPU fallback)"
+        self.wl = wl
+        dev = wl.q.device
+        self.shape = B.make_shape(wl.n_seq, wl.Hq, wl.Hkv, wl.max_pages, wl.n_phys)
+        self.set_schedule(schedule or wl.schedule)
+        self.summaries = torch.zeros((wl.n_phys, wl.Hkv, 2, 128), dtype=torch.bfloat16, device=dev)
+        self.sel_count = torch.zeros((wl.n_seq,), dtype=torch.int32, device=dev)
+        self.out = torch.zeros((wl.n_seq, wl.Hq, 128), dtype=torch.bfloat16, device=dev)
+        self.lse = torch.zeros((wl.n_seq, wl.Hq), dtype=torch.float32, device=dev)
+        self.out_dense = torch.zeros_like(self.out)
+        self.lse_dense = torch.zeros_like(self.lse)
+        self.select_ws = torch.zeros((B.sparrow_select_workspace_bytes(self.shape),), dtype=torch.uint8, device=dev)
+        self.scores = (torch.full((wl.n_seq, wl.Hkv, wl.max_pages), float("nan"), dtype=torch.float32, device=dev)
+                       if want_scores else None)
+        self.dense_ws = torch.empty((B.sparrow_decode_workspace_bytes(self.shape, 0),), dtype=torch.uint8, device=dev)
+
+    def set_schedule(self, spec: dict):
+        dev = self.wl.q.device
+        self.sched_spec = dict(spec)
+        self.sched = B.make_schedule(spec)
+        max_len = int(self.wl.seq_lens.max().item())
+        self.max_sel = max(1, B.sparrow_max_sel_pages(self.sched, max_len))
+        self.sel_pages = torch.full((self.wl.n_seq, self.wl.Hkv, self.max_sel), -1, dtype=torch.int32, device=dev)
+        self.sparse_ws = torch.empty((B.sparrow_decode_workspace_bytes(self.shape, self.max_sel),), dtype=torch.uint8, device=dev)
+
+    # ---- a1
+    def summarize(self, page_ids: Optional[torch.Tensor], n_valid: Optional[torch.Tensor], n_update: Optional[int] = None, stream=None):
+        n = int(page_ids.numel()) if page_ids is not None else int(n_update)
+        return B.sparrow_summarize(self.wl.k_cache, self.summaries, page_ids, n_valid, n, self.shape, stream)
+
+    def summarize_all(self, stream=None):
+        """Post-prefill bulk call over every page the batch owns (partial last pages use n_valid)."""
+        ids, nv = full_page_updates(self.wl)
+        dev = self.wl.q.device
+        self._ids, self._nv = ids.to(dev), nv.to(dev)
+        return self.summarize(self._ids, self._nv, stream=stream)
+
+    # ---- a2-a5
+    def select(self, q=None, stream=None):
+        wl = self.wl
+        return B.sparrow_select(wl.q if q is None else q, self.summaries, wl.page_table, wl.seq_lens, self.sched,
+                                self.sel_pages, self.max_sel, self.sel_count, self.scores, self.select_ws, self.shape, stream)
+
+    # ---- a6-a7
+    def sparse_decode(self, q=None, stream=None):
+        wl = self.wl
+        return B.sparrow_sparse_decode(wl.q if q is None else q, wl.k_cache, wl.v_cache, wl.page_table, wl.seq_lens,
+                                       self.sel_pages, self.max_sel, self.sel_count, self.out, self.lse, wl.sm_scale,
+                                       self.sparse_ws, self.shape, stream)
+
+    # ---- a8
+    def dense_decode(self, q=None, stream=None):
+        wl = self.wl
+        return B.sparrow_dense_decode(wl.q if q is None else q, wl.k_cache, wl.v_cache, wl.page_table, wl.seq_lens,
+                                      self.out_dense, self.lse_dense, wl.sm_scale, self.dense_ws, self.shape, stream)
+
+    def step(self, q=None, updates=None, stream=None):
+        """One pass of the hot path: summarize the pages that just filled, select, sparse decode."""
+        if updates is not None and updates[0].numel() > 0:
+            self.summarize(updates[0], updates[1], stream=stream)
+        self.select(q, stream)
+        self.sparse_decode(q, stream)
+        return self.out

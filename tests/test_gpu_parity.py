@@ -1,0 +1,210 @@
+"""GPU parity tests (``-m gpu``): the CUDA library, called through the C ABI binding, against the fp64 oracle,
+element by element on the same seeded inputs.  Sizes span several tiles / chunks and ragged tails; the
+full-size BASELINE.json configs are checked on sampled sequences in the launch configuration bench.py times."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2606_08446_b200 import workloads as W
+
+from parity_util import check_dense, check_sparse_step, check_summaries, check_outputs, sub_host
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+
+
+def _engine(wl, **kw):
+    from paper_2606_08446_b200.engine import SparrowEngine
+    eng = SparrowEngine(wl, **kw)
+    eng.summarize_all()
+    return eng
+
+
+def _run_sparse(wl, **kw):
+    eng = _engine(wl, **kw)
+    eng.select()
+    eng.sparse_decode()
+    torch.cuda.synchronize()
+    return eng
+
+
+def test_library_loaded_is_in_tree():
+    from paper_2606_08446_b200 import binding as B
+    assert B.LIB_PATH.endswith("paper_2606_08446_b200/libsparrow_b200.so") and B.sparrow_version() >= 100
+
+
+def test_cfg1_sparse_matches_oracle():
+    wl = W.make_config("cfg1", device=DEV)
+    eng = _run_sparse(wl, want_scores=True)
+    st = check_sparse_step(eng, wl)
+    assert eng.sel_count.tolist() == [16, 16]
+    assert st["units"] == 4
+
+
+def test_cfg1_budget_covers_context_equals_dense():
+    wl = W.make_config("cfg1_dense", device=DEV)
+    eng = _run_sparse(wl)
+    st = check_sparse_step(eng, wl)
+    assert eng.sel_count.tolist() == [64, 94] and st["differing_units"] == 0
+    eng.dense_decode()
+    torch.cuda.synchronize()
+    check_dense(eng, wl)
+    # sparse entry with B >= L vs dense entry: same tolerances (bitwise equality not required)
+    assert (eng.out.float() - eng.out_dense.float()).abs().max().item() <= 2e-2
+    assert (eng.lse - eng.lse_dense).abs().max().item() <= 1e-3
+
+
+@pytest.mark.parametrize("Hq,Hkv", [(2, 2), (4, 2), (8, 2), (5, 1), (16, 2), (40, 8)])
+def test_ragged_lengths_all_group_sizes(Hq, Hkv):
+    lens = [1, 15, 16, 17, 33, 250, 256, 257, 1000, 2049, 4099]
+    sched = W._sched("fixed", 16, 64, fixed_tokens=200)
+    wl = W.make_workload(n_seq=len(lens), Hq=Hq, Hkv=Hkv, lengths=("list", lens), schedule=sched, seed=Hq * 100 + Hkv,
+                         device=DEV, poison_tail=True, plant=True)
+    eng = _run_sparse(wl, want_scores=True)
+    check_sparse_step(eng, wl)
+    eng.dense_decode()
+    torch.cuda.synchronize()
+    check_dense(eng, wl)
+
+
+@pytest.mark.parametrize("sched", [
+    W._sched("clamp_frac", 64, 512, f0_ppm=125000, floor_tokens=2048),
+    W._sched("linear_frac", 64, 512, f0_ppm=250000, f1_ppm=62500, L0=8192, L1=32768, floor_tokens=2048),
+    W._sched("clamp_frac", 0, 0, f0_ppm=50000, floor_tokens=64),
+    W._sched("table", 32, 100, table_pages=(8, 20, 40, 50, 64, 70), bin_tokens=2048),
+    W._sched("fixed", 700, 900, fixed_tokens=64),      # forced pages exceed the budget: k = 0 (R2)
+    W._sched("dense", 0, 0),
+], ids=["cfg2-clamp", "cfg3-linear", "nosink-nolocal", "table-2k-bins", "forced-exceed-budget", "dense-kind"])
+def test_schedules_medium_batch(sched):
+    # lengths span one to ~44 select chunks (256 pages) and many decode splits, with ragged tails
+    lens = [300, 2047, 2048, 2049, 4096, 5000, 8191, 9001, 11111, 700, 16, 6143]
+    wl = W.make_workload(n_seq=len(lens), Hq=8, Hkv=2, lengths=("list", lens), schedule=sched, seed=77, device=DEV, plant=True)
+    eng = _run_sparse(wl, want_scores=True)
+    check_sparse_step(eng, wl)
+
+
+def test_all_ties_zero_query_picks_lowest_pages():
+    lens = [1200, 640, 5000]
+    sched = W._sched("fixed", 16, 32, fixed_tokens=320)
+    wl = W.make_workload(n_seq=3, Hq=4, Hkv=2, lengths=("list", lens), schedule=sched, seed=5, device=DEV)
+    wl.q.zero_()
+    eng = _run_sparse(wl)
+    st = check_sparse_step(eng, wl)
+    assert st["differing_units"] == 0       # exact ties resolve to the lower page index on both sides
+    assert eng.sel_pages[0, 0, :20].tolist() == list(range(18)) + [73, 74]   # F = {0, 73, 74}, k = 17
+
+
+def test_summarize_bulk_identity_and_partial_pages():
+    from paper_2606_08446_b200.engine import SparrowEngine
+    wl = W.make_workload(n_seq=3, Hq=4, Hkv=4, lengths=("list", [100, 37, 513]), schedule=W._sched("dense", 0, 0), seed=9, device=DEV)
+    h = wl.host()
+    eng = SparrowEngine(wl)
+    eng.summarize(None, None, n_update=wl.n_phys)            # page_ids = NULL: pages 0..n-1, all 16 tokens
+    torch.cuda.synchronize()
+    check_summaries(eng.summaries, h, np.arange(wl.n_phys), None)
+    ids = torch.tensor([5, 0, 7], dtype=torch.int32, device=DEV)
+    nv = torch.tensor([1, 9, 16], dtype=torch.int32, device=DEV)
+    eng.summarize(ids, nv)
+    torch.cuda.synchronize()
+    check_summaries(eng.summaries, h, ids.cpu().numpy(), nv.cpu().numpy())
+
+
+def test_select_is_repeatable_and_graph_capturable():
+    wl = W.make_workload(n_seq=6, Hq=8, Hkv=4, lengths=("list", [3000, 4000, 513, 9000, 77, 2500]),
+                         schedule=W._sched("fixed", 64, 256, fixed_tokens=1024), seed=3, device=DEV, plant=True)
+    eng = _run_sparse(wl)
+    ref_sel, ref_out = eng.sel_pages.clone(), eng.out.clone()
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        eng.sel_pages.fill_(-1); eng.out.zero_()
+        eng.step(stream=st)                                   # warm-up on the capture stream
+        st.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=st):
+            eng.step(stream=st)
+        for _ in range(3):
+            eng.sel_pages.fill_(-1); eng.out.zero_()
+            g.replay()
+    st.synchronize()
+    torch.cuda.synchronize()
+    assert torch.equal(eng.sel_pages, ref_sel) and torch.equal(eng.out, ref_out)
+    check_sparse_step(eng, wl)
+
+
+def test_step_host_entry_matches_device_path():
+    from paper_2606_08446_b200 import binding as B
+    wl = W.make_workload(n_seq=5, Hq=8, Hkv=2, lengths=("list", [2048, 4000, 160, 3333, 4096]),
+                         schedule=W._sched("clamp_frac", 64, 256, f0_ppm=125000, floor_tokens=512), seed=13, device=DEV, plant=True)
+    eng = _run_sparse(wl)
+    ids, nv = W.just_filled_updates(wl)
+    assert ids.numel() == 3
+    scratch = torch.zeros((B.sparrow_step_scratch_bytes(eng.shape, eng.max_sel),), dtype=torch.uint8, device=DEV)
+    q_h = wl.q.cpu().pin_memory(); lens_h = wl.seq_lens.cpu().pin_memory()
+    out_h = torch.zeros_like(q_h).pin_memory()
+    eng.summaries[ids.long().to(DEV)] = 0                     # the step must rebuild the summaries of just-filled pages
+    B.sparrow_step_host(q_h, lens_h, ids, nv, ids.numel(), wl.k_cache, wl.v_cache, eng.summaries, wl.page_table,
+                        eng.sched, eng.max_sel, wl.sm_scale, out_h, scratch, eng.shape)
+    assert B.sparrow_last_launch_count() == 4                 # summarize, select, decode, merge
+    assert torch.equal(out_h, eng.out.cpu())
+    check_summaries(eng.summaries, wl.host(), ids.numpy(), nv.numpy())
+
+
+def test_error_statuses_on_device_calls():
+    from paper_2606_08446_b200 import binding as B
+    wl = W.make_config("cfg1", device=DEV)
+    eng = _engine(wl)
+    small = torch.empty((16,), dtype=torch.uint8, device=DEV)
+    rc = B.sparrow_sparse_decode(wl.q, wl.k_cache, wl.v_cache, wl.page_table, wl.seq_lens, eng.sel_pages, eng.max_sel,
+                                 eng.sel_count, eng.out, eng.lse, wl.sm_scale, small, eng.shape, check=False)
+    assert rc == -3
+    q_mis = torch.empty((wl.q.numel() + 8,), dtype=torch.bfloat16, device=DEV)[1:1 + wl.q.numel()].view_as(wl.q)
+    assert q_mis.is_contiguous() and q_mis.data_ptr() % 16 != 0
+    rc = B.sparrow_select(q_mis, eng.summaries, wl.page_table, wl.seq_lens, eng.sched, eng.sel_pages, eng.max_sel,
+                          eng.sel_count, None, eng.select_ws, eng.shape, check=False)
+    assert rc == -1                                            # misaligned device pointer
+    with pytest.raises(B.SparrowError):
+        B.sparrow_dense_decode(wl.q, wl.k_cache, wl.v_cache, wl.page_table, wl.seq_lens, eng.out_dense, eng.lse_dense,
+                               wl.sm_scale, small, eng.shape)
+
+
+# ------------------------------------------------------------------ full-size BASELINE.json configs (sampled) ----
+@pytest.mark.parametrize("cfg,n_sample", [("cfg2", 6), ("cfg5", 3), ("cfg3", 3)])
+def test_full_size_config_sampled_against_oracle(cfg, n_sample):
+    wl = W.make_config(cfg, device=DEV)
+    eng = _run_sparse(wl, want_scores=True)
+    eng.dense_decode()
+    torch.cuda.synchronize()
+    h = wl.host()
+    lens = h["seq_lens"]
+    # sample: the shortest, the longest and a few seeded others
+    rng = np.random.default_rng(1)
+    idx = sorted(set([int(lens.argmin()), int(lens.argmax())] + rng.choice(wl.n_seq, n_sample, replace=False).tolist()))[: n_sample + 2]
+    st = check_sparse_step(eng, wl, h=h, idx=idx)
+    sd = check_dense(eng, wl, h=h, idx=idx[:2])
+    print(f"{cfg}: sampled seqs {idx}: {st}; dense {sd}")
+    # properties that hold at any size, on ALL sequences
+    sched = oracle.Schedule.from_spec(wl.schedule)
+    cnt = eng.sel_count.cpu().numpy()
+    sel = eng.sel_pages.cpu().numpy()
+    for i in range(wl.n_seq):
+        L = int(lens[i]); n_pages = -(-L // 16)
+        K = oracle.k_pages(sched, L)
+        F = np.flatnonzero(oracle.forced_pages(L, sched.sink_tokens, sched.local_tokens))
+        assert cnt[i] == (n_pages if K >= n_pages else max(K, len(F)))
+        for g in range(wl.Hkv):
+            row = sel[i, g, :cnt[i]]
+            assert (np.diff(row) > 0).all() and row[0] >= 0 and row[-1] < n_pages and np.isin(F, row).all()
+    assert torch.isfinite(eng.out.float()).all() and torch.isfinite(eng.lse).all()
+    # planted pages that are candidates are (almost all) recovered: the selector is meaningful on this workload
+    rec, tot = 0, 0
+    for i in idx:
+        L = int(lens[i]); n_pages = -(-L // 16)
+        F = set(np.flatnonzero(oracle.forced_pages(L, sched.sink_tokens, sched.local_tokens)).tolist())
+        k = cnt[i] - len(F)
+        for g in range(wl.Hkv):
+            row = set(sel[i, g, :cnt[i]].tolist())
+            pl = [p for p in wl.planted[i][g].tolist() if p not in F]
+            rec += sum(p in row for p in pl); tot += min(len(pl), k)
+    print(f"{cfg}: planted candidates recovered {rec}/{tot}")
+    assert rec >= 0.8 * tot
