@@ -138,7 +138,7 @@ def test_step_host_entry_matches_device_path():
                          schedule=W._sched("clamp_frac", 64, 256, f0_ppm=125000, floor_tokens=512), seed=13, device=DEV, plant=True)
     eng = _run_sparse(wl)
     ids, nv = W.just_filled_updates(wl)
-    assert ids.numel() == 3
+    assert ids.numel() == 4
     scratch = torch.zeros((B.sparrow_step_scratch_bytes(eng.shape, eng.max_sel),), dtype=torch.uint8, device=DEV)
     q_h = wl.q.cpu().pin_memory(); lens_h = wl.seq_lens.cpu().pin_memory()
     out_h = torch.zeros_like(q_h).pin_memory()
