@@ -1,0 +1,335 @@
+#!/usr/bin/env python
+"""bench.py -- sparse decode-attention throughput of libsparrow_b200 on synthetic Qwen3-shaped rollouts.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg2] [--impl sparrow|reference]
+
+A "step" is one pass of the whole hot path over one batch: summarize the pages that just filled
+-> fused score + top-k select -> split-K sparse decode + LSE merge.  Inputs are resident in HBM when the timed
+region starts (`value`); `e2e` repeats the measurement through the host-buffer C-ABI entry (sparrow_step_host) with
+the H2D / D2H copies inside the timed region.  One JSON line is printed by rank 0.  N > 1: replicas only, no
+data-path collective (each rank its own batch and page pool; weak scaling).
+
+`--impl reference` times the fp64 CPU oracle (as it stands, on the host cores) on a bounded sample of the same
+workload: it is a deliberately slow checker, a reported baseline and not the target.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+import torch  # noqa: E402
+
+from paper_2606_08446_b200 import dist as D  # noqa: E402
+from paper_2606_08446_b200 import workloads as W  # noqa: E402
+
+METRIC = "sparse decode-attn tokens/s"
+UNIT = "tokens/s"
+KV_TILE_BYTES = 2 * 16 * 128 * 2        # K + V of one (page, kv-head): 8 KiB
+SUMMARY_BYTES = 2 * 128 * 2             # min + max of one (page, kv-head): 512 B
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy bandwidth)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "50"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.06)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 6:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def algorithmic_bytes(wl, eng, lens, cnt):
+    """Bytes the method itself must move per step: selected K/V tiles, candidate summaries,
+    page-table / index traffic, q / out.  Returned per kernel."""
+    n_pages = -(-lens // 16)
+    forced = np.array([W_forced(eng, int(L)) for L in lens])
+    dense_seq = cnt >= n_pages
+    cand = np.where(dense_seq, 0, n_pages - forced)
+    qo = wl.n_seq * wl.Hq * 128 * 2
+    decode = int(cnt.sum()) * wl.Hkv * KV_TILE_BYTES + int(cnt.sum()) * wl.Hkv * 4 + int(cnt.sum()) * 4 + 2 * qo
+    select = int(cand.sum()) * wl.Hkv * SUMMARY_BYTES + int(cand.sum()) * 4 + int(cnt.sum()) * wl.Hkv * 4 + qo
+    dense = int(n_pages.sum()) * wl.Hkv * KV_TILE_BYTES + int(n_pages.sum()) * 4 + 2 * qo
+    return dict(decode=decode, select=select, dense=dense, sel_tiles=int(cnt.sum()) * wl.Hkv, cand_tiles=int(cand.sum()) * wl.Hkv)
+
+
+def W_forced(eng, L):
+    from paper_2606_08446_b200 import binding as B
+    return B.sparrow_forced_count(eng.sched, L)
+
+
+def time_oracle_sample(wl, h, budget_s=12.0):
+    """The oracle as it stands on the host cores, on a bounded sample of sequences of the same batch."""
+    import oracle
+    sched = oracle.Schedule.from_spec(wl.schedule)
+    n_try, best = 2, None
+    while True:
+        idx = np.arange(min(n_try, wl.n_seq))
+        t0 = time.perf_counter()
+        oracle.sparse_step(np.ascontiguousarray(h["q"][idx]), h["k_cache"], h["v_cache"], np.ascontiguousarray(h["page_table"][idx]),
+                           np.ascontiguousarray(h["seq_lens"][idx]), sched, wl.sm_scale)
+        dt = time.perf_counter() - t0
+        best = (len(idx), dt)
+        if len(idx) >= wl.n_seq or dt * 2.2 > budget_s:
+            break
+        n_try = min(wl.n_seq, max(n_try + 1, int(n_try * min(4.0, budget_s / max(dt, 1e-3) / 2.2))))
+    return best[0], best[1], oracle.num_threads()
+
+
+def run_reference(args, rank):
+    """--impl reference: the CPU oracle arm (rank 0 only)."""
+    if rank != 0:
+        return
+    import oracle
+    wl = W.make_config(args.workload, device="cuda" if torch.cuda.is_available() else "cpu")
+    h = wl.host()
+    sched = oracle.Schedule.from_spec(wl.schedule)
+    # bounded sample: as many sequences as keep one step near ~1.5 s, so steps+warmup end within a few minutes
+    n_s, dt, cores = time_oracle_sample(wl, h, budget_s=3.0)
+    idx = np.arange(n_s)
+    sub = (np.ascontiguousarray(h["q"][idx]), h["k_cache"], h["v_cache"], np.ascontiguousarray(h["page_table"][idx]),
+           np.ascontiguousarray(h["seq_lens"][idx]))
+    for _ in range(min(args.warmup, 2)):
+        oracle.sparse_step(*sub, sched, wl.sm_scale)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.sparse_step(*sub, sched, wl.sm_scale)
+    dt = (time.perf_counter() - t0) / args.steps
+    val = n_s / dt
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload, "n_seq_sampled": int(n_s), "n_seq": wl.n_seq, "Hq": wl.Hq, "Hkv": wl.Hkv},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": f"first {n_s} of {wl.n_seq} sequences of {args.workload}, full select + sparse attention per step"},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--workload", default="cfg2", choices=[c for c in W.CONFIGS if c != "cfg4"])
+    ap.add_argument("--impl", default="sparrow", choices=["sparrow", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-check", action="store_true", help="skip the sampled oracle self-check before timing")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+
+    rank, local_rank, world = D.env_world()
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device: there is no CPU fallback"
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    D.init("nccl")
+    from paper_2606_08446_b200 import binding as B
+    from paper_2606_08446_b200.engine import SparrowEngine
+
+    base_seed = 1000 * int("".join(ch for ch in args.workload if ch.isdigit()) or 0)
+    wl = W.make_config(args.workload, seed=D.replica_seed(base_seed, rank), device=dev)
+    eng = SparrowEngine(wl)
+    st = torch.cuda.Stream(device=dev)
+    upd = tuple(t.to(dev) for t in W.just_filled_updates(wl))
+    with torch.cuda.stream(st):
+        eng.summarize_all(stream=st)
+        t_sum0, t_sum1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t_sum0.record(st); eng.summarize_all(stream=st); t_sum1.record(st)
+    st.synchronize()
+    bulk_sum_ms = t_sum0.elapsed_time(t_sum1)
+    n_bulk = int(eng._ids.numel())
+
+    lens = wl.seq_lens.cpu().numpy()
+    # ---- correctness gate before timing (rank 0, a few sampled sequences) ----
+    h = None
+    if rank == 0 and not args.no_check:
+        sys.path.insert(0, os.path.join(ROOT, "tests"))
+        from parity_util import check_sparse_step
+        with torch.cuda.stream(st):
+            eng.step(updates=upd, stream=st)
+        st.synchronize()
+        h = wl.host()
+        idx = sorted({int(lens.argmin()), int(lens.argmax()), 0})
+        chk = check_sparse_step(eng, wl, h=h, idx=idx)
+    else:
+        chk = None
+
+    def one_step():
+        n = 0
+        if upd[0].numel() > 0:
+            eng.summarize(upd[0], upd[1], stream=st); n += B.sparrow_last_launch_count()
+        eng.select(stream=st); n += B.sparrow_last_launch_count()
+        return n
+
+    # ---- timed region: K steps, device-resident inputs, events on the launching stream ----
+    K, Wm = args.steps, args.warmup
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(K)]
+    launches = 0
+    with torch.cuda.stream(st):
+        for _ in range(Wm):
+            one_step(); eng.sparse_decode(stream=st)
+        st.synchronize()
+        D.barrier()
+        torch.cuda.synchronize()
+        clocks = ClockSampler(local_rank); clocks.start()
+        for k in range(K):
+            ev[k][0].record(st)
+            launches += one_step()
+            ev[k][1].record(st)
+            eng.sparse_decode(stream=st); launches += B.sparrow_last_launch_count()
+            ev[k][2].record(st)
+        t_end = torch.cuda.Event(enable_timing=True); t_end.record(st)
+        st.synchronize()
+        torch.cuda.synchronize()
+        D.barrier()
+        clk = clocks.stop()
+    total_ms = ev[0][0].elapsed_time(t_end)
+    sel_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in ev]))
+    dec_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in ev]))
+    value, t_max = D.whole_job_throughput(wl.n_seq * K, total_ms * 1e-3, device=dev)
+
+    # ---- dense path of the same library on the same inputs (speedup denominator) ----
+    Kd = max(3, min(K, 10))
+    with torch.cuda.stream(st):
+        for _ in range(2):
+            eng.dense_decode(stream=st)
+        d0, d1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        d0.record(st)
+        for _ in range(Kd):
+            eng.dense_decode(stream=st)
+        d1.record(st)
+    st.synchronize()
+    dense_ms = d0.elapsed_time(d1) / Kd
+
+    # ---- end to end through the host-buffer C-ABI entry (H2D + D2H inside the timed region) ----
+    scratch = torch.zeros((B.sparrow_step_scratch_bytes(eng.shape, eng.max_sel),), dtype=torch.uint8, device=dev)
+    q_h, lens_h = wl.q.cpu().pin_memory(), wl.seq_lens.cpu().pin_memory()
+    ids_h, nv_h = upd[0].cpu().pin_memory(), upd[1].cpu().pin_memory()
+    out_h = torch.empty_like(q_h).pin_memory()
+    n_upd = int(ids_h.numel())
+
+    def host_step():
+        B.sparrow_step_host(q_h, lens_h, ids_h if n_upd else None, nv_h if n_upd else None, n_upd, wl.k_cache, wl.v_cache,
+                            eng.summaries, wl.page_table, eng.sched, eng.max_sel, wl.sm_scale, out_h, scratch, eng.shape, st)
+    for _ in range(Wm):
+        host_step()
+    D.barrier(); torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(st)
+    for _ in range(K):
+        host_step()
+    e1.record(st); st.synchronize()
+    e2e_value, _ = D.whole_job_throughput(wl.n_seq * K, e0.elapsed_time(e1) * 1e-3, device=dev)
+    h2d = int(q_h.numel() * 2 + lens_h.numel() * 4 + n_upd * 8)
+    d2h = int(out_h.numel() * 2)
+    e2e_match = bool(torch.equal(out_h, eng.out.cpu()))
+
+    if rank != 0:
+        return
+    cnt = eng.sel_count.cpu().numpy()
+    ab = algorithmic_bytes(wl, eng, lens, cnt)
+    peak, peak_src = measured_peaks()
+    dec_gbs = ab["decode"] / (dec_ms * 1e-3) / 1e9
+    sel_gbs = ab["select"] / (sel_ms * 1e-3) / 1e9
+    dense_gbs = ab["dense"] / (dense_ms * 1e-3) / 1e9
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    if os.path.exists(tp):
+        traffic = json.load(open(tp)).get(args.workload, {}).get("decode_kernel_bytes_per_launch")
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+        "ms_per_step": t_max * 1e3 / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "bf16", "data": "synthetic",
+        "config": {"workload": args.workload, "n_seq": wl.n_seq, "Hq": wl.Hq, "Hkv": wl.Hkv, "head_dim": 128, "page_size": 16,
+                   "len_min": int(lens.min()), "len_max": int(lens.max()), "schedule": wl.schedule["kind"],
+                   "sink_tokens": wl.schedule["sink_tokens"], "local_tokens": wl.schedule["local_tokens"],
+                   "selected_pages_per_seq_mean": float(cnt.mean()), "parallelism": f"replicas x{world} (no collective)",
+                   "l2": "inputs larger than L2: %.0f MB touched per step vs 126 MB L2" % ((ab["decode"] + ab["select"]) / 1e6)},
+        "roofline": {"bound": "hbm", "kernel": "decode_kernel<sparse> (+ merge_kernel, one sparrow_sparse_decode call)",
+                     "achieved": dec_gbs, "peak": peak, "unit": "GB/s", "frac": dec_gbs / peak, "traffic": traffic,
+                     "peak_source": peak_src, "algorithmic_bytes_per_launch": ab["decode"], "avg_launch_ms": dec_ms,
+                     "frac_of_8TBs_nominal": dec_gbs / 8000.0},
+        "kernels": {"select": {"ms": sel_ms, "algorithmic_bytes": ab["select"], "achieved_GBs": sel_gbs, "frac": sel_gbs / peak},
+                    "sparse_decode": {"ms": dec_ms, "algorithmic_bytes": ab["decode"], "achieved_GBs": dec_gbs, "frac": dec_gbs / peak},
+                    "dense_decode": {"ms": dense_ms, "algorithmic_bytes": ab["dense"], "achieved_GBs": dense_gbs, "frac": dense_gbs / peak},
+                    "bulk_summarize": {"ms": bulk_sum_ms, "pages": n_bulk,
+                                       "achieved_GBs": n_bulk * wl.Hkv * (4096 + 512) / (bulk_sum_ms * 1e-3) / 1e9}},
+        "sparse_path_GBs": (ab["decode"] + ab["select"]) / (t_max / K) / 1e9,
+        "dense_tokens_per_s": wl.n_seq / (dense_ms * 1e-3),
+        "speedup_vs_dense": dense_ms / (t_max * 1e3 / K),
+        "ideal_speedup_bytes_ratio": ab["dense"] / (ab["decode"] + ab["select"]),
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "matches_device_path": e2e_match},
+        "gpu_launches": launches,
+        "clocks": clk,
+        "paper_context": "Sparrow rollout speedups 2.2x/2.4x/2.0x for Qwen3-1.7B/4B/8B on 4xH200 (PAPER.md:7; whole-engine, not this kernel path)",
+    }
+    if chk is not None:
+        line["self_check"] = {"sampled_seqs": len(idx), **{k: chk[k] for k in ("units", "differing_units", "max_abs", "mean_abs", "lse_max_abs")}}
+    if not args.no_cpu_baseline:
+        h = h or wl.host()
+        n_s, dt, cores = time_oracle_sample(wl, h)
+        line["cpu_baseline"] = {"value": n_s / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": f"first {n_s} of {wl.n_seq} sequences of {args.workload}: one full select + sparse-attention step in {dt:.2f} s"}
+    print(json.dumps(line), flush=True)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,41 @@
+"""world_size-2 gloo tests (CPU) of the N>1 plumbing: replicas only, no data-path collective."""
+import os
+
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+from paper_2606_08446_b200 import dist as D
+
+
+def _worker(rank, world, port, q):
+    os.environ.update(RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    r, lr, w = D.init("gloo")
+    assert (r, w) == (rank, world)
+    D.barrier()
+    # rank r "processes" 64 sequences per step for 10 steps in (1 + r) seconds
+    thr, t = D.whole_job_throughput(64 * 10, 1.0 + rank)
+    shard = D.shard_sequences(129, rank, world)
+    q.put((rank, thr, t, D.replica_seed(2000, rank), len(shard), shard[0], shard[-1]))
+    D.barrier()
+    dist.destroy_process_group()
+
+
+def test_two_rank_replicas_aggregate_over_max_time():
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 29500 + os.getpid() % 400
+    ps = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    [p.start() for p in ps]
+    res = sorted(q.get(timeout=120) for _ in range(2))
+    [p.join(timeout=60) for p in ps]
+    assert all(p.exitcode == 0 for p in ps)
+    for rank, thr, t, seed, n, lo, hi in res:
+        assert t == 2.0 and thr == (640 + 640) / 2.0           # whole-job units / max-over-ranks time
+    assert res[0][3] != res[1][3]                               # replicas draw different batches
+    assert (res[0][4], res[0][5], res[0][6]) == (65, 0, 64) and (res[1][4], res[1][5], res[1][6]) == (64, 65, 128)
+
+
+def test_single_process_defaults():
+    assert D.env_world()[2] >= 1
+    assert D.max_over_ranks(3.5) == 3.5 and D.shard_sequences(10, 0, 1) == list(range(10))
