@@ -62,7 +62,8 @@ typedef struct sparrow_shape {
 } sparrow_shape_t;
 
 /* Dynamic sparsity schedule B(L) in EXACT integer arithmetic (R3), so that host, device and any checker
- * agree bit for bit.  Fractions are parts per million.  After the kind-specific value B is clamped to
+ * agree bit for bit.  Fractions are parts per million in [0, 1000000] (L1 - L0 < 2^31); anything else is
+ * SPARROW_ERR_INVALID_ARG.  After the kind-specific value B is clamped to
  * at least floor_tokens (kinds 2, 3) and at most L.  K_pages = min(ceil(B/16), ceil(L/16)) (R4); a
  * sequence with K_pages >= n_pages is dense. */
 enum {

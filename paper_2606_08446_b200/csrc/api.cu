@@ -60,9 +60,12 @@ int to_dev_sched(const sparrow_schedule_t *in, SchedDev *out)
     out->L1 = in->L1;
     out->bin_tokens = in->bin_tokens;
     if (in->kind == SPARROW_SCHED_FIXED && in->fixed_tokens < 0) return SPARROW_ERR_INVALID_ARG;
-    if (in->kind == SPARROW_SCHED_CLAMP_FRAC && (in->f0_ppm < 0 || in->floor_tokens < 0)) return SPARROW_ERR_INVALID_ARG;
+    constexpr int64_t kPpmMax = 1000000;                 // keep fractions are in [0, 1]
+    if (in->kind == SPARROW_SCHED_CLAMP_FRAC && (in->f0_ppm < 0 || in->f0_ppm > kPpmMax || in->floor_tokens < 0))
+        return SPARROW_ERR_INVALID_ARG;
     if (in->kind == SPARROW_SCHED_LINEAR_FRAC &&
-        (in->L1 <= in->L0 || in->f0_ppm < 0 || in->f1_ppm < 0 || in->floor_tokens < 0))
+        (in->L0 < 0 || in->L1 <= in->L0 || in->L1 - in->L0 > 0x7fffffffLL || in->f0_ppm < 0 || in->f0_ppm > kPpmMax ||
+         in->f1_ppm < 0 || in->f1_ppm > kPpmMax || in->floor_tokens < 0))
         return SPARROW_ERR_INVALID_ARG;
     if (in->kind == SPARROW_SCHED_TABLE) {
         if (!in->table_pages || in->table_len <= 0 || in->table_len > SPARROW_MAX_TABLE_BINS || in->bin_tokens <= 0)

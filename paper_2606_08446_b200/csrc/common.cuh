@@ -25,6 +25,20 @@ struct SchedDev {
 
 __host__ __device__ inline int64_t ceil_div64(int64_t a, int64_t b) { return (a + b - 1) / b; }
 
+// floor(a * b / c) for a, b >= 0, c > 0, exact.  A 128-bit division is hundreds of instructions on the GPU, so the
+// quotient is estimated in fp64 (three roundings: off by a few units at most while it is below 2^50) and then fixed
+// with exact 128-bit products; larger quotients (host callers only) take the plain 128-bit division.
+__host__ __device__ inline int64_t muldiv_floor(int64_t a, int64_t b, int64_t c)
+{
+    const __int128 prod = (__int128)a * b;
+    const double est = (double)a * (double)b / (double)c;
+    if (!(est < 1125899906842624.0)) return (int64_t)(prod / c);
+    int64_t qv = (int64_t)est;
+    while ((__int128)qv * c > prod) --qv;
+    while ((__int128)(qv + 1) * c <= prod) ++qv;
+    return qv;
+}
+
 // a2: B(L) in tokens, exact integers (R3).
 __host__ __device__ inline int64_t budget_tokens(const SchedDev &s, int64_t L)
 {
@@ -33,15 +47,16 @@ __host__ __device__ inline int64_t budget_tokens(const SchedDev &s, int64_t L)
     case SPARROW_SCHED_DENSE: B = L; break;
     case SPARROW_SCHED_FIXED: B = s.fixed_tokens; break;
     case SPARROW_SCHED_CLAMP_FRAC:
-        B = (int64_t)(((__int128)L * s.f0_ppm) / 1000000);
+        B = muldiv_floor(L, s.f0_ppm, 1000000);
         if (B < s.floor_tokens) B = s.floor_tokens;
         break;
     case SPARROW_SCHED_LINEAR_FRAC: {
         int64_t Lc = L < s.L0 ? s.L0 : (L > s.L1 ? s.L1 : L);
         int64_t span = s.L1 - s.L0;
-        __int128 num = (__int128)s.f0_ppm * span - (__int128)(s.f0_ppm - s.f1_ppm) * (Lc - s.L0);
-        __int128 den = (__int128)1000000 * span;
-        B = (int64_t)(((__int128)L * num) / den);
+        // validated on entry: 0 <= f <= 1e6 ppm and span < 2^31, so num and den stay below 2^51
+        const int64_t num = s.f0_ppm * span - (s.f0_ppm - s.f1_ppm) * (Lc - s.L0);
+        const int64_t den = 1000000 * span;
+        B = muldiv_floor(L, num, den);
         if (B < s.floor_tokens) B = s.floor_tokens;
         break;
     }

@@ -1,7 +1,7 @@
 // select.cuh -- kernel (b): fused page scoring + per-(sequence, kv-head) top-k page selection.
 // SURVEY.md 8(a) a2-a5; PAPER.md:138-147 ("landmark scores", Top-k), north_star (b).
 //
-// Grid = (page chunks, kv-heads, sequences).  Every CTA scores a chunk of 256 logical pages (phase A, the
+// Grid = (page chunks, kv-heads, sequences).  Every CTA scores a chunk of kSelChunk logical pages (phase A, the
 // HBM stream: 512 B of summary per candidate page, gathered through the page table); the LAST CTA of a
 // (sequence, kv-head) to finish -- found with one atomic counter -- runs the top-k over that unit's scores
 // (phase B: radix select on order-preserving keys + ordered compaction).  So the summary stream is spread
@@ -10,13 +10,26 @@
 // Score (reading R5): s[p] = sum_{h in group} sum_d max(q_h[d]*mn[d], q_h[d]*mx[d])
 //                          = sum_d ( Q+[d]*mx[d] + Q-[d]*mn[d] ),  Q+ = sum_h max(q_h,0), Q- = sum_h min(q_h,0)
 // i.e. one 256-long fp32 dot product per page, independent of the GQA ratio r.
+//
+// Phase A data path: a warp owns 32 consecutive logical pages; one load instruction of the warp reads the whole
+// 512-byte summary of ONE page (lane = 16-byte chunk: lanes 0-15 the min vector, 16-31 the max vector), and
+// kSelBatch such loads are issued back to back before the first is consumed (kSelBatch x 16 B in flight per lane,
+// kSelBatch x 4 KiB per CTA).  Each lane needs only its 8 entries of Q-/Q+ in registers.  The per-page partial
+// sums are combined with a transpose-reduce (8 values over 32 lanes in 9 shuffles).
 #pragma once
 #include "common.cuh"
 
 namespace sparrow {
 
 constexpr int kSelThreads = 256;
-constexpr int kSelChunk = 256;       // logical pages per CTA in phase A
+constexpr int kSelWarps = kSelThreads / 32;
+#ifndef SPARROW_SEL_PPW
+#define SPARROW_SEL_PPW 32
+#endif
+constexpr int kSelPagesPerWarp = SPARROW_SEL_PPW;       // consecutive logical pages owned by one warp (<= 32: one lane per table entry)
+constexpr int kSelChunk = kSelWarps * kSelPagesPerWarp; // logical pages per CTA in phase A
+constexpr int kSelBatch = 8;         // summaries in flight per warp
+constexpr int kSelMinBlocks = 4;     // CTAs / SM the register budget is held to
 constexpr int kSelMaxPages = 16384;  // keys of one unit live in shared memory (64 KiB): 262144 tokens
 
 // fp32 -> uint32 whose unsigned order is the float order (larger score = larger key); never 0 for a real score
@@ -26,43 +39,80 @@ __device__ __forceinline__ uint32_t order_key(float f)
     return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
 }
 
-// exclusive prefix of a 0/1 flag over the 256 threads of the CTA; *total = sum.  warp_sums: 8 ints of smem.
-__device__ __forceinline__ int block_excl_scan_flag(bool flag, int *warp_sums, int *total)
+// exclusive prefix sum of one int per thread over the CTA; *total = sum.  warp_sums: kSelWarps ints of smem.
+__device__ __forceinline__ int block_excl_scan(int v, int *warp_sums, int *total)
 {
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const uint32_t b = __ballot_sync(0xffffffffu, flag);
-    const int within = __popc(b & ((1u << lane) - 1u));
+    int inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
     __syncthreads();                       // previous users of warp_sums are done
-    if (lane == 0) warp_sums[w] = __popc(b);
+    if (lane == 31) warp_sums[w] = inc;
     __syncthreads();
     int before = 0, tot = 0;
 #pragma unroll
-    for (int i = 0; i < kSelThreads / 32; ++i) {
-        const int v = warp_sums[i];
-        if (i < w) before += v;
-        tot += v;
+    for (int i = 0; i < kSelWarps; ++i) {
+        const int s = warp_sums[i];
+        if (i < w) before += s;
+        tot += s;
     }
     *total = tot;
-    return before + within;
+    return before + inc - v;
 }
 
-__global__ void __launch_bounds__(kSelThreads)
+__device__ __forceinline__ float dot8(const float (&qr)[8], const uint4 v, float acc)
+{
+    acc = fmaf(qr[0], bf16_lo(v.x), acc); acc = fmaf(qr[1], bf16_hi(v.x), acc);
+    acc = fmaf(qr[2], bf16_lo(v.y), acc); acc = fmaf(qr[3], bf16_hi(v.y), acc);
+    acc = fmaf(qr[4], bf16_lo(v.z), acc); acc = fmaf(qr[5], bf16_hi(v.z), acc);
+    acc = fmaf(qr[6], bf16_lo(v.w), acc); acc = fmaf(qr[7], bf16_hi(v.w), acc);
+    return acc;
+}
+
+__global__ void __launch_bounds__(kSelThreads, kSelMinBlocks)
 select_kernel(const uint16_t *__restrict__ q, const uint16_t *__restrict__ summaries,
               const int32_t *__restrict__ page_table, const int32_t *__restrict__ seq_lens,
               const SchedDev sched, int32_t *__restrict__ sel_pages, int max_sel, int32_t *__restrict__ sel_count,
               float *__restrict__ scores_ws, int32_t *__restrict__ counters, float *__restrict__ scores_dbg,
               int n_q_heads, int n_kv_heads, int max_pages)
 {
-    extern __shared__ uint32_t s_keys[];                 // [max_pages] (phase B only)
+    extern __shared__ uint32_t s_keys[];                 // [n_pages] (phase B only)
     __shared__ float s_q[2][kDim];                       // [0] = Q- (pairs with min), [1] = Q+ (pairs with max)
     __shared__ int s_hist[256];
-    __shared__ int s_warp[kSelThreads / 32];
-    __shared__ int s_bcast[2];
+    __shared__ int s_warp[kSelWarps];
+    __shared__ int s_bcast[4][3];
+    __shared__ SeqPlan s_plan;
 
     const int chunk = blockIdx.x, g = blockIdx.y, seq = blockIdx.z;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int r = n_q_heads / n_kv_heads;
-    const SeqPlan pl = make_plan(sched, seq_lens[seq]);
+
+    // Independent global loads first (sequence length, this lane's page-table entry, q), so that their latencies
+    // overlap instead of chaining: only the summary gather depends on them.
+    const int my_page = chunk * kSelChunk + warp * kSelPagesPerWarp + lane;   // logical page of this lane's table entry
+    const bool my_slot = lane < kSelPagesPerWarp;
+    const int L = seq_lens[seq];
+    const int my_phys = (my_slot && my_page < max_pages) ? __ldg(page_table + (int64_t)seq * max_pages + my_page) : 0;
+    float qp = 0.f, qm = 0.f;
+    if (tid < kDim) {
+        const uint16_t *qs = q + ((int64_t)seq * n_q_heads + g * r) * kDim + tid;
+        for (int j = 0; j < r; ++j) {
+            const float v = __uint_as_float((uint32_t)__ldg(qs + j * kDim) << 16);
+            qp += fmaxf(v, 0.f);
+            qm += fminf(v, 0.f);
+        }
+    }
+    // B(L) and the forced-page rule are exact 64/128-bit integer arithmetic: one thread evaluates them for the CTA.
+    if (tid == 0) s_plan = make_plan(sched, L);
+    if (tid < kDim) {
+        s_q[0][tid] = qm;
+        s_q[1][tid] = qp;
+    }
+    __syncthreads();
+    const SeqPlan pl = s_plan;
     int32_t *out = sel_pages + ((int64_t)seq * n_kv_heads + g) * max_sel;
 
     if (pl.dense) {                                      // R13: all pages, no scoring
@@ -76,64 +126,63 @@ select_kernel(const uint16_t *__restrict__ q, const uint16_t *__restrict__ summa
     if (chunk >= n_chunks) return;
 
     // ---------------------------------------------------------------- phase A: score this chunk ----
-    if (tid < kDim) {
-        float qp = 0.f, qm = 0.f;
-        const uint16_t *qs = q + ((int64_t)seq * n_q_heads + g * r) * kDim + tid;
-        for (int j = 0; j < r; ++j) {
-            const float v = __uint_as_float((uint32_t)qs[j * kDim] << 16);
-            qp += fmaxf(v, 0.f);
-            qm += fminf(v, 0.f);
+    float qr[8];                                         // lane = 16-byte chunk of the summary: 8 channels of min or max
+#pragma unroll
+    for (int e = 0; e < 8; ++e) qr[e] = (&s_q[0][0])[lane * 8 + e];
+
+    const bool my_cand = my_slot && my_page < pl.n_pages && !pl.forced(my_page);
+    const uint32_t cand_mask = __ballot_sync(0xffffffffu, my_cand);      // bit j: page warp_base + j is a candidate
+    const uint16_t *sum_g = summaries + (int64_t)g * kSumElems + lane * 8;
+    const int64_t page_stride = (int64_t)n_kv_heads * kSumElems;
+    float my_score = 0.f;                                // score of page warp_base + lane, gathered below
+
+#pragma unroll 1
+    for (int b0 = 0; b0 < kSelPagesPerWarp; b0 += kSelBatch) {
+        const uint32_t bm = (cand_mask >> b0) & ((1u << kSelBatch) - 1u);
+        if (bm == 0) continue;                           // warp-uniform
+        uint4 v[kSelBatch];
+#pragma unroll
+        for (int j = 0; j < kSelBatch; ++j) {            // all loads of the batch first
+            const int phys = __shfl_sync(0xffffffffu, my_phys, b0 + j);
+            v[j] = (bm >> j) & 1u ? ldg_stream16(sum_g + phys * page_stride) : make_uint4(0u, 0u, 0u, 0u);
         }
-        s_q[0][tid] = qm;
-        s_q[1][tid] = qp;
+        float a[kSelBatch];
+#pragma unroll
+        for (int j = 0; j < kSelBatch; ++j) a[j] = dot8(qr, v[j], 0.f);
+        // transpose-reduce: after the three halving steps lane l holds page j = 4*b4 + 2*b3 + b2 (bits of l),
+        // summed over the lanes that differ from l in bits 4, 3, 2; two more butterflies finish the sum.
+        static_assert(kSelBatch == 8, "transpose-reduce is written for 8 pages per batch");
+        {
+            const bool hi = lane & 16;
+            float k0 = hi ? a[4] : a[0], k1 = hi ? a[5] : a[1], k2 = hi ? a[6] : a[2], k3 = hi ? a[7] : a[3];
+            float s0 = hi ? a[0] : a[4], s1 = hi ? a[1] : a[5], s2 = hi ? a[2] : a[6], s3 = hi ? a[3] : a[7];
+            k0 += __shfl_xor_sync(0xffffffffu, s0, 16);
+            k1 += __shfl_xor_sync(0xffffffffu, s1, 16);
+            k2 += __shfl_xor_sync(0xffffffffu, s2, 16);
+            k3 += __shfl_xor_sync(0xffffffffu, s3, 16);
+            const bool h8 = lane & 8;
+            float m0 = h8 ? k2 : k0, m1 = h8 ? k3 : k1;
+            float t0 = h8 ? k0 : k2, t1 = h8 ? k1 : k3;
+            m0 += __shfl_xor_sync(0xffffffffu, t0, 8);
+            m1 += __shfl_xor_sync(0xffffffffu, t1, 8);
+            const bool h4 = lane & 4;
+            float z = h4 ? m1 : m0, y = h4 ? m0 : m1;
+            z += __shfl_xor_sync(0xffffffffu, y, 4);
+            z += __shfl_xor_sync(0xffffffffu, z, 2);
+            z += __shfl_xor_sync(0xffffffffu, z, 1);
+            // lane l now holds the score of batch page j(l) = ((l>>4)&1)*4 + ((l>>3)&1)*2 + ((l>>2)&1);
+            // hand it to the lane that owns that page's table entry (lane b0 + j): source lane for j is
+            // 16*(j>>2) + 8*((j>>1)&1) + 4*(j&1).
+            const int j = lane - b0;
+            const int src = ((j >> 2) & 1) * 16 + ((j >> 1) & 1) * 8 + (j & 1) * 4;
+            const float got = __shfl_sync(0xffffffffu, z, src & 31);
+            if (j >= 0 && j < kSelBatch) my_score = got;
+        }
     }
-    __syncthreads();
-
-    // 8 lanes per page: lane sub-id s reads 16-byte chunks {s, 8+s, 16+s, 24+s} of the 512-byte summary
-    // (chunks 0-15 = min, 16-31 = max), so each load instruction of a warp reads 4 x 128 contiguous bytes.
-    const int s = lane & 7, slot = lane >> 3;
-    float qr[4][8];
-    const float *sq = &s_q[0][0];
-#pragma unroll
-    for (int i = 0; i < 4; ++i)
-#pragma unroll
-        for (int e = 0; e < 8; ++e) qr[i][e] = sq[(i * 8 + s) * 8 + e];
-
-    const int32_t *pt = page_table + (int64_t)seq * max_pages;
     float *ws = scores_ws + ((int64_t)seq * n_kv_heads + g) * max_pages;
-    constexpr int kIters = kSelChunk / (kSelThreads / 32 * 4);      // 8
-    int p_of[kIters];
-    int phys[kIters];
-#pragma unroll
-    for (int it = 0; it < kIters; ++it) {
-        const int p = chunk * kSelChunk + it * 32 + warp * 4 + slot;
-        const bool cand = p < pl.n_pages && !pl.forced(p);
-        p_of[it] = cand ? p : -1;
-        phys[it] = cand ? pt[p] : 0;
-    }
-#pragma unroll
-    for (int it = 0; it < kIters; ++it) {
-        float acc = 0.f;
-        if (p_of[it] >= 0) {
-            const uint16_t *src = summaries + ((int64_t)phys[it] * n_kv_heads + g) * kSumElems + s * 8;
-            uint4 v[4];
-#pragma unroll
-            for (int i = 0; i < 4; ++i) v[i] = ldg_stream16(src + i * 64);
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                acc = fmaf(qr[i][0], bf16_lo(v[i].x), acc); acc = fmaf(qr[i][1], bf16_hi(v[i].x), acc);
-                acc = fmaf(qr[i][2], bf16_lo(v[i].y), acc); acc = fmaf(qr[i][3], bf16_hi(v[i].y), acc);
-                acc = fmaf(qr[i][4], bf16_lo(v[i].z), acc); acc = fmaf(qr[i][5], bf16_hi(v[i].z), acc);
-                acc = fmaf(qr[i][6], bf16_lo(v[i].w), acc); acc = fmaf(qr[i][7], bf16_hi(v[i].w), acc);
-            }
-        }
-        acc += __shfl_xor_sync(0xffffffffu, acc, 1);
-        acc += __shfl_xor_sync(0xffffffffu, acc, 2);
-        acc += __shfl_xor_sync(0xffffffffu, acc, 4);
-        if (s == 0 && p_of[it] >= 0) {
-            ws[p_of[it]] = acc;
-            if (scores_dbg) scores_dbg[((int64_t)seq * n_kv_heads + g) * max_pages + p_of[it]] = acc;
-        }
+    if (my_cand) {                                       // one coalesced 128-byte store per warp
+        ws[my_page] = my_score;
+        if (scores_dbg) scores_dbg[((int64_t)seq * n_kv_heads + g) * max_pages + my_page] = my_score;
     }
 
     // ------------------------------------------------ last CTA of this (sequence, kv-head)? --------
@@ -144,32 +193,35 @@ select_kernel(const uint16_t *__restrict__ q, const uint16_t *__restrict__ summa
         const int old = atomicAdd(ctr, 1);
         const int last = (old == n_chunks - 1);
         if (last) *ctr = 0;                              // restore the zero for the next call
-        s_bcast[0] = last;
+        s_bcast[0][0] = last;
     }
     __syncthreads();
-    if (!s_bcast[0]) return;
+    if (!s_bcast[0][0]) return;
     __threadfence();
 
     // ---------------------------------------------------------------- phase B: top-k of the unit ----
-    for (int p = tid; p < pl.n_pages; p += kSelThreads)
+    const int n_pages = pl.n_pages;
+    for (int p = tid; p < n_pages; p += kSelThreads)
         s_keys[p] = pl.forced(p) ? 0u : order_key(__ldcg(ws + p));
+    s_hist[tid] = 0;
     __syncthreads();
 
-    uint32_t thr = 0xffffffffu;      // key of the k-th best candidate
-    int need_eq = 0;                 // how many candidates with key == thr are taken (lowest page index first, R10)
+    // Radix select, 8 bits per pass, most significant first.  Invariant: the k-th best key has (key & mask) == prefix
+    // and is the kk-th best inside that class.  Stops early when the class is taken whole (kk == its size).
+    uint32_t prefix = 0, mask = 0;
+    int need_eq = 0;                 // how many keys of the final class are taken (lowest page index first, R10)
     if (pl.k > 0) {
-        uint32_t prefix = 0, mask = 0;
-        int kk = pl.k;               // rank still to resolve inside the current prefix class (1 = best)
-        for (int shift = 24; shift >= 0; shift -= 8) {
-            s_hist[tid] = 0;
-            __syncthreads();
-            for (int p = tid; p < pl.n_pages; p += kSelThreads) {
+        int kk = pl.k;
+        for (int pass = 0; pass < 4; ++pass) {
+            const int shift = 24 - 8 * pass;
+            for (int p = tid; p < n_pages; p += kSelThreads) {
                 const uint32_t key = s_keys[p];
-                if ((key & mask) == prefix) atomicAdd(&s_hist[(key >> shift) & 255u], 1);
+                if (key != 0u && (key & mask) == prefix) atomicAdd(&s_hist[(key >> shift) & 255u], 1);
             }
             __syncthreads();
             // suffix sums over the 256 bins: S[t] = sum_{j >= t} hist[j]
             const int h = s_hist[tid];
+            s_hist[tid] = 0;                             // ready for the next pass
             int suf = h;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
@@ -178,39 +230,55 @@ select_kernel(const uint16_t *__restrict__ q, const uint16_t *__restrict__ summa
             }
             if (lane == 0) s_warp[warp] = suf;
             __syncthreads();
-            for (int w2 = warp + 1; w2 < kSelThreads / 32; ++w2) suf += s_warp[w2];
+            for (int w2 = warp + 1; w2 < kSelWarps; ++w2) suf += s_warp[w2];
             if (suf >= kk && suf - h < kk) {             // exactly one bin holds the kk-th best key
-                s_bcast[0] = tid;
-                s_bcast[1] = kk - (suf - h);
+                s_bcast[pass][0] = tid;
+                s_bcast[pass][1] = kk - (suf - h);
+                s_bcast[pass][2] = h;
             }
             __syncthreads();
-            prefix |= (uint32_t)s_bcast[0] << shift;
+            prefix |= (uint32_t)s_bcast[pass][0] << shift;
             mask |= 255u << shift;
-            kk = s_bcast[1];
-            __syncthreads();
+            kk = s_bcast[pass][1];
+            need_eq = kk;
+            if (kk == s_bcast[pass][2]) break;           // the whole class is taken: no need to split it further
         }
-        thr = prefix;
-        need_eq = kk;
     }
 
-    // ordered compaction: forced pages, keys above the threshold, and the first need_eq keys equal to it
-    int base_out = 0, base_eq = 0;
-    for (int p0 = 0; p0 < pl.n_pages; p0 += kSelThreads) {
-        const int p = p0 + tid;
-        const bool inb = p < pl.n_pages;
-        const uint32_t key = inb ? s_keys[p] : 0u;
-        const bool f = inb && pl.forced(p);
-        const bool eq = inb && !f && key == thr;
-        const bool gt = inb && !f && key > thr;
-        int tot_eq, tot_take;
-        const int eq_rank = base_eq + block_excl_scan_flag(eq, s_warp, &tot_eq);
-        const bool take = f || gt || (eq && eq_rank < need_eq);
-        const int pos = base_out + block_excl_scan_flag(take, s_warp, &tot_take);
-        if (take && pos < max_sel) out[pos] = p;
-        base_eq += tot_eq;
-        base_out += tot_take;
+    // Ordered compaction.  Thread t owns the contiguous pages [t*ipt, (t+1)*ipt): forced pages, keys above the class,
+    // and the first need_eq keys of the class (page order) are emitted in ascending page order.
+    const int ipt = (n_pages + kSelThreads - 1) / kSelThreads;
+    const int p_lo = tid * ipt, p_hi = min(p_lo + ipt, n_pages);
+    int n_eq = 0, n_sure = 0;
+    for (int p = p_lo; p < p_hi; ++p) {
+        const uint32_t key = s_keys[p];
+        if (key == 0u) n_sure += pl.forced(p);
+        else if (pl.k > 0) {
+            const uint32_t c = key & mask;
+            n_sure += c > prefix;
+            n_eq += c == prefix;
+        }
     }
-    if (g == 0 && tid == 0) sel_count[seq] = base_out < max_sel ? base_out : max_sel;
+    int tot_eq, tot_take;
+    const int eq_base = block_excl_scan(n_eq, s_warp, &tot_eq);
+    int eq_left = need_eq - eq_base;                     // class members this thread may still take
+    eq_left = eq_left < 0 ? 0 : (eq_left > n_eq ? n_eq : eq_left);
+    int pos = block_excl_scan(n_sure + eq_left, s_warp, &tot_take);
+    for (int p = p_lo; p < p_hi; ++p) {
+        const uint32_t key = s_keys[p];
+        bool take;
+        if (key == 0u) take = pl.forced(p);
+        else if (pl.k > 0) {
+            const uint32_t c = key & mask;
+            take = c > prefix;
+            if (c == prefix && eq_left > 0) { take = true; --eq_left; }
+        } else take = false;
+        if (take) {
+            if (pos < max_sel) out[pos] = p;
+            ++pos;
+        }
+    }
+    if (g == 0 && tid == 0) sel_count[seq] = tot_take < max_sel ? tot_take : max_sel;
 }
 
 }  // namespace sparrow
