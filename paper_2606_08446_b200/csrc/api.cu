@@ -59,6 +59,7 @@ int to_dev_sched(const sparrow_schedule_t *in, SchedDev *out)
     out->L0 = in->L0;
     out->L1 = in->L1;
     out->bin_tokens = in->bin_tokens;
+    out->inv_den = 1.0;
     if (in->kind == SPARROW_SCHED_FIXED && in->fixed_tokens < 0) return SPARROW_ERR_INVALID_ARG;
     constexpr int64_t kPpmMax = 1000000;                 // keep fractions are in [0, 1]
     if (in->kind == SPARROW_SCHED_CLAMP_FRAC && (in->f0_ppm < 0 || in->f0_ppm > kPpmMax || in->floor_tokens < 0))
@@ -67,6 +68,7 @@ int to_dev_sched(const sparrow_schedule_t *in, SchedDev *out)
         (in->L0 < 0 || in->L1 <= in->L0 || in->L1 - in->L0 > 0x7fffffffLL || in->f0_ppm < 0 || in->f0_ppm > kPpmMax ||
          in->f1_ppm < 0 || in->f1_ppm > kPpmMax || in->floor_tokens < 0))
         return SPARROW_ERR_INVALID_ARG;
+    if (in->kind == SPARROW_SCHED_LINEAR_FRAC) out->inv_den = 1.0 / (1.0e6 * (double)(in->L1 - in->L0));
     if (in->kind == SPARROW_SCHED_TABLE) {
         if (!in->table_pages || in->table_len <= 0 || in->table_len > SPARROW_MAX_TABLE_BINS || in->bin_tokens <= 0)
             return SPARROW_ERR_INVALID_ARG;
@@ -161,10 +163,21 @@ int select_impl(const void *q, const void *summaries, const int32_t *page_table,
 {
     if (workspace_bytes < sparrow_select_workspace_bytes(s)) return SPARROW_ERR_WORKSPACE_TOO_SMALL;
     if (s->max_pages_per_seq > kSelMaxPages) return SPARROW_ERR_UNSUPPORTED;
+    if (s->n_phys_pages * s->n_kv_heads >= (1LL << 27)) return SPARROW_ERR_UNSUPPORTED;   // 32-bit offsets in 16-byte units
     if (s->n_seq == 0) return SPARROW_OK;
     int32_t *counters = reinterpret_cast<int32_t *>(workspace);
     float *scores_ws = reinterpret_cast<float *>(reinterpret_cast<uint8_t *>(workspace) +
                                                  align256((size_t)s->n_seq * s->n_kv_heads * sizeof(int32_t)));
+    // Pages per CTA: as large as keeps >= 4 CTAs per resident slot (4 per SM) so the tail stays short, because the
+    // per-CTA prologue (plan, Q+/Q-, first table entries) is amortised over the pages a CTA streams.
+    const int64_t units = (int64_t)s->n_seq * s->n_kv_heads;
+    int pages_per_cta = kSelCtaPagesMin;
+    for (int p = 4 * kSelCtaPagesMin; p > kSelCtaPagesMin; p >>= 1) {
+        if (units * ((s->max_pages_per_seq + p - 1) / p) >= 4 * kSelMinBlocks * kNumSmsB200) { pages_per_cta = p; break; }
+    }
+#ifdef SPARROW_SEL_PPC_FIXED
+    pages_per_cta = SPARROW_SEL_PPC_FIXED;
+#endif
     const size_t dyn = (size_t)s->max_pages_per_seq * sizeof(uint32_t);
     static size_t dyn_set = 0;
     if (dyn > 48 * 1024 && dyn > dyn_set) {
@@ -172,10 +185,10 @@ int select_impl(const void *q, const void *summaries, const int32_t *page_table,
         if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(select_kernel)");
         dyn_set = dyn;
     }
-    dim3 grid((s->max_pages_per_seq + kSelChunk - 1) / kSelChunk, s->n_kv_heads, s->n_seq);
+    dim3 grid((s->max_pages_per_seq + pages_per_cta - 1) / pages_per_cta, s->n_kv_heads, s->n_seq);
     select_kernel<<<grid, kSelThreads, dyn, st>>>((const uint16_t *)q, (const uint16_t *)summaries, page_table, seq_lens,
                                                   sd, sel_pages, max_sel, sel_count, scores_ws, counters, scores_dbg,
-                                                  s->n_q_heads, s->n_kv_heads, s->max_pages_per_seq);
+                                                  s->n_q_heads, s->n_kv_heads, s->max_pages_per_seq, pages_per_cta);
     SPARROW_CHECK_LAUNCH("select_kernel");
     return SPARROW_OK;
 }

@@ -20,22 +20,28 @@ constexpr int kSumElems = 2 * kDim;             // one (page, kv-head) summary: 
 struct SchedDev {
     int32_t kind, sink_tokens, local_tokens, table_len, bin_tokens;
     int64_t fixed_tokens, floor_tokens, f0_ppm, f1_ppm, L0, L1;
+    double inv_den;              // LINEAR_FRAC: 1.0 / (1e6 * (L1 - L0)), the quotient estimate's multiplier
     int32_t table[SPARROW_MAX_TABLE_BINS];
 };
 
 __host__ __device__ inline int64_t ceil_div64(int64_t a, int64_t b) { return (a + b - 1) / b; }
 
-// floor(a * b / c) for a, b >= 0, c > 0, exact.  A 128-bit division is hundreds of instructions on the GPU, so the
-// quotient is estimated in fp64 (three roundings: off by a few units at most while it is below 2^50) and then fixed
-// with exact 128-bit products; larger quotients (host callers only) take the plain 128-bit division.
-__host__ __device__ inline int64_t muldiv_floor(int64_t a, int64_t b, int64_t c)
+// floor(a * b / c) for a, b >= 0, c > 0, exact; inv_c = 1.0 / c rounded to fp64 (the host puts it in SchedDev).
+// A 128-bit (or even 64-bit) division is hundreds of instructions on the GPU and sits on every CTA's critical path,
+// so the quotient is estimated with two fp64 multiplies (off by a unit or two at most while it is below 2^50) and
+// then fixed with the exact remainder a*b - q*c, which is tiny and therefore survives 64-bit wrap-around
+// arithmetic.  Larger quotients (possible only for host callers: device lengths are int32) take the plain
+// 128-bit division.
+__host__ __device__ inline int64_t muldiv_floor(int64_t a, int64_t b, int64_t c, double inv_c)
 {
-    const __int128 prod = (__int128)a * b;
-    const double est = (double)a * (double)b / (double)c;
-    if (!(est < 1125899906842624.0)) return (int64_t)(prod / c);
+    const double est = (double)a * (double)b * inv_c;
+#ifndef __CUDA_ARCH__
+    if (!(est < 1125899906842624.0)) return (int64_t)(((__int128)a * b) / c);
+#endif
     int64_t qv = (int64_t)est;
-    while ((__int128)qv * c > prod) --qv;
-    while ((__int128)(qv + 1) * c <= prod) ++qv;
+    int64_t rem = (int64_t)((uint64_t)a * (uint64_t)b - (uint64_t)qv * (uint64_t)c);
+    while (rem < 0) { --qv; rem += c; }
+    while (rem >= c) { ++qv; rem -= c; }
     return qv;
 }
 
@@ -47,7 +53,7 @@ __host__ __device__ inline int64_t budget_tokens(const SchedDev &s, int64_t L)
     case SPARROW_SCHED_DENSE: B = L; break;
     case SPARROW_SCHED_FIXED: B = s.fixed_tokens; break;
     case SPARROW_SCHED_CLAMP_FRAC:
-        B = muldiv_floor(L, s.f0_ppm, 1000000);
+        B = muldiv_floor(L, s.f0_ppm, 1000000, 1.0e-6);
         if (B < s.floor_tokens) B = s.floor_tokens;
         break;
     case SPARROW_SCHED_LINEAR_FRAC: {
@@ -56,12 +62,16 @@ __host__ __device__ inline int64_t budget_tokens(const SchedDev &s, int64_t L)
         // validated on entry: 0 <= f <= 1e6 ppm and span < 2^31, so num and den stay below 2^51
         const int64_t num = s.f0_ppm * span - (s.f0_ppm - s.f1_ppm) * (Lc - s.L0);
         const int64_t den = 1000000 * span;
-        B = muldiv_floor(L, num, den);
+        B = muldiv_floor(L, num, den, s.inv_den);
         if (B < s.floor_tokens) B = s.floor_tokens;
         break;
     }
     default: {  // TABLE: pages per length bin, B = pagesize x num_pages
+#ifdef __CUDA_ARCH__
+        int64_t b = L > 0 ? (int64_t)((uint32_t)(L - 1) / (uint32_t)s.bin_tokens) : 0;   // device lengths are int32
+#else
         int64_t b = (L - 1) / s.bin_tokens;
+#endif
         if (b < 0) b = 0;
         if (b >= s.table_len) b = s.table_len - 1;
         B = (int64_t)s.table[b] * kPage;
@@ -123,5 +133,44 @@ __device__ __forceinline__ uint4 ldg_stream16(const void *p)
 }
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+// ---- mbarrier + bulk-copy (TMA) primitives; shared-memory operands are 32-bit shared::cta addresses ----
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+// make freshly initialised barriers visible to the async proxy (the TMA unit completes transactions on them)
+__device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    while (!mbar_try_wait(bar, parity)) {}
+}
+// 1-D bulk copy global -> shared (UBLKCP): bytes and both addresses multiples of 16; completes `bytes` on `bar`
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ uint4 lds128(uint32_t addr)
+{
+    uint4 r;
+    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(addr));
+    return r;
+}
 
 }  // namespace sparrow

@@ -1,7 +1,7 @@
 // select.cuh -- kernel (b): fused page scoring + per-(sequence, kv-head) top-k page selection.
 // SURVEY.md 8(a) a2-a5; PAPER.md:138-147 ("landmark scores", Top-k), north_star (b).
 //
-// Grid = (page chunks, kv-heads, sequences).  Every CTA scores a chunk of kSelChunk logical pages (phase A, the
+// Grid = (page slices, kv-heads, sequences).  Every CTA scores a slice of pages_per_cta logical pages (phase A, the
 // HBM stream: 512 B of summary per candidate page, gathered through the page table); the LAST CTA of a
 // (sequence, kv-head) to finish -- found with one atomic counter -- runs the top-k over that unit's scores
 // (phase B: radix select on order-preserving keys + ordered compaction).  So the summary stream is spread
@@ -11,11 +11,14 @@
 //                          = sum_d ( Q+[d]*mx[d] + Q-[d]*mn[d] ),  Q+ = sum_h max(q_h,0), Q- = sum_h min(q_h,0)
 // i.e. one 256-long fp32 dot product per page, independent of the GQA ratio r.
 //
-// Phase A data path: a warp owns 32 consecutive logical pages; one load instruction of the warp reads the whole
-// 512-byte summary of ONE page (lane = 16-byte chunk: lanes 0-15 the min vector, 16-31 the max vector), and
-// kSelBatch such loads are issued back to back before the first is consumed (kSelBatch x 16 B in flight per lane,
-// kSelBatch x 4 KiB per CTA).  Each lane needs only its 8 entries of Q-/Q+ in registers.  The per-page partial
-// sums are combined with a transpose-reduce (8 values over 32 lanes in 9 shuffles).
+// Phase A data path: a CTA owns `pages_per_cta` consecutive logical pages of one (sequence, kv-head); its 8 warps
+// take 32-page warp-chunks round-robin, with the page-table entries of the next warp-chunk prefetched.  One load
+// instruction of a warp reads the whole 512-byte summary of ONE page (lane = 16-byte chunk: lanes 0-15 the min
+// vector, 16-31 the max vector), and kSelBatch such loads are issued back to back before the first is consumed
+// (kSelBatch x 16 B in flight per lane, kSelBatch x 4 KiB per CTA).  Each lane needs only its 8 entries of Q-/Q+
+// in registers.  The per-page partial sums are combined with a transpose-reduce (8 values over 32 lanes in 9
+// shuffles).  (A TMA bulk-copy ring was measured and rejected here: at 512 B per request the copy engine's
+// request rate, not HBM, became the limit -- profiles/r1_select_notes.md.)
 #pragma once
 #include "common.cuh"
 
@@ -23,13 +26,10 @@ namespace sparrow {
 
 constexpr int kSelThreads = 256;
 constexpr int kSelWarps = kSelThreads / 32;
-#ifndef SPARROW_SEL_PPW
-#define SPARROW_SEL_PPW 32
-#endif
-constexpr int kSelPagesPerWarp = SPARROW_SEL_PPW;       // consecutive logical pages owned by one warp (<= 32: one lane per table entry)
-constexpr int kSelChunk = kSelWarps * kSelPagesPerWarp; // logical pages per CTA in phase A
-constexpr int kSelBatch = 8;         // summaries in flight per warp
-constexpr int kSelMinBlocks = 4;     // CTAs / SM the register budget is held to
+constexpr int kSelPagesPerWarp = 32;                    // one warp-chunk: one lane per page-table entry
+constexpr int kSelBatch = 8;                            // summaries in flight per warp
+constexpr int kSelMinBlocks = 4;                        // CTAs / SM the register budget is held to
+constexpr int kSelCtaPagesMin = kSelWarps * kSelPagesPerWarp;                // pages_per_cta is a multiple of this
 constexpr int kSelMaxPages = 16384;  // keys of one unit live in shared memory (64 KiB): 262144 tokens
 
 // fp32 -> uint32 whose unsigned order is the float order (larger score = larger key); never 0 for a real score
@@ -77,7 +77,7 @@ select_kernel(const uint16_t *__restrict__ q, const uint16_t *__restrict__ summa
               const int32_t *__restrict__ page_table, const int32_t *__restrict__ seq_lens,
               const SchedDev sched, int32_t *__restrict__ sel_pages, int max_sel, int32_t *__restrict__ sel_count,
               float *__restrict__ scores_ws, int32_t *__restrict__ counters, float *__restrict__ scores_dbg,
-              int n_q_heads, int n_kv_heads, int max_pages)
+              int n_q_heads, int n_kv_heads, int max_pages, int pages_per_cta)
 {
     extern __shared__ uint32_t s_keys[];                 // [n_pages] (phase B only)
     __shared__ float s_q[2][kDim];                       // [0] = Q- (pairs with min), [1] = Q+ (pairs with max)
@@ -86,16 +86,21 @@ select_kernel(const uint16_t *__restrict__ q, const uint16_t *__restrict__ summa
     __shared__ int s_bcast[4][3];
     __shared__ SeqPlan s_plan;
 
-    const int chunk = blockIdx.x, g = blockIdx.y, seq = blockIdx.z;
+    const int slice = blockIdx.x, g = blockIdx.y, seq = blockIdx.z;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int r = n_q_heads / n_kv_heads;
+    const int cta_page0 = slice * pages_per_cta;
+    const int32_t *pt = page_table + (int64_t)seq * max_pages;
 
-    // Independent global loads first (sequence length, this lane's page-table entry, q), so that their latencies
+    // Independent global loads first (sequence length, q, the first page-table entries), so that their latencies
     // overlap instead of chaining: only the summary gather depends on them.
-    const int my_page = chunk * kSelChunk + warp * kSelPagesPerWarp + lane;   // logical page of this lane's table entry
-    const bool my_slot = lane < kSelPagesPerWarp;
     const int L = seq_lens[seq];
-    const int my_phys = (my_slot && my_page < max_pages) ? __ldg(page_table + (int64_t)seq * max_pages + my_page) : 0;
+    int phys_cur = 0, phys_nxt = 0;                      // table entries of this warp's chunks i, i+1 (lane = page)
+    {
+        const int p0 = cta_page0 + warp * kSelPagesPerWarp + lane, p1 = p0 + kSelCtaPagesMin;
+        if (p0 < max_pages) phys_cur = __ldg(pt + p0);
+        if (p1 < max_pages && p1 < cta_page0 + pages_per_cta) phys_nxt = __ldg(pt + p1);
+    }
     float qp = 0.f, qm = 0.f;
     if (tid < kDim) {
         const uint16_t *qs = q + ((int64_t)seq * n_q_heads + g * r) * kDim + tid;
@@ -105,7 +110,7 @@ select_kernel(const uint16_t *__restrict__ q, const uint16_t *__restrict__ summa
             qm += fminf(v, 0.f);
         }
     }
-    // B(L) and the forced-page rule are exact 64/128-bit integer arithmetic: one thread evaluates them for the CTA.
+    // B(L) and the forced-page rule are exact integer arithmetic: one thread evaluates them for the CTA.
     if (tid == 0) s_plan = make_plan(sched, L);
     if (tid < kDim) {
         s_q[0][tid] = qm;
@@ -116,43 +121,61 @@ select_kernel(const uint16_t *__restrict__ q, const uint16_t *__restrict__ summa
     int32_t *out = sel_pages + ((int64_t)seq * n_kv_heads + g) * max_sel;
 
     if (pl.dense) {                                      // R13: all pages, no scoring
-        if (chunk == 0) {
+        if (slice == 0) {
             for (int p = tid; p < pl.n_pages && p < max_sel; p += kSelThreads) out[p] = p;
             if (g == 0 && tid == 0) sel_count[seq] = pl.n_pages < max_sel ? pl.n_pages : max_sel;
         }
         return;
     }
-    const int n_chunks = (pl.n_pages + kSelChunk - 1) / kSelChunk;
-    if (chunk >= n_chunks) return;
+    const int n_chunks = (pl.n_pages + pages_per_cta - 1) / pages_per_cta;
+    if (slice >= n_chunks) return;
 
-    // ---------------------------------------------------------------- phase A: score this chunk ----
+    // ---------------------------------------------------------------- phase A: score this CTA's pages ----
     float qr[8];                                         // lane = 16-byte chunk of the summary: 8 channels of min or max
 #pragma unroll
     for (int e = 0; e < 8; ++e) qr[e] = (&s_q[0][0])[lane * 8 + e];
 
-    const bool my_cand = my_slot && my_page < pl.n_pages && !pl.forced(my_page);
-    const uint32_t cand_mask = __ballot_sync(0xffffffffu, my_cand);      // bit j: page warp_base + j is a candidate
-    const uint16_t *sum_g = summaries + (int64_t)g * kSumElems + lane * 8;
-    const int64_t page_stride = (int64_t)n_kv_heads * kSumElems;
-    float my_score = 0.f;                                // score of page warp_base + lane, gathered below
-
+    const int cta_pages = min(pages_per_cta, pl.n_pages - cta_page0);
+    const int n_wc_cta = (cta_pages + kSelPagesPerWarp - 1) / kSelPagesPerWarp;
+    const int n_wc = n_wc_cta > warp ? (n_wc_cta - warp + kSelWarps - 1) / kSelWarps : 0;   // warp-chunks of this warp
+    float *ws = scores_ws + ((int64_t)seq * n_kv_heads + g) * max_pages;
+    const uint4 *sum16 = reinterpret_cast<const uint4 *>(summaries);     // summaries in 16-byte units: 32 per (page, head)
 #pragma unroll 1
-    for (int b0 = 0; b0 < kSelPagesPerWarp; b0 += kSelBatch) {
-        const uint32_t bm = (cand_mask >> b0) & ((1u << kSelBatch) - 1u);
-        if (bm == 0) continue;                           // warp-uniform
-        uint4 v[kSelBatch];
-#pragma unroll
-        for (int j = 0; j < kSelBatch; ++j) {            // all loads of the batch first
-            const int phys = __shfl_sync(0xffffffffu, my_phys, b0 + j);
-            v[j] = (bm >> j) & 1u ? ldg_stream16(sum_g + phys * page_stride) : make_uint4(0u, 0u, 0u, 0u);
-        }
-        float a[kSelBatch];
-#pragma unroll
-        for (int j = 0; j < kSelBatch; ++j) a[j] = dot8(qr, v[j], 0.f);
-        // transpose-reduce: after the three halving steps lane l holds page j = 4*b4 + 2*b3 + b2 (bits of l),
-        // summed over the lanes that differ from l in bits 4, 3, 2; two more butterflies finish the sum.
-        static_assert(kSelBatch == 8, "transpose-reduce is written for 8 pages per batch");
+    for (int i = 0; i < n_wc; ++i) {
+        const int my_page = cta_page0 + (warp + i * kSelWarps) * kSelPagesPerWarp + lane;
+        const bool my_cand = my_page < pl.n_pages && !pl.forced(my_page);
+        const uint32_t cand_mask = __ballot_sync(0xffffffffu, my_cand);  // bit j: page chunk base + j is a candidate
+        // offset of this lane's page summary in 16-byte units (< 2^32: up to 64 GiB of summaries)
+        uint32_t my_off16 = ((uint32_t)phys_cur * (uint32_t)n_kv_heads + (uint32_t)g) * 32u;
+        // Pages that are not candidates (forced, or past the end) read the first candidate's summary instead (an L2
+        // hit) and their score is never stored: every load of a batch is then unconditional, which keeps the loads
+        // independent of one another (a predicated load is compiled as load-to-temporary + copy, which serialises).
         {
+            const uint32_t safe = __shfl_sync(0xffffffffu, my_off16, cand_mask ? __ffs(cand_mask) - 1 : 0);
+            if (!my_cand) my_off16 = safe;
+        }
+        phys_cur = phys_nxt;                             // prefetch the table entries of the warp-chunk after next
+        {
+            const int p2 = my_page + 2 * kSelCtaPagesMin;
+            phys_nxt = (i + 2 < n_wc && p2 < pl.n_pages) ? __ldg(pt + p2) : 0;
+        }
+        float my_score = 0.f;                            // score of page chunk base + lane, gathered below
+#pragma unroll 1
+        for (int b0 = 0; b0 < kSelPagesPerWarp; b0 += kSelBatch) {
+            const uint32_t bm = (cand_mask >> b0) & ((1u << kSelBatch) - 1u);
+            if (bm == 0) continue;                       // warp-uniform
+            uint4 v[kSelBatch];
+#pragma unroll
+            for (int j = 0; j < kSelBatch; ++j) {        // all loads of the batch first
+                const uint32_t off = __shfl_sync(0xffffffffu, my_off16, b0 + j) + lane;
+                v[j] = ldg_stream16(sum16 + off);
+            }
+            float a[kSelBatch];
+#pragma unroll
+            for (int j = 0; j < kSelBatch; ++j) a[j] = dot8(qr, v[j], 0.f);
+            // transpose-reduce: after the three halving steps lane l holds page j = 4*b4 + 2*b3 + b2 (bits of l),
+            // summed over the lanes that differ from l in bits 4, 3, 2; two more butterflies finish the sum.
+            static_assert(kSelBatch == 8, "transpose-reduce is written for 8 pages per batch");
             const bool hi = lane & 16;
             float k0 = hi ? a[4] : a[0], k1 = hi ? a[5] : a[1], k2 = hi ? a[6] : a[2], k3 = hi ? a[7] : a[3];
             float s0 = hi ? a[0] : a[4], s1 = hi ? a[1] : a[5], s2 = hi ? a[2] : a[6], s3 = hi ? a[3] : a[7];
@@ -170,19 +193,17 @@ select_kernel(const uint16_t *__restrict__ q, const uint16_t *__restrict__ summa
             z += __shfl_xor_sync(0xffffffffu, y, 4);
             z += __shfl_xor_sync(0xffffffffu, z, 2);
             z += __shfl_xor_sync(0xffffffffu, z, 1);
-            // lane l now holds the score of batch page j(l) = ((l>>4)&1)*4 + ((l>>3)&1)*2 + ((l>>2)&1);
-            // hand it to the lane that owns that page's table entry (lane b0 + j): source lane for j is
-            // 16*(j>>2) + 8*((j>>1)&1) + 4*(j&1).
+            // lane l now holds the score of batch page j(l) = ((l>>4)&1)*4 + ((l>>3)&1)*2 + ((l>>2)&1); hand it to
+            // the lane that owns that page's table entry (lane b0 + j): source lane for j is 16*(j>>2) + 8*((j>>1)&1) + 4*(j&1).
             const int j = lane - b0;
             const int src = ((j >> 2) & 1) * 16 + ((j >> 1) & 1) * 8 + (j & 1) * 4;
             const float got = __shfl_sync(0xffffffffu, z, src & 31);
             if (j >= 0 && j < kSelBatch) my_score = got;
         }
-    }
-    float *ws = scores_ws + ((int64_t)seq * n_kv_heads + g) * max_pages;
-    if (my_cand) {                                       // one coalesced 128-byte store per warp
-        ws[my_page] = my_score;
-        if (scores_dbg) scores_dbg[((int64_t)seq * n_kv_heads + g) * max_pages + my_page] = my_score;
+        if (my_cand) {                                   // one coalesced 128-byte store per warp
+            ws[my_page] = my_score;
+            if (scores_dbg) scores_dbg[((int64_t)seq * n_kv_heads + g) * max_pages + my_page] = my_score;
+        }
     }
 
     // ------------------------------------------------ last CTA of this (sequence, kv-head)? --------
