@@ -114,14 +114,17 @@ int sparrow_select(const void *q, const void *summaries, const int32_t *page_tab
 /* ---- a6 + a7: split-K flash-decode over the selected pages, log-sum-exp merge ---------------------
  * out[i][h] = softmax_t(sm_scale * q[i][h].K_t) V_t over tokens t < L of the pages sel_pages[i][h/r][0..sel_count[i]),
  * gathered through page_table; fp32 accumulation, bf16 output; lse (optional, may be NULL) = ln sum exp.
- * workspace: sparrow_decode_workspace_bytes(shape, max_sel) bytes, contents irrelevant. */
+ * workspace: sparrow_decode_workspace_bytes(shape, max_sel) bytes, ZERO-INITIALISED once by the caller (it
+ * holds the split-K arrival counters; the kernel restores the zeros it uses, so it can be reused call
+ * after call, but not by two calls in flight at the same time).  n_seq <= 8192.  The merge of the splits
+ * is fused into the same launch (one kernel per call). */
 int sparrow_sparse_decode(const void *q, const void *k_cache, const void *v_cache, const int32_t *page_table,
                           const int32_t *seq_lens, const int32_t *sel_pages, int32_t max_sel,
                           const int32_t *sel_count, void *out, float *lse, float sm_scale,
                           void *workspace, size_t workspace_bytes, const sparrow_shape_t *shape, void *stream);
 
 /* ---- a8: dense decode = the same kernels with B(L) = L (all ceil(L/16) pages) ---
- * workspace: sparrow_decode_workspace_bytes(shape, 0) bytes. */
+ * workspace: sparrow_decode_workspace_bytes(shape, 0) bytes, zero-initialised once like the sparse entry's. */
 int sparrow_dense_decode(const void *q, const void *k_cache, const void *v_cache, const int32_t *page_table,
                          const int32_t *seq_lens, void *out, float *lse, float sm_scale,
                          void *workspace, size_t workspace_bytes, const sparrow_shape_t *shape, void *stream);

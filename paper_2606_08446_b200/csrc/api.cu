@@ -81,32 +81,19 @@ int to_dev_sched(const sparrow_schedule_t *in, SchedDev *out)
     return SPARROW_OK;
 }
 
-// Pages of the list that one CTA (= one split) handles.  Larger chunks amortise the per-CTA prologue and the
-// partial write; smaller ones give enough CTAs to fill 148 SMs x 2 resident CTAs for several waves.
-int pick_chunk_pages(int64_t n_units, int max_cnt)
-{
-    const int64_t want = 4 * 2 * kNumSmsB200;
-    for (int c = kMaxChunkPages; c > kDecWarps; c >>= 1) {
-        const int64_t items = n_units * ((max_cnt + c - 1) / c);
-        if (items >= want) return c;
-    }
-    return kDecWarps;
-}
-
+// Decode workspace: fp32 partial slots (one per (unit, covering warp) pair, indexed unit + warp), their (m, l)
+// pairs, and one arrival counter per (sequence, kv-head) unit (zero between calls).
 struct DecodeGeom {
-    int max_cnt, chunk, n_splits;
-    size_t bytes_o, bytes_ml;
+    size_t bytes_o, bytes_ml, bytes_ctr;
 };
-DecodeGeom decode_geom(const sparrow_shape_t *s, int max_sel)
+DecodeGeom decode_geom(const sparrow_shape_t *s)
 {
     DecodeGeom gm;
-    gm.max_cnt = max_sel > 0 ? (max_sel < s->max_pages_per_seq ? max_sel : s->max_pages_per_seq) : s->max_pages_per_seq;
-    const int64_t units = (int64_t)s->n_seq * s->n_kv_heads;
-    gm.chunk = pick_chunk_pages(units, gm.max_cnt);
-    gm.n_splits = (gm.max_cnt + gm.chunk - 1) / gm.chunk;
-    const size_t rows = (size_t)units * gm.n_splits * (s->n_q_heads / s->n_kv_heads);
+    const size_t units = (size_t)s->n_seq * s->n_kv_heads;
+    const size_t rows = (units + (size_t)kDecGrid * kDecWarps) * (s->n_q_heads / s->n_kv_heads);
     gm.bytes_o = (rows * kDim * sizeof(float) + 255) & ~(size_t)255;
     gm.bytes_ml = (rows * 2 * sizeof(float) + 255) & ~(size_t)255;
+    gm.bytes_ctr = (units * sizeof(int32_t) + 255) & ~(size_t)255;
     return gm;
 }
 
@@ -118,29 +105,33 @@ int launch_decode(const void *q, const void *k_cache, const void *v_cache, const
                   void *out, float *lse, float sm_scale, void *workspace, size_t workspace_bytes,
                   const sparrow_shape_t *s, cudaStream_t st)
 {
-    const DecodeGeom gm = decode_geom(s, kDense ? 0 : max_sel);
-    if (workspace_bytes < gm.bytes_o + gm.bytes_ml) return SPARROW_ERR_WORKSPACE_TOO_SMALL;
+    const DecodeGeom gm = decode_geom(s);
+    if (workspace_bytes < gm.bytes_ctr + gm.bytes_o + gm.bytes_ml) return SPARROW_ERR_WORKSPACE_TOO_SMALL;
+    if (s->n_seq > kDecMaxSeq) return SPARROW_ERR_UNSUPPORTED;
+    {   // flat tile positions are 32-bit
+        const int64_t max_cnt = kDense ? s->max_pages_per_seq : (max_sel < s->max_pages_per_seq ? max_sel : s->max_pages_per_seq);
+        if ((int64_t)s->n_seq * max_cnt * s->n_kv_heads >= (1LL << 31) || s->n_phys_pages * s->n_kv_heads >= (1LL << 31))
+            return SPARROW_ERR_UNSUPPORTED;
+    }
     if (s->n_seq == 0) return SPARROW_OK;
-    float *ws_o = reinterpret_cast<float *>(workspace);
-    float *ws_ml = reinterpret_cast<float *>(reinterpret_cast<uint8_t *>(workspace) + gm.bytes_o);
+    int32_t *counters = reinterpret_cast<int32_t *>(workspace);
+    float *ws_o = reinterpret_cast<float *>(reinterpret_cast<uint8_t *>(workspace) + gm.bytes_ctr);
+    float *ws_ml = reinterpret_cast<float *>(reinterpret_cast<uint8_t *>(workspace) + gm.bytes_ctr + gm.bytes_o);
 
+    constexpr int kSmemMax = kDecRingBytes + ((kDecMaxSeq + 1) * 4 + 15) / 16 * 16;
     static bool attr_done[2] = {false, false};
     if (!attr_done[kDense]) {
-        cudaError_t e = cudaFuncSetAttribute(decode_kernel<kDense>, cudaFuncAttributeMaxDynamicSharedMemorySize, kDecSmemBytes);
+        cudaError_t e = cudaFuncSetAttribute(decode_kernel<kDense>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemMax);
         if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(decode_kernel)");
         attr_done[kDense] = true;
     }
     const float scale_log2 = sm_scale * 1.4426950408889634f;
-    dim3 grid(gm.n_splits, s->n_kv_heads, s->n_seq);
-    decode_kernel<kDense><<<grid, kDecThreads, kDecSmemBytes, st>>>(
+    const int smem = kDecRingBytes + ((s->n_seq + 1) * 4 + 15) / 16 * 16;
+    decode_kernel<kDense><<<kDecGrid, kDecThreads, smem, st>>>(
         (const uint16_t *)q, (const uint16_t *)k_cache, (const uint16_t *)v_cache, page_table, seq_lens, sel_pages,
-        max_sel, sel_count, ws_o, ws_ml, gm.chunk, gm.n_splits, scale_log2, s->n_q_heads, s->n_kv_heads,
-        s->max_pages_per_seq);
+        max_sel, sel_count, ws_o, ws_ml, counters, (uint16_t *)out, lse, scale_log2, s->n_seq, s->n_q_heads,
+        s->n_kv_heads, s->max_pages_per_seq);
     SPARROW_CHECK_LAUNCH("decode_kernel");
-    dim3 mgrid(s->n_q_heads, s->n_seq);
-    merge_kernel<kDense><<<mgrid, kDim, 0, st>>>(ws_o, ws_ml, seq_lens, sel_count, max_sel, (uint16_t *)out, lse,
-                                                  gm.chunk, gm.n_splits, s->n_q_heads, s->n_kv_heads);
-    SPARROW_CHECK_LAUNCH("merge_kernel");
     return SPARROW_OK;
 }
 
@@ -222,8 +213,9 @@ size_t sparrow_select_workspace_bytes(const sparrow_shape_t *s)
 size_t sparrow_decode_workspace_bytes(const sparrow_shape_t *s, int32_t max_sel)
 {
     if (check_shape(s) != SPARROW_OK) return 0;
-    const DecodeGeom gm = decode_geom(s, max_sel);
-    return gm.bytes_o + gm.bytes_ml;
+    (void)max_sel;                                           // the stream-K partition needs no per-list sizing
+    const DecodeGeom gm = decode_geom(s);
+    return gm.bytes_ctr + gm.bytes_o + gm.bytes_ml;
 }
 
 int64_t sparrow_budget_tokens(const sparrow_schedule_t *sched, int64_t L)

@@ -29,7 +29,7 @@ class SparrowEngine:
         self.select_ws = torch.zeros((B.sparrow_select_workspace_bytes(self.shape),), dtype=torch.uint8, device=dev)
         self.scores = (torch.full((wl.n_seq, wl.Hkv, wl.max_pages), float("nan"), dtype=torch.float32, device=dev)
                        if want_scores else None)
-        self.dense_ws = torch.empty((B.sparrow_decode_workspace_bytes(self.shape, 0),), dtype=torch.uint8, device=dev)
+        self.dense_ws = torch.zeros((B.sparrow_decode_workspace_bytes(self.shape, 0),), dtype=torch.uint8, device=dev)
 
     def set_schedule(self, spec: dict):
         dev = self.wl.q.device
@@ -38,7 +38,7 @@ class SparrowEngine:
         max_len = int(self.wl.seq_lens.max().item())
         self.max_sel = max(1, B.sparrow_max_sel_pages(self.sched, max_len))
         self.sel_pages = torch.full((self.wl.n_seq, self.wl.Hkv, self.max_sel), -1, dtype=torch.int32, device=dev)
-        self.sparse_ws = torch.empty((B.sparrow_decode_workspace_bytes(self.shape, self.max_sel),), dtype=torch.uint8, device=dev)
+        self.sparse_ws = torch.zeros((B.sparrow_decode_workspace_bytes(self.shape, self.max_sel),), dtype=torch.uint8, device=dev)
 
     # ---- a1
     def summarize(self, page_ids: Optional[torch.Tensor], n_valid: Optional[torch.Tensor], n_update: Optional[int] = None, stream=None):
