@@ -81,19 +81,22 @@ int to_dev_sched(const sparrow_schedule_t *in, SchedDev *out)
     return SPARROW_OK;
 }
 
-// Decode workspace: fp32 partial slots (one per (unit, covering warp) pair, indexed unit + warp), their (m, l)
-// pairs, and one arrival counter per (sequence, kv-head) unit (zero between calls).
+// Decode workspace: arrival counters (one per (sequence, kv-head) unit) + the two counters of the range scheduler
+// (all zero between calls), then the fp32 partial slots (indexed unit + range index) and their (m, l) pairs.
 struct DecodeGeom {
     size_t bytes_o, bytes_ml, bytes_ctr;
+    int max_rounds;
 };
-DecodeGeom decode_geom(const sparrow_shape_t *s)
+DecodeGeom decode_geom(const sparrow_shape_t *s, int32_t max_sel /* 0 = dense */)
 {
     DecodeGeom gm;
     const size_t units = (size_t)s->n_seq * s->n_kv_heads;
-    const size_t rows = (units + (size_t)kDecGrid * kDecWarps) * (s->n_q_heads / s->n_kv_heads);
+    const int64_t max_cnt = (max_sel > 0 && max_sel < s->max_pages_per_seq) ? max_sel : s->max_pages_per_seq;
+    gm.max_rounds = decode_max_rounds((int64_t)units * max_cnt);
+    const size_t rows = (units + (size_t)kDecW * gm.max_rounds) * (s->n_q_heads / s->n_kv_heads);
     gm.bytes_o = (rows * kDim * sizeof(float) + 255) & ~(size_t)255;
     gm.bytes_ml = (rows * 2 * sizeof(float) + 255) & ~(size_t)255;
-    gm.bytes_ctr = (units * sizeof(int32_t) + 255) & ~(size_t)255;
+    gm.bytes_ctr = ((units + 2) * sizeof(int32_t) + 255) & ~(size_t)255;
     return gm;
 }
 
@@ -105,7 +108,7 @@ int launch_decode(const void *q, const void *k_cache, const void *v_cache, const
                   void *out, float *lse, float sm_scale, void *workspace, size_t workspace_bytes,
                   const sparrow_shape_t *s, cudaStream_t st)
 {
-    const DecodeGeom gm = decode_geom(s);
+    const DecodeGeom gm = decode_geom(s, kDense ? 0 : max_sel);
     if (workspace_bytes < gm.bytes_ctr + gm.bytes_o + gm.bytes_ml) return SPARROW_ERR_WORKSPACE_TOO_SMALL;
     if (s->n_seq > kDecMaxSeq) return SPARROW_ERR_UNSUPPORTED;
     {   // flat tile positions are 32-bit
@@ -129,8 +132,8 @@ int launch_decode(const void *q, const void *k_cache, const void *v_cache, const
     const int smem = kDecRingBytes + ((s->n_seq + 1) * 4 + 15) / 16 * 16;
     decode_kernel<kDense><<<kDecGrid, kDecThreads, smem, st>>>(
         (const uint16_t *)q, (const uint16_t *)k_cache, (const uint16_t *)v_cache, page_table, seq_lens, sel_pages,
-        max_sel, sel_count, ws_o, ws_ml, counters, (uint16_t *)out, lse, scale_log2, s->n_seq, s->n_q_heads,
-        s->n_kv_heads, s->max_pages_per_seq);
+        max_sel, sel_count, ws_o, ws_ml, counters, counters + (size_t)s->n_seq * s->n_kv_heads, (uint16_t *)out, lse,
+        scale_log2, s->n_seq, s->n_q_heads, s->n_kv_heads, s->max_pages_per_seq, gm.max_rounds);
     SPARROW_CHECK_LAUNCH("decode_kernel");
     return SPARROW_OK;
 }
@@ -213,8 +216,7 @@ size_t sparrow_select_workspace_bytes(const sparrow_shape_t *s)
 size_t sparrow_decode_workspace_bytes(const sparrow_shape_t *s, int32_t max_sel)
 {
     if (check_shape(s) != SPARROW_OK) return 0;
-    (void)max_sel;                                           // the stream-K partition needs no per-list sizing
-    const DecodeGeom gm = decode_geom(s);
+    const DecodeGeom gm = decode_geom(s, max_sel);
     return gm.bytes_ctr + gm.bytes_o + gm.bytes_ml;
 }
 
