@@ -130,10 +130,15 @@ int launch_decode(const void *q, const void *k_cache, const void *v_cache, const
     }
     const float scale_log2 = sm_scale * 1.4426950408889634f;
     const int smem = kDecRingBytes + ((s->n_seq + 1) * 4 + 15) / 16 * 16;
-    decode_kernel<kDense><<<kDecGrid, kDecThreads, smem, st>>>(
-        (const uint16_t *)q, (const uint16_t *)k_cache, (const uint16_t *)v_cache, page_table, seq_lens, sel_pages,
-        max_sel, sel_count, ws_o, ws_ml, counters, counters + (size_t)s->n_seq * s->n_kv_heads, (uint16_t *)out, lse,
-        scale_log2, s->n_seq, s->n_q_heads, s->n_kv_heads, s->max_pages_per_seq, gm.max_rounds);
+    DecodeArgs A;
+    A.q = (const uint16_t *)q; A.k_cache = (const uint16_t *)k_cache; A.v_cache = (const uint16_t *)v_cache;
+    A.page_table = page_table; A.seq_lens = seq_lens; A.sel_pages = sel_pages; A.sel_count = sel_count;
+    A.max_sel = max_sel; A.ws_o = ws_o; A.ws_ml = ws_ml; A.counters = counters;
+    A.sched_ctr = counters + (size_t)s->n_seq * s->n_kv_heads;
+    A.out = (uint16_t *)out; A.lse = lse; A.scale_log2 = scale_log2;
+    A.n_seq = s->n_seq; A.n_q_heads = s->n_q_heads; A.n_kv_heads = s->n_kv_heads; A.max_pages = s->max_pages_per_seq;
+    A.ready = nullptr;
+    decode_kernel<kDense><<<kDecGrid, kDecThreads, smem, st>>>(A, gm.max_rounds);
     SPARROW_CHECK_LAUNCH("decode_kernel");
     return SPARROW_OK;
 }

@@ -39,7 +39,7 @@ namespace sparrow {
 #define SPARROW_DEC_WARPS 8
 #endif
 #ifndef SPARROW_DEC_STAGES
-#define SPARROW_DEC_STAGES 3
+#define SPARROW_DEC_STAGES 2
 #endif
 #ifndef SPARROW_DEC_MAXSEQ
 #define SPARROW_DEC_MAXSEQ 8192
@@ -48,7 +48,7 @@ constexpr int kDecWarps = SPARROW_DEC_WARPS;
 constexpr int kDecThreads = kDecWarps * 32;
 constexpr int kDecStages = SPARROW_DEC_STAGES;                                   // per-warp ring depth
 constexpr int kStageBytes = 2 * kTileBytes;                     // K tile + V tile = 8 KiB
-constexpr int kDecRingBytes = kDecWarps * kDecStages * kStageBytes;   // 192 KiB -> one CTA per SM
+constexpr int kDecRingBytes = kDecWarps * kDecStages * kStageBytes;   // 128 KiB (2 stages measured as fast as 3; one CTA per SM by registers)
 constexpr int kMaxGroup = 8;                                    // r <= 8 (rows 0..7 of the m16 tile)
 constexpr int kDecMaxSeq = SPARROW_DEC_MAXSEQ;                                // prefix table of the batch lives in shared memory
 constexpr int kDecGrid = 148;                                   // persistent: one CTA per B200 SM
@@ -98,6 +98,16 @@ __host__ inline int decode_max_rounds(int64_t t_max)
     return rounds < kDecMaxRounds ? rounds : kDecMaxRounds;
 }
 
+__device__ __forceinline__ int ld_acquire(const int32_t *p)
+{
+    int v;
+    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release(int32_t *p, int v)
+{
+    asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void *src)
 {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
@@ -145,56 +155,40 @@ __device__ __forceinline__ uint32_t tile_off(int t, int c)
 
 constexpr int kMetaFirst = 1 << 8, kMetaLast = 1 << 9;
 
-template <bool kDense>
-__global__ void __launch_bounds__(kDecThreads, 1)
-decode_kernel(const uint16_t *__restrict__ q, const uint16_t *__restrict__ k_cache, const uint16_t *__restrict__ v_cache,
-              const int32_t *__restrict__ page_table, const int32_t *__restrict__ seq_lens,
-              const int32_t *__restrict__ sel_pages, int max_sel, const int32_t *__restrict__ sel_count,
-              float *__restrict__ ws_o, float *__restrict__ ws_ml, int32_t *__restrict__ counters,
-              int32_t *__restrict__ sched_ctr, uint16_t *__restrict__ out, float *__restrict__ lse,
-              float scale_log2, int n_seq, int n_q_heads, int n_kv_heads, int max_pages, int max_rounds)
-{
-    extern __shared__ __align__(1024) uint8_t smem[];
-    int32_t *s_prefix = reinterpret_cast<int32_t *>(smem + kDecRingBytes);     // [n_seq + 1] list entries before sequence i
-    __shared__ int s_scan[kDecWarps];
-    __shared__ DecSchedule s_sched;
+// Everything the streaming part of the decode needs (kernel arguments, passed on unchanged).
+struct DecodeArgs {
+    const uint16_t *q, *k_cache, *v_cache;
+    const int32_t *page_table, *seq_lens, *sel_pages, *sel_count;
+    int max_sel;
+    float *ws_o, *ws_ml;
+    int32_t *counters, *sched_ctr;
+    uint16_t *out;
+    float *lse;
+    float scale_log2;
+    int n_seq, n_q_heads, n_kv_heads, max_pages;
+    const int32_t *ready;        // fused step only: per-unit flag, non-zero once the unit's page list is written
+};
 
+// One warp's share of the decode: streams its ranges of the flat tile stream (s_prefix = list entries before
+// sequence i, s_sched = the range table, both in shared memory) through its K/V ring at `ring`.
+// kFused: the page lists are being written by the same launch (step.cuh); a look-up waits for its unit's flag.
+template <bool kDense, bool kFused>
+__device__ __forceinline__ void decode_warp_stream(const DecodeArgs &A, const int32_t *s_prefix, const DecSchedule &s_sched,
+                                                   uint8_t *ring)
+{
+    const uint16_t *__restrict__ q = A.q, *__restrict__ k_cache = A.k_cache, *__restrict__ v_cache = A.v_cache;
+    const int32_t *__restrict__ page_table = A.page_table, *__restrict__ seq_lens = A.seq_lens;
+    const int32_t *__restrict__ sel_pages = A.sel_pages;
+    float *__restrict__ ws_o = A.ws_o, *__restrict__ ws_ml = A.ws_ml;
+    int32_t *__restrict__ counters = A.counters, *__restrict__ sched_ctr = A.sched_ctr;
+    uint16_t *__restrict__ out = A.out;
+    float *__restrict__ lse = A.lse;
+    const float scale_log2 = A.scale_log2;
+    const int max_sel = A.max_sel, n_seq = A.n_seq, n_q_heads = A.n_q_heads, n_kv_heads = A.n_kv_heads, max_pages = A.max_pages;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int r = n_q_heads / n_kv_heads;
     constexpr uint32_t kFull = 0xffffffffu;
 
-    // ---- prologue: list length of every sequence -> exclusive prefix in shared memory; the range table ----
-    {
-        const int per = (n_seq + kDecThreads - 1) / kDecThreads;
-        const int s0 = min(tid * per, n_seq), s1 = min(s0 + per, n_seq);
-        auto count_of = [&](int s) {
-            int c;
-            if (kDense) c = (__ldg(seq_lens + s) + kPage - 1) / kPage;
-            else { c = __ldg(sel_count + s); c = c < max_sel ? c : max_sel; }
-            return c > 0 ? c : 0;
-        };
-        int sum = 0;
-        for (int s = s0; s < s1; ++s) sum += count_of(s);
-        int inc = sum;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const int t = __shfl_up_sync(kFull, inc, o);
-            if (lane >= o) inc += t;
-        }
-        if (lane == 31) s_scan[warp] = inc;
-        __syncthreads();
-        int run = inc - sum;
-        for (int w = 0; w < warp; ++w) run += s_scan[w];
-        for (int s = s0; s < s1; ++s) {
-            s_prefix[s] = run;
-            run += count_of(s);
-        }
-        if (tid == kDecThreads - 1) {
-            s_prefix[n_seq] = run;
-            decode_schedule(run * n_kv_heads, max_rounds, s_sched);
-        }
-        __syncthreads();
-    }
     const int T = s_prefix[n_seq] * n_kv_heads;                  // tiles of the whole batch
     const int NR = s_sched.total;                                // ranges of the whole batch
     const int gw = blockIdx.x * kDecWarps + warp;
@@ -236,7 +230,12 @@ decode_kernel(const uint16_t *__restrict__ q, const uint16_t *__restrict__ k_cac
             m.seq = seq;
             m.unit = seq * n_kv_heads + g;
             m.info = ((i == 0 || p == ra) ? kMetaFirst : 0) | ((i == c - 1 || p == rb - 1) ? kMetaLast : 0);
-            m.logical = kDense ? i : __ldg(sel_pages + ((int64_t)m.unit) * max_sel + i);
+            if (kFused) {                                        // the list is written by this launch: wait for it
+                while (ld_acquire(A.ready + m.unit) == 0) __nanosleep(64);
+                m.logical = __ldcg(sel_pages + ((int64_t)m.unit) * max_sel + i);
+            } else {
+                m.logical = kDense ? i : __ldg(sel_pages + ((int64_t)m.unit) * max_sel + i);
+            }
             m.len = __ldg(seq_lens + seq);
         }
     };
@@ -297,7 +296,7 @@ decode_kernel(const uint16_t *__restrict__ q, const uint16_t *__restrict__ k_cac
         if (nxt_stage < 3 && target >= 3) { stage_c(nxt); nxt_stage = 3; }
     };
 
-    const uint32_t ring_u32 = smem_u32(smem + warp * (kDecStages * kStageBytes));
+    const uint32_t ring_u32 = smem_u32(ring);
     auto issue = [&](int tile, int stage) {       // copy one K tile and one V tile into a ring stage
         const uint8_t *ksrc = reinterpret_cast<const uint8_t *>(k_cache + (int64_t)tile * kTileElems);
         const uint8_t *vsrc = reinterpret_cast<const uint8_t *>(v_cache + (int64_t)tile * kTileElems);
@@ -550,12 +549,63 @@ decode_kernel(const uint16_t *__restrict__ q, const uint16_t *__restrict__ k_cac
         else { nn = 0; nxt_stage = 3; }
     }
     cp_async_wait<0>();
+}
+
+template <bool kDense>
+__global__ void __launch_bounds__(kDecThreads, 1)
+decode_kernel(const DecodeArgs A, int max_rounds)
+{
+    extern __shared__ __align__(1024) uint8_t smem[];
+    int32_t *s_prefix = reinterpret_cast<int32_t *>(smem + kDecRingBytes);     // [n_seq + 1] list entries before sequence i
+    __shared__ int s_scan[kDecWarps];
+    __shared__ DecSchedule s_sched;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int n_seq = A.n_seq, n_kv_heads = A.n_kv_heads, max_sel = A.max_sel;
+    const int32_t *__restrict__ seq_lens = A.seq_lens;
+    constexpr uint32_t kFull = 0xffffffffu;
+
+
+
+    // ---- prologue: list length of every sequence -> exclusive prefix in shared memory; the range table ----
+    {
+        const int per = (n_seq + kDecThreads - 1) / kDecThreads;
+        const int s0 = min(tid * per, n_seq), s1 = min(s0 + per, n_seq);
+        auto count_of = [&](int s) {
+            int c;
+            if (kDense) c = (__ldg(seq_lens + s) + kPage - 1) / kPage;
+            else { c = __ldg(A.sel_count + s); c = c < max_sel ? c : max_sel; }
+            return c > 0 ? c : 0;
+        };
+        int sum = 0;
+        for (int s = s0; s < s1; ++s) sum += count_of(s);
+        int inc = sum;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(kFull, inc, o);
+            if (lane >= o) inc += t;
+        }
+        if (lane == 31) s_scan[warp] = inc;
+        __syncthreads();
+        int run = inc - sum;
+        for (int w = 0; w < warp; ++w) run += s_scan[w];
+        for (int s = s0; s < s1; ++s) {
+            s_prefix[s] = run;
+            run += count_of(s);
+        }
+        if (tid == kDecThreads - 1) {
+            s_prefix[n_seq] = run;
+            decode_schedule(run * n_kv_heads, max_rounds, s_sched);
+        }
+        __syncthreads();
+    }
+    decode_warp_stream<kDense, false>(A, s_prefix, s_sched, smem + warp * (kDecStages * kStageBytes));
     // ---- the last warp out restores the scheduler's zeros for the next call ----
     if (lane == 0) {
-        const int done = atomicAdd(sched_ctr + 1, 1);
+        const int done = atomicAdd(A.sched_ctr + 1, 1);
         if (done == kDecW - 1) {
-            sched_ctr[0] = 0;
-            sched_ctr[1] = 0;
+            A.sched_ctr[0] = 0;
+            A.sched_ctr[1] = 0;
         }
     }
 }
