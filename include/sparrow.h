@@ -129,10 +129,26 @@ int sparrow_dense_decode(const void *q, const void *k_cache, const void *v_cache
                          const int32_t *seq_lens, void *out, float *lse, float sm_scale,
                          void *workspace, size_t workspace_bytes, const sparrow_shape_t *shape, void *stream);
 
+/* ---- a2..a7 fused: the whole sparse step in ONE persistent launch ----------------------------------
+ * Same results as sparrow_select followed by sparrow_sparse_decode on the same arguments (the selected lists
+ * and sel_count are written too), but the summary stream, the per-unit top-k and the K/V stream share one
+ * cooperative launch: every warp moves from scoring to decoding as soon as its share is done, and a decode
+ * look-up waits only for the one (sequence, kv-head) list it needs.  Falls back to the two launches when the
+ * shape does not fit the fused kernel's shared memory (roughly n_seq + max_pages_per_seq/2 > 12000) or the device
+ * cannot keep 148 CTAs resident.  sched->kind == DENSE is allowed (identity lists).  workspace:
+ * sparrow_step_workspace_bytes(shape, max_sel) bytes, ZERO-INITIALISED once by the caller, restored to zero by
+ * the call like the other workspaces; not shareable by two calls in flight. */
+int sparrow_step(const void *q, const void *k_cache, const void *v_cache, const void *summaries,
+                 const int32_t *page_table, const int32_t *seq_lens, const sparrow_schedule_t *sched,
+                 int32_t *sel_pages, int32_t max_sel, int32_t *sel_count, float *scores_dbg,
+                 void *out, float *lse, float sm_scale, void *workspace, size_t workspace_bytes,
+                 const sparrow_shape_t *shape, void *stream);
+size_t sparrow_step_workspace_bytes(const sparrow_shape_t *shape, int32_t max_sel);
+
 /* ---- whole step through HOST buffers (the end-to-end measurement path) ----------------------------
  * Copies this step's inputs from host memory (q_host [n][Hq][128] bf16, seq_lens_host [n] int32; pinned
  * memory makes the copies asynchronous), runs summarize (n_update pages, page_ids/n_valid are HOST arrays,
- * n_update may be 0) -> select -> sparse decode (or the dense path when sched->kind == DENSE) on `stream`,
+ * n_update may be 0) -> the fused select + sparse decode step (or the dense path when sched->kind == DENSE) on `stream`,
  * copies out back to out_host [n][Hq][128] bf16 and WAITS for the stream.  The K/V pools, summaries and
  * page_table are the resident cache state and stay device pointers.  `scratch` is a device buffer of at
  * least sparrow_step_scratch_bytes(shape, max_sel) bytes, zero-initialised once by the caller. */

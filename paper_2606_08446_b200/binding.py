@@ -61,6 +61,8 @@ _SIGS = {
     "sparrow_select": (C.c_int, [_vp, _vp, _vp, _vp, _SCH, _vp, _i32, _vp, _vp, _vp, _sz, _SHP, _vp]),
     "sparrow_sparse_decode": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _i32, _vp, _vp, _vp, _f, _vp, _sz, _SHP, _vp]),
     "sparrow_dense_decode": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _f, _vp, _sz, _SHP, _vp]),
+    "sparrow_step": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _SCH, _vp, _i32, _vp, _vp, _vp, _vp, _f, _vp, _sz, _SHP, _vp]),
+    "sparrow_step_workspace_bytes": (_sz, [_SHP, _i32]),
     "sparrow_step_host": (C.c_int, [_vp, _vp, _vp, _vp, _i64, _vp, _vp, _vp, _vp, _SCH, _i32, _f, _vp, _vp, _sz, _SHP, _vp]),
     "sparrow_select_workspace_bytes": (_sz, [_SHP]),
     "sparrow_decode_workspace_bytes": (_sz, [_SHP, _i32]),
@@ -124,6 +126,10 @@ def sparrow_decode_workspace_bytes(shape, max_sel: int) -> int:
     return _lib.sparrow_decode_workspace_bytes(_by(shape), max_sel)
 
 
+def sparrow_step_workspace_bytes(shape, max_sel: int) -> int:
+    return _lib.sparrow_step_workspace_bytes(_by(shape), max_sel)
+
+
 def sparrow_step_scratch_bytes(shape, max_sel: int) -> int:
     return _lib.sparrow_step_scratch_bytes(_by(shape), max_sel)
 
@@ -182,6 +188,17 @@ def sparrow_dense_decode(q, k_cache, v_cache, page_table, seq_lens, out, lse, sm
                                    0 if workspace is None else workspace.numel() * workspace.element_size(), _by(shape), _stream(stream))
     if check:
         _check(rc, "sparrow_dense_decode")
+    return rc
+
+
+def sparrow_step(q, k_cache, v_cache, summaries, page_table, seq_lens, sched, sel_pages, max_sel: int, sel_count, scores_dbg,
+                 out, lse, sm_scale: float, workspace, shape, stream=None, *, check=True):
+    rc = _lib.sparrow_step(_ptr(q), _ptr(k_cache), _ptr(v_cache), _ptr(summaries), _ptr(page_table), _ptr(seq_lens), _by(sched),
+                           _ptr(sel_pages), max_sel, _ptr(sel_count), _ptr(scores_dbg), _ptr(out), _ptr(lse), sm_scale,
+                           _ptr(workspace), 0 if workspace is None else workspace.numel() * workspace.element_size(),
+                           _by(shape), _stream(stream))
+    if check:
+        _check(rc, "sparrow_step")
     return rc
 
 

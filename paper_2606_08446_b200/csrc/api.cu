@@ -6,6 +6,7 @@
 #include "common.cuh"
 #include "decode.cuh"
 #include "select.cuh"
+#include "step.cuh"
 #include "summarize.cuh"
 
 using namespace sparrow;
@@ -192,6 +193,96 @@ int select_impl(const void *q, const void *summaries, const int32_t *page_table,
     return SPARROW_OK;
 }
 
+// Workspace of the fused step: select workspace (unit counters + scores) | unit flags | decode workspace.
+struct StepGeom {
+    size_t sel_bytes, flag_bytes, dec_bytes;
+};
+StepGeom step_geom(const sparrow_shape_t *s, int32_t max_sel)
+{
+    StepGeom g;
+    const size_t units = (size_t)s->n_seq * s->n_kv_heads;
+    const size_t stride = ((size_t)s->max_pages_per_seq + 31) & ~(size_t)31;     // score rows own their 128-byte lines
+    g.sel_bytes = align256(units * sizeof(int32_t)) + align256(units * stride * sizeof(float));
+    g.flag_bytes = align256((size_t)s->n_seq * s->n_kv_heads * sizeof(int32_t));
+    g.dec_bytes = sparrow_decode_workspace_bytes(s, max_sel);
+    return g;
+}
+
+// a2-a7 in one cooperative launch (step.cuh); falls back to the select and decode launches when the shape does not
+// fit the fused kernel's shared memory or the device cannot hold the grid (still the same CUDA path, two kernels).
+int step_impl(const void *q, const void *k_cache, const void *v_cache, const void *summaries, const int32_t *page_table,
+              const int32_t *seq_lens, const SchedDev &sd, int32_t *sel_pages, int32_t max_sel, int32_t *sel_count,
+              float *scores_dbg, void *out, float *lse, float sm_scale, void *workspace, size_t workspace_bytes,
+              const sparrow_shape_t *s, cudaStream_t st)
+{
+    const StepGeom g = step_geom(s, max_sel);
+    if (workspace_bytes < g.sel_bytes + g.flag_bytes + g.dec_bytes) return SPARROW_ERR_WORKSPACE_TOO_SMALL;
+    if (s->n_seq == 0) return SPARROW_OK;
+    uint8_t *base = reinterpret_cast<uint8_t *>(workspace);
+    uint8_t *sel_ws = base, *flags = base + g.sel_bytes, *dec_ws = flags + g.flag_bytes;
+    const size_t units = (size_t)s->n_seq * s->n_kv_heads;
+    // shared memory: K/V ring | two prefix tables | top-k scratch (one per warp when that fits, else one per CTA)
+    const size_t dyn_base = (size_t)kDecRingBytes + ((2 * (size_t)(s->n_seq + 1) * 4 + 15) & ~(size_t)15);
+    const size_t keys = ((size_t)s->max_pages_per_seq + 31) & ~(size_t)31;
+    constexpr size_t kSmemBudget = 227 * 1024 - 12 * 1024;          // static shared memory and alignment slack
+    const bool per_warp = dyn_base + kDecWarps * keys * 4 <= kSmemBudget;
+    const size_t dyn = dyn_base + (per_warp ? kDecWarps : 1) * keys * 4;
+    static int fused_ok = -1;                    // -1 unknown, 0 the device cannot run the cooperative grid, 1 yes
+    bool fused = fused_ok != 0 && dyn <= kSmemBudget && s->n_seq <= kDecMaxSeq &&
+                 s->n_phys_pages * s->n_kv_heads < (1LL << 27) &&
+                 (int64_t)s->n_seq * s->max_pages_per_seq * s->n_kv_heads < (1LL << 31);
+    if (fused && fused_ok < 0) {
+        int dev = 0, coop = 0, sms = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        fused_ok = (coop && sms >= kDecGrid) ? 1 : 0;
+        fused = fused_ok == 1;
+    }
+    if (fused) {
+        static size_t dyn_set = 0;
+        if (dyn > dyn_set) {
+            cudaError_t e = cudaFuncSetAttribute(step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
+            if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(step_kernel)");
+            dyn_set = dyn;
+        }
+        const DecodeGeom gm = decode_geom(s, max_sel);
+        StepArgs S;
+        DecodeArgs &A = S.dec;
+        A.q = (const uint16_t *)q; A.k_cache = (const uint16_t *)k_cache; A.v_cache = (const uint16_t *)v_cache;
+        A.page_table = page_table; A.seq_lens = seq_lens; A.sel_pages = sel_pages; A.sel_count = sel_count;
+        A.max_sel = max_sel;
+        A.counters = reinterpret_cast<int32_t *>(dec_ws);
+        A.sched_ctr = A.counters + units;
+        A.ws_o = reinterpret_cast<float *>(dec_ws + gm.bytes_ctr);
+        A.ws_ml = reinterpret_cast<float *>(dec_ws + gm.bytes_ctr + gm.bytes_o);
+        A.out = (uint16_t *)out; A.lse = lse; A.scale_log2 = sm_scale * 1.4426950408889634f;
+        A.n_seq = s->n_seq; A.n_q_heads = s->n_q_heads; A.n_kv_heads = s->n_kv_heads; A.max_pages = s->max_pages_per_seq;
+        A.ready = reinterpret_cast<const int32_t *>(flags);
+        S.summaries = (const uint16_t *)summaries;
+        S.sel_pages = sel_pages; S.sel_count = sel_count;
+        S.sel_counters = reinterpret_cast<int32_t *>(sel_ws);
+        S.scores_ws = reinterpret_cast<float *>(sel_ws + align256(units * sizeof(int32_t)));
+        S.ws_stride = (int)(((size_t)s->max_pages_per_seq + 31) & ~(size_t)31);
+        S.scores_dbg = scores_dbg;
+        S.ready = reinterpret_cast<int32_t *>(flags);
+        S.max_rounds = gm.max_rounds;
+        S.scratch_stride = per_warp ? (int)keys : 0;
+        SchedDev sd_copy = sd;
+        void *args[] = {&S, &sd_copy};
+        cudaError_t e = cudaLaunchCooperativeKernel((const void *)step_kernel, dim3(kDecGrid), dim3(kDecThreads), args, dyn, st);
+        if (e == cudaSuccess) { ++g_launches; return SPARROW_OK; }
+        if (e != cudaErrorCooperativeLaunchTooLarge) return cuda_fail(e, "step_kernel");
+        (void)cudaGetLastError();
+        fused_ok = 0;                            // the grid cannot be co-resident here: two launches from now on
+    }
+    int rc = select_impl(q, summaries, page_table, seq_lens, sd, sel_pages, max_sel, sel_count, scores_dbg, sel_ws,
+                         g.sel_bytes, s, st);
+    if (rc) return rc;
+    return launch_decode<false>(q, k_cache, v_cache, page_table, seq_lens, sel_pages, max_sel, sel_count, out, lse, sm_scale,
+                                dec_ws, g.dec_bytes, s, st);
+}
+
 }  // namespace
 
 extern "C" {
@@ -320,8 +411,37 @@ int sparrow_dense_decode(const void *q, const void *k_cache, const void *v_cache
                                workspace, workspace_bytes, shape, (cudaStream_t)stream);
 }
 
+size_t sparrow_step_workspace_bytes(const sparrow_shape_t *s, int32_t max_sel)
+{
+    if (check_shape(s) != SPARROW_OK || max_sel <= 0) return 0;
+    const StepGeom g = step_geom(s, max_sel);
+    return g.sel_bytes + g.flag_bytes + g.dec_bytes;
+}
+
+int sparrow_step(const void *q, const void *k_cache, const void *v_cache, const void *summaries,
+                 const int32_t *page_table, const int32_t *seq_lens, const sparrow_schedule_t *sched,
+                 int32_t *sel_pages, int32_t max_sel, int32_t *sel_count, float *scores_dbg, void *out, float *lse,
+                 float sm_scale, void *workspace, size_t workspace_bytes, const sparrow_shape_t *shape, void *stream)
+{
+    g_launches = 0;
+    int rc = check_shape(shape);
+    if (rc) return rc;
+    SchedDev sd;
+    rc = to_dev_sched(sched, &sd);
+    if (rc) return rc;
+    if (!q || !k_cache || !v_cache || !summaries || !page_table || !seq_lens || !sel_pages || !sel_count || !out ||
+        !workspace || max_sel <= 0)
+        return SPARROW_ERR_INVALID_ARG;
+    if (!aligned16(q) || !aligned16(k_cache) || !aligned16(v_cache) || !aligned16(summaries) || !aligned16(out) ||
+        !aligned16(workspace))
+        return SPARROW_ERR_INVALID_ARG;
+    if (shape->max_pages_per_seq > kSelMaxPages) return SPARROW_ERR_UNSUPPORTED;
+    return step_impl(q, k_cache, v_cache, summaries, page_table, seq_lens, sd, sel_pages, max_sel, sel_count, scores_dbg,
+                     out, lse, sm_scale, workspace, workspace_bytes, shape, (cudaStream_t)stream);
+}
+
 // Device scratch of the host-buffer step, carved in this order (each 256-byte aligned):
-//   q | seq_lens | page_ids | n_valid | sel_pages | sel_count | out | select workspace | decode workspace
+//   q | seq_lens | page_ids | n_valid | sel_pages | sel_count | out | fused-step workspace | dense decode workspace
 namespace {
 struct StepCarve {
     size_t q, lens, ids, nval, sel, cnt, out, sel_ws, dec_ws, total;
@@ -340,10 +460,9 @@ StepCarve step_carve(const sparrow_shape_t *s, int32_t max_sel)
     c.sel = o; o += align256(n * s->n_kv_heads * (size_t)(max_sel > 0 ? max_sel : 1) * 4);
     c.cnt = o; o += align256(n * 4);
     c.out = o; o += align256(n * s->n_q_heads * kDim * 2);
-    c.sel_ws_bytes = sparrow_select_workspace_bytes(s);
+    c.sel_ws_bytes = sparrow_step_workspace_bytes(s, max_sel > 0 ? max_sel : 1);
     c.sel_ws = o; o += c.sel_ws_bytes;
-    const size_t d1 = sparrow_decode_workspace_bytes(s, max_sel), d0 = sparrow_decode_workspace_bytes(s, 0);
-    c.dec_ws_bytes = d1 > d0 ? d1 : d0;
+    c.dec_ws_bytes = sparrow_decode_workspace_bytes(s, 0);
     c.dec_ws = o; o += c.dec_ws_bytes;
     c.total = o;
     return c;
@@ -398,12 +517,9 @@ int sparrow_step_host(const void *q_host, const int32_t *seq_lens_host, const in
         rc = launch_decode<true>(base + c.q, k_cache, v_cache, page_table, lens_d, nullptr, 0, nullptr, base + c.out, nullptr,
                                  sm_scale, base + c.dec_ws, c.dec_ws_bytes, s, st);
     } else {
-        rc = select_impl(base + c.q, summaries, page_table, lens_d, sd, reinterpret_cast<int32_t *>(base + c.sel), max_sel,
-                         reinterpret_cast<int32_t *>(base + c.cnt), nullptr, base + c.sel_ws, c.sel_ws_bytes, s, st);
-        if (rc) return rc;
-        rc = launch_decode<false>(base + c.q, k_cache, v_cache, page_table, lens_d, reinterpret_cast<int32_t *>(base + c.sel),
-                                  max_sel, reinterpret_cast<int32_t *>(base + c.cnt), base + c.out, nullptr, sm_scale,
-                                  base + c.dec_ws, c.dec_ws_bytes, s, st);
+        rc = step_impl(base + c.q, k_cache, v_cache, summaries, page_table, lens_d, sd, reinterpret_cast<int32_t *>(base + c.sel),
+                       max_sel, reinterpret_cast<int32_t *>(base + c.cnt), nullptr, base + c.out, nullptr, sm_scale,
+                       base + c.sel_ws, c.sel_ws_bytes, s, st);
     }
     if (rc) return rc;
     if ((e = cudaMemcpyAsync(out_host, base + c.out, qbytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e, "D2H out");

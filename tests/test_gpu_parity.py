@@ -21,10 +21,24 @@ def _engine(wl, **kw):
     return eng
 
 
+FUSED = False
+
+
+@pytest.fixture(autouse=True, params=["two-launches", "fused-step"])
+def _path(request):
+    """Every test runs on both forms of the sparse step: sparrow_select + sparrow_sparse_decode, and sparrow_step."""
+    global FUSED
+    FUSED = request.param == "fused-step"
+    yield
+
+
 def _run_sparse(wl, **kw):
     eng = _engine(wl, **kw)
-    eng.select()
-    eng.sparse_decode()
+    if FUSED:
+        eng.fused_step()
+    else:
+        eng.select()
+        eng.sparse_decode()
     torch.cuda.synchronize()
     return eng
 
@@ -118,11 +132,11 @@ def test_select_is_repeatable_and_graph_capturable():
     st = torch.cuda.Stream()
     with torch.cuda.stream(st):
         eng.sel_pages.fill_(-1); eng.out.zero_()
-        eng.step(stream=st)                                   # warm-up on the capture stream
+        eng.step(stream=st, fused=FUSED)                      # warm-up on the capture stream
         st.synchronize()
         g = torch.cuda.CUDAGraph()
         with torch.cuda.graph(g, stream=st):
-            eng.step(stream=st)
+            eng.step(stream=st, fused=FUSED)
         for _ in range(3):
             eng.sel_pages.fill_(-1); eng.out.zero_()
             g.replay()
@@ -145,7 +159,7 @@ def test_step_host_entry_matches_device_path():
     eng.summaries[ids.long().to(DEV)] = 0                     # the step must rebuild the summaries of just-filled pages
     B.sparrow_step_host(q_h, lens_h, ids, nv, ids.numel(), wl.k_cache, wl.v_cache, eng.summaries, wl.page_table,
                         eng.sched, eng.max_sel, wl.sm_scale, out_h, scratch, eng.shape)
-    assert B.sparrow_last_launch_count() == 3                 # summarize, select, decode (merge fused)
+    assert B.sparrow_last_launch_count() == 2                 # summarize + the fused step (select, decode, merge)
     assert torch.equal(out_h, eng.out.cpu())
     check_summaries(eng.summaries, wl.host(), ids.numpy(), nv.numpy())
 
