@@ -148,7 +148,7 @@ size_t sparrow_step_workspace_bytes(const sparrow_shape_t *shape, int32_t max_se
 /* ---- whole step through HOST buffers (the end-to-end measurement path) ----------------------------
  * Copies this step's inputs from host memory (q_host [n][Hq][128] bf16, seq_lens_host [n] int32; pinned
  * memory makes the copies asynchronous), runs summarize (n_update pages, page_ids/n_valid are HOST arrays,
- * n_update may be 0) -> the fused select + sparse decode step (or the dense path when sched->kind == DENSE) on `stream`,
+ * n_update may be 0) -> select -> sparse decode (or the dense path when sched->kind == DENSE) on `stream`,
  * copies out back to out_host [n][Hq][128] bf16 and WAITS for the stream.  The K/V pools, summaries and
  * page_table are the resident cache state and stay device pointers.  `scratch` is a device buffer of at
  * least sparrow_step_scratch_bytes(shape, max_sel) bytes, zero-initialised once by the caller. */

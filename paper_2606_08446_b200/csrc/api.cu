@@ -517,9 +517,15 @@ int sparrow_step_host(const void *q_host, const int32_t *seq_lens_host, const in
         rc = launch_decode<true>(base + c.q, k_cache, v_cache, page_table, lens_d, nullptr, 0, nullptr, base + c.out, nullptr,
                                  sm_scale, base + c.dec_ws, c.dec_ws_bytes, s, st);
     } else {
-        rc = step_impl(base + c.q, k_cache, v_cache, summaries, page_table, lens_d, sd, reinterpret_cast<int32_t *>(base + c.sel),
-                       max_sel, reinterpret_cast<int32_t *>(base + c.cnt), nullptr, base + c.out, nullptr, sm_scale,
-                       base + c.sel_ws, c.sel_ws_bytes, s, st);
+        // two launches: measured faster than the fused step kernel on every configuration
+        uint8_t *ws = base + c.sel_ws;
+        const StepGeom g = step_geom(s, max_sel);
+        rc = select_impl(base + c.q, summaries, page_table, lens_d, sd, reinterpret_cast<int32_t *>(base + c.sel), max_sel,
+                         reinterpret_cast<int32_t *>(base + c.cnt), nullptr, ws, g.sel_bytes, s, st);
+        if (rc) return rc;
+        rc = launch_decode<false>(base + c.q, k_cache, v_cache, page_table, lens_d, reinterpret_cast<int32_t *>(base + c.sel),
+                                  max_sel, reinterpret_cast<int32_t *>(base + c.cnt), base + c.out, nullptr, sm_scale,
+                                  ws + g.sel_bytes + g.flag_bytes, g.dec_bytes, s, st);
     }
     if (rc) return rc;
     if ((e = cudaMemcpyAsync(out_host, base + c.out, qbytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e, "D2H out");

@@ -70,89 +70,199 @@ __device__ __forceinline__ float transpose_reduce8(const float (&a)[8], int lane
 }
 
 // Top-k of one (sequence, kv-head) unit by ONE warp (a5): scores of the unit's candidate pages in `ws` (global,
-// written by the scoring warps), s_keys / s_hist = CTA-shared scratch already locked by the caller.
-// Writes the ascending list: forced pages, every key above the k-th, and the first ties of the k-th in page order.
+// written by the scoring warps); s_keys (16-byte aligned, >= n_pages rounded up to 4 entries) and s_hist (256) are
+// this warp's scratch.  Writes the ascending list: forced pages, every key above the k-th, and the first ties of
+// the k-th in page order (R10).  Every scan handles 4 consecutive pages per lane (one 16-byte shared-memory access).
+//   1. one cp.async round brings all the scores in; keys = order-preserving uint32 of the fp32 score (exact order)
+//   2. a histogram over 256 LINEAR bins of the score range (monotone in the score, so it never reorders keys, and
+//      unlike the top bits of a float it spreads the keys: no atomic pile-up) finds the bin of the k-th key
+//   3. keys of higher bins become kSure, of lower bins kNever; an 8-bit radix select over the exact keys that are
+//      left (few) finds the k-th key itself;  4. ordered compaction.
+constexpr uint32_t kKeyForced = 0u, kKeyNever = 1u, kKeySure = 0xffffffffu;     // no finite score has these keys
+
+__device__ __forceinline__ float key_to_float(uint32_t key)
+{
+    return __uint_as_float((key & 0x80000000u) ? (key & 0x7fffffffu) : ~key);
+}
+
+// suffix scan over the 256 bins of s_hist: finds the bin holding the kk-th key counted from the top.
+// Returns the bin; kk becomes the rank inside that bin, hcnt the bin's population.
+__device__ __forceinline__ int find_bin(const int *s_hist, int &kk, int &hcnt, int lane)
+{
+    constexpr uint32_t kFull = 0xffffffffu;
+    int h[8], tot = 0;                   // lane owns bins [8*lane, 8*lane + 8)
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { h[i] = s_hist[lane * 8 + i]; tot += h[i]; }
+    int inc = tot;                       // inclusive suffix sum over lanes
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int v = __shfl_down_sync(kFull, inc, o);
+        if (lane + o < 32) inc += v;
+    }
+    int run = inc - tot, bin = -1, kk_new = 0, hc = 0;
+#pragma unroll
+    for (int i = 7; i >= 0; --i) {
+        if (run < kk && run + h[i] >= kk) { bin = lane * 8 + i; kk_new = kk - run; hc = h[i]; }
+        run += h[i];
+    }
+    const uint32_t who = __ballot_sync(kFull, bin >= 0);             // exactly one lane holds it
+    const int src = who ? __ffs(who) - 1 : 0;
+    kk = __shfl_sync(kFull, kk_new, src);
+    hcnt = __shfl_sync(kFull, hc, src);
+    return __shfl_sync(kFull, bin, src);
+}
+
 __device__ __forceinline__ void warp_topk(const SeqPlan &pl, const float *__restrict__ ws, uint32_t *s_keys, int *s_hist,
                                           int32_t *__restrict__ out, int max_sel, int lane)
 {
     constexpr uint32_t kFull = 0xffffffffu;
     const int n_pages = pl.n_pages;
-    // all the scores at once: 4-byte cp.async straight into the scratch (one round trip, no registers), then the
-    // order-preserving key in place
-    {
+    const int n4 = (n_pages + 3) >> 2;
+    uint4 *k4 = reinterpret_cast<uint4 *>(s_keys);
+    {   // 1. scores -> keys
         const uint32_t dst = smem_u32(s_keys);
-        for (int p = lane * 4; p < n_pages; p += 128)             // rows are 128-byte aligned and padded: 16-byte copies, L2 only
-            cp_async16(dst + p * 4, ws + p);
+        for (int v = lane; v < n4; v += 32) cp_async16(dst + v * 16, ws + v * 4);    // rows are 128-byte aligned and padded
         cp_async_commit();
         cp_async_wait<0>();
         __syncwarp();
-        for (int p = lane; p < n_pages; p += 32) s_keys[p] = pl.forced(p) ? 0u : order_key(__uint_as_float(s_keys[p]));
-        __syncwarp();
     }
+    uint32_t kmin = 0xffffffffu, kmax = 0u;
+#pragma unroll 2
+    for (int v = lane; v < n4; v += 32) {
+        uint4 x = k4[v];
+        uint32_t e[4] = {x.x, x.y, x.z, x.w};
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int p = v * 4 + i;
+            const bool cand = p < n_pages && !pl.forced(p);
+            e[i] = cand ? order_key(__uint_as_float(e[i])) : kKeyForced;
+            if (cand) { kmin = min(kmin, e[i]); kmax = max(kmax, e[i]); }
+        }
+        k4[v] = make_uint4(e[0], e[1], e[2], e[3]);
+    }
+#pragma unroll
+    for (int of = 16; of > 0; of >>= 1) {
+        kmin = min(kmin, __shfl_xor_sync(kFull, kmin, of));
+        kmax = max(kmax, __shfl_xor_sync(kFull, kmax, of));
+    }
+    __syncwarp();
 
     uint32_t prefix = 0, mask = 0;
     int need_eq = 0;
     if (pl.k > 0) {
-        int kk = pl.k;
+        // 2. linear bins: bin(key) = floor((score - vmin) * scale), monotone in the score
+        const float vmin = key_to_float(kmin), vmax = key_to_float(kmax);
+        const float scale = vmax > vmin ? 255.f / (vmax - vmin) : 0.f;
+        auto lin_bin = [&](uint32_t key) {
+            const int b = (int)((key_to_float(key) - vmin) * scale);
+            return b < 0 ? 0 : (b > 255 ? 255 : b);
+        };
+#pragma unroll
+        for (int i = 0; i < 8; ++i) s_hist[i * 32 + lane] = 0;
+        __syncwarp();
+#pragma unroll 2
+        for (int v = lane; v < n4; v += 32) {
+            const uint4 x = k4[v];
+            const uint32_t e[4] = {x.x, x.y, x.z, x.w};
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+                if (e[i] != kKeyForced) atomicAdd(&s_hist[lin_bin(e[i])], 1);
+        }
+        __syncwarp();
+        int kk = pl.k, hcnt = 0;
+        const int bstar = find_bin(s_hist, kk, hcnt, lane);
+        need_eq = kk;
+        __syncwarp();
+        // 3. classify by bin; radix select over the exact keys of the k-th key's bin (the rewrite rides on pass 0)
+        const bool whole = kk == hcnt;                               // the bin is taken whole: no exact pass needed
         for (int pass = 0; pass < 4; ++pass) {
             const int shift = 24 - 8 * pass;
 #pragma unroll
             for (int i = 0; i < 8; ++i) s_hist[i * 32 + lane] = 0;
             __syncwarp();
-            for (int p = lane; p < n_pages; p += 32) {
-                const uint32_t key = s_keys[p];
-                if (key != 0u && (key & mask) == prefix) atomicAdd(&s_hist[(key >> shift) & 255u], 1);
+#pragma unroll 2
+            for (int v = lane; v < n4; v += 32) {
+                const uint4 x = k4[v];
+                uint32_t e[4] = {x.x, x.y, x.z, x.w};
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    if (pass == 0 && e[i] != kKeyForced) {
+                        const int b = lin_bin(e[i]);
+                        if (b > bstar || (whole && b == bstar)) e[i] = kKeySure;
+                        else if (b < bstar) e[i] = kKeyNever;
+                    }
+                    const bool in_class = e[i] != kKeyForced && e[i] != kKeyNever && e[i] != kKeySure;
+                    if (!whole && in_class && (e[i] & mask) == prefix) atomicAdd(&s_hist[(e[i] >> shift) & 255u], 1);
+                }
+                if (pass == 0) k4[v] = make_uint4(e[0], e[1], e[2], e[3]);
             }
             __syncwarp();
-            // lane owns bins [8*lane, 8*lane + 8); above = keys in the bins of higher lanes
-            int h[8], tot = 0;
-#pragma unroll
-            for (int i = 0; i < 8; ++i) { h[i] = s_hist[lane * 8 + i]; tot += h[i]; }
-            int inc = tot;                                           // inclusive suffix sum over lanes
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const int v = __shfl_down_sync(kFull, inc, o);
-                if (lane + o < 32) inc += v;
-            }
-            int run = inc - tot, bin = -1, kk_new = 0, hcnt = 0;
-#pragma unroll
-            for (int i = 7; i >= 0; --i) {
-                if (run < kk && run + h[i] >= kk) { bin = lane * 8 + i; kk_new = kk - run; hcnt = h[i]; }
-                run += h[i];
-            }
-            const uint32_t who = __ballot_sync(kFull, bin >= 0);     // exactly one lane holds the k-th key's bin
-            const int src = __ffs(who) - 1;
-            bin = __shfl_sync(kFull, bin, src);
-            kk = __shfl_sync(kFull, kk_new, src);
-            hcnt = __shfl_sync(kFull, hcnt, src);
+            if (whole) break;
+            const int bin = find_bin(s_hist, kk, hcnt, lane);
             prefix |= (uint32_t)bin << shift;
             mask |= 255u << shift;
             need_eq = kk;
+            __syncwarp();
             if (kk == hcnt) break;                                   // the whole class is taken
         }
+        if (whole) { need_eq = 0; prefix = 0xffffffffu; mask = 0xffffffffu; }   // nothing of the class is left to pick
     }
-    // ordered compaction, 32 pages per round
+    __syncwarp();
+
+    // 4. ordered compaction: lane owns pages 4v .. 4v + 3; exclusive scans over the lanes keep page order
     int pos = 0, eq_seen = 0;
-    const uint32_t lt = (1u << lane) - 1u;
-    for (int p0 = 0; p0 < n_pages; p0 += 32) {
-        const int p = p0 + lane;
-        bool take = false, eq = false;
-        if (p < n_pages) {
-            const uint32_t key = s_keys[p];
-            if (key == 0u) take = pl.forced(p);
-            else if (pl.k > 0) {
-                const uint32_t c = key & mask;
-                take = c > prefix;
-                eq = c == prefix;
+    for (int v0 = 0; v0 < n4; v0 += 32) {
+        const int v = v0 + lane;
+        uint32_t e[4] = {kKeyNever, kKeyNever, kKeyNever, kKeyNever};
+        if (v < n4) {
+            const uint4 x = k4[v];
+            e[0] = x.x; e[1] = x.y; e[2] = x.z; e[3] = x.w;
+        }
+        bool take[4], eq[4];
+        int n_eq = 0;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int p = v * 4 + i;
+            take[i] = false; eq[i] = false;
+            if (p < n_pages) {
+                if (e[i] == kKeyForced) take[i] = pl.forced(p);
+                else if (e[i] == kKeySure) take[i] = true;
+                else if (e[i] != kKeyNever && pl.k > 0) {
+                    const uint32_t c = e[i] & mask;
+                    take[i] = c > prefix;
+                    eq[i] = c == prefix;
+                }
+            }
+            n_eq += eq[i];
+        }
+        int eq_inc = n_eq;                                           // ties: rank in page order
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(kFull, eq_inc, o);
+            if (lane >= o) eq_inc += t;
+        }
+        int rank = eq_seen + eq_inc - n_eq, n_take = 0;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            if (eq[i]) { if (rank < need_eq) take[i] = true; ++rank; }
+            n_take += take[i];
+        }
+        int tk_inc = n_take;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(kFull, tk_inc, o);
+            if (lane >= o) tk_inc += t;
+        }
+        int idx = pos + tk_inc - n_take;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            if (take[i]) {
+                if (idx < max_sel) out[idx] = v * 4 + i;
+                ++idx;
             }
         }
-        const uint32_t em = __ballot_sync(kFull, eq);
-        if (eq && eq_seen + __popc(em & lt) < need_eq) take = true;
-        const uint32_t tm = __ballot_sync(kFull, take);
-        const int idx = pos + __popc(tm & lt);
-        if (take && idx < max_sel) out[idx] = p;
-        pos += __popc(tm);
-        eq_seen += __popc(em);
+        pos += __shfl_sync(kFull, tk_inc, 31);
+        eq_seen += __shfl_sync(kFull, eq_inc, 31);
     }
 }
 
@@ -231,9 +341,12 @@ step_kernel(const StepArgs S, const SchedDev sched)
         const int a = min(gw * per, WC), b = min(a + per, WC);
         const uint4 *sum16 = reinterpret_cast<const uint4 *>(S.summaries);
 
-        float qc[8], qn[8];              // Q- (lanes 0-15) or Q+ (lanes 16-31), this lane's 8 channels: current / next chunk
-        ChunkDesc d, dn;                 // the chunk being scored / the one after it
-        d.unit = -1; d.seq = -1; dn.unit = -1; dn.seq = -1;
+        // Q- (lanes 0-15) or Q+ (lanes 16-31), this lane's 8 channels, and the description of the chunk being scored (d),
+        // of the next one (dn: its summaries are being requested) and of the one after (dnn: its page-table entries
+        // are in flight, a whole chunk ahead of their first use)
+        float qc[8], qn[8], qnn[8];
+        ChunkDesc d, dn, dnn;
+        d.unit = -1; d.seq = -1; dn.unit = -1; dn.seq = -1; dnn.unit = -1; dnn.seq = -1;
         // describe chunk c; `prev` = the description before it (plan and q are reused when they can be)
         auto describe = [&](int c, ChunkDesc &d, const ChunkDesc &prev, float (&qd)[8], const float (&qprev)[8]) {
             int lo = 0, hi = n_seq - 1;
@@ -273,60 +386,59 @@ step_kernel(const StepArgs S, const SchedDev sched)
                 }
             }
         };
-        // request the summaries of pages [16*half, 16*half + 16) of the chunk into ring stage `stage`
-        auto issue_half = [&](const ChunkDesc &d, int half, int stage) {
+        // The warp's ring (2 x 8 KiB) is used as four 4 KiB slots; slot qi holds quarter qi of a chunk = the summaries
+        // of its pages [8*qi, 8*qi + 8).  Three quarters are in flight while the fourth is being scored.
+        static_assert(kDecStages * kStageBytes >= 4 * 4096, "the scoring pipeline needs 16 KiB of ring per warp");
+        auto issue_q = [&](const ChunkDesc &d, int qi) {
             const uint32_t off16 = ((uint32_t)d.phys * (uint32_t)n_kv_heads + (uint32_t)d.g) * 32u;
-            const uint32_t dst = ring_u32 + stage * kStageBytes + lane * 16;
+            const uint32_t dst = ring_u32 + qi * 4096 + lane * 16;
 #pragma unroll
-            for (int j = 0; j < 16; ++j) {
-                const uint32_t o = __shfl_sync(kFull, off16, half * 16 + j);
-                if ((d.cand_mask >> (half * 16 + j)) & 1u) cp_async16(dst + j * 512, sum16 + o + lane);
+            for (int j = 0; j < 8; ++j) {
+                const uint32_t o = __shfl_sync(kFull, off16, qi * 8 + j);
+                if ((d.cand_mask >> (qi * 8 + j)) & 1u) cp_async16(dst + j * 512, sum16 + o + lane);
             }
         };
-        // scores of those 16 pages from ring stage `stage`: lane 16*half + j receives page j's score
-        auto score_half = [&](const ChunkDesc &d, const float (&qd)[8], int half, int stage, float &my_score) {
-            const uint32_t src = ring_u32 + stage * kStageBytes + lane * 16;
+        // scores of those 8 pages: lane 8*qi + j receives page j's score
+        auto score_q = [&](const ChunkDesc &d, const float (&qd)[8], int qi, float &my_score) {
+            const uint32_t bm = (d.cand_mask >> (qi * 8)) & 0xffu;
+            if (bm == 0) return;                                     // warp-uniform
+            const uint32_t src = ring_u32 + qi * 4096 + lane * 16;
+            float acc[8];
 #pragma unroll
-            for (int b8 = 0; b8 < 2; ++b8) {
-                const uint32_t bm = (d.cand_mask >> (half * 16 + b8 * 8)) & 0xffu;
-                if (bm == 0) continue;                               // warp-uniform
-                float acc[8];
-#pragma unroll
-                for (int j = 0; j < 8; ++j) {
-                    acc[j] = 0.f;
-                    if ((bm >> j) & 1u) acc[j] = dot8(qd, lds128(src + (b8 * 8 + j) * 512), 0.f);
-                }
-                const float z = transpose_reduce8(acc, lane);
-                const int j = lane - (half * 16 + b8 * 8);
-                const int from = ((j >> 2) & 1) * 16 + ((j >> 1) & 1) * 8 + (j & 1) * 4;
-                const float got = __shfl_sync(kFull, z, from & 31);
-                if (j >= 0 && j < 8) my_score = got;
+            for (int j = 0; j < 8; ++j) {
+                acc[j] = 0.f;
+                if ((bm >> j) & 1u) acc[j] = dot8(qd, lds128(src + j * 512), 0.f);
             }
+            const float z = transpose_reduce8(acc, lane);
+            const int j = lane - qi * 8;
+            const int from = ((j >> 2) & 1) * 16 + ((j >> 1) & 1) * 8 + (j & 1) * 4;
+            const float got = __shfl_sync(kFull, z, from & 31);
+            if (j >= 0 && j < 8) my_score = got;
         };
 
         int done_in_unit = 0;
-        if (a < b) {
-            describe(a, d, dn, qc, qn);
-            issue_half(d, 0, 0);
+        if (a < b) describe(a, d, dn, qc, qn);
+        if (a + 1 < b) describe(a + 1, dn, d, qn, qc);
+#pragma unroll
+        for (int qi = 0; qi < 3; ++qi) {
+            if (a < b) issue_q(d, qi);
+            cp_async_commit();
         }
-        cp_async_commit();
 #pragma unroll 1
         for (int c = a; c < b; ++c) {
-            issue_half(d, 1, 1);
-            cp_async_commit();
             const bool more = c + 1 < b;
-            if (more) describe(c + 1, dn, d, qn, qc);
+            if (c + 2 < b) describe(c + 2, dnn, dn, qnn, qn);        // its page-table entries are in flight from here
             float my_score = 0.f;
-            cp_async_wait<1>();
-            __syncwarp();
-            score_half(d, qc, 0, 0, my_score);
-            __syncwarp();                                            // stage 0 is free again
-            if (more) issue_half(dn, 0, 0);
-            cp_async_commit();
-            cp_async_wait<1>();
-            __syncwarp();
-            score_half(d, qc, 1, 1, my_score);
-            __syncwarp();
+#pragma unroll
+            for (int qi = 0; qi < 4; ++qi) {
+                if (qi == 0) issue_q(d, 3);                          // quarter t + 3 goes into the slot freed by t - 1
+                else if (more) issue_q(dn, qi - 1);
+                cp_async_commit();
+                cp_async_wait<3>();
+                __syncwarp();
+                score_q(d, qc, qi, my_score);
+                __syncwarp();
+            }
             // ---- results of the chunk ----
             int32_t *list = S.sel_pages + (int64_t)d.unit * max_sel;
             if (d.pl.dense) {                                        // R13: identity list, no scoring
@@ -338,8 +450,9 @@ step_kernel(const StepArgs S, const SchedDev sched)
             ++done_in_unit;
             auto turn = [&]() {
                 d = dn;
+                dn = dnn;
 #pragma unroll
-                for (int e = 0; e < 8; ++e) qc[e] = qn[e];
+                for (int e = 0; e < 8; ++e) { qc[e] = qn[e]; qn[e] = qnn[e]; }
             };
             if (more && dn.unit == d.unit) { turn(); continue; }
             // ---- this warp's share of the unit is done: arrive; the last warp to arrive selects ----

@@ -79,9 +79,9 @@ class SparrowEngine:
                               self.sched, self.sel_pages, self.max_sel, self.sel_count, self.scores, self.out, self.lse,
                               wl.sm_scale, self.step_ws, self.shape, stream)
 
-    def step(self, q=None, updates=None, stream=None, fused=True):
-        """One pass of the hot path: summarize the pages that just filled, then select + sparse decode (one fused
-        launch by default, or the two separate calls)."""
+    def step(self, q=None, updates=None, stream=None, fused=False):
+        """One pass of the hot path: summarize the pages that just filled, then select + sparse decode as two launches
+        (the measured-faster form) or, with fused=True, as the one cooperative launch of sparrow_step."""
         if updates is not None and updates[0].numel() > 0:
             self.summarize(updates[0], updates[1], stream=stream)
         if fused:

@@ -159,7 +159,7 @@ def test_step_host_entry_matches_device_path():
     eng.summaries[ids.long().to(DEV)] = 0                     # the step must rebuild the summaries of just-filled pages
     B.sparrow_step_host(q_h, lens_h, ids, nv, ids.numel(), wl.k_cache, wl.v_cache, eng.summaries, wl.page_table,
                         eng.sched, eng.max_sel, wl.sm_scale, out_h, scratch, eng.shape)
-    assert B.sparrow_last_launch_count() == 2                 # summarize + the fused step (select, decode, merge)
+    assert B.sparrow_last_launch_count() == 3                 # summarize, select, decode (merge fused in the decode launch)
     assert torch.equal(out_h, eng.out.cpu())
     check_summaries(eng.summaries, wl.host(), ids.numpy(), nv.numpy())
 
