@@ -129,6 +129,17 @@ int sparrow_dense_decode(const void *q, const void *k_cache, const void *v_cache
                          const int32_t *seq_lens, void *out, float *lse, float sm_scale,
                          void *workspace, size_t workspace_bytes, const sparrow_shape_t *shape, void *stream);
 
+/* ---- rollout step, cache side: append one token per sequence, summarize on page fill ----
+ * The rollout decodes token after token; the budget follows the growing length (:109-119).
+ * For every sequence i with L = seq_lens[i] tokens cached: the rows k_new[i], v_new[i] ([n_seq][n_kv_heads][128]
+ * bf16) are written at token position L (logical page L/16 through page_table, row L%16), seq_lens[i] becomes
+ * L + 1, and if the token fills its page (L%16 == 15) that page's min/max summary is (re)computed in the same
+ * launch -- a1 "on page fill".  A sequence whose page table has no room (L/16 >= max_pages_per_seq) is left
+ * untouched.  The caller then runs sparrow_select / sparrow_sparse_decode (or sparrow_step) with the new lengths;
+ * a partially filled last page needs no summary because it is always kept (R9). */
+int sparrow_append(const void *k_new, const void *v_new, void *k_cache, void *v_cache, void *summaries,
+                   const int32_t *page_table, int32_t *seq_lens, const sparrow_shape_t *shape, void *stream);
+
 /* ---- a2..a7 fused: the whole sparse step in ONE persistent launch ----------------------------------
  * Same results as sparrow_select followed by sparrow_sparse_decode on the same arguments (the selected lists
  * and sel_count are written too), but the summary stream, the per-unit top-k and the K/V stream share one

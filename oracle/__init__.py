@@ -20,5 +20,7 @@ from .oracle import (  # noqa: F401
     sparse_step,
     attention_on_sets,
     dense_step,
+    append_step,
+    rollout,
     num_threads,
 )

@@ -271,3 +271,45 @@ def dense_step(q, k_cache, v_cache, page_table, seq_lens, sm_scale: float):
         _i64(n), _i64(Hq), _i64(Hkv), _i64(P), _i64(D), _i64(page_table.shape[1]), C.c_double(sm_scale),
         _p(out), _p(lse))
     return out, lse
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# the multi-step rollout loop.  PAPER.md:138-147 -- every generated token runs landmark scoring ->
+# Top-k -> attention over the budget; PAPER.md:109-119 -- the budget follows the growing sequence length; the cache
+# side (the token's K/V appended at position L, landmarks of pages that fill) is what any paged decode does.  Written
+# out step by step with the functions above; plain numpy indexing for the data movement.
+def append_step(k_cache, v_cache, page_table, seq_lens, k_new, v_new, page_size: int = 16):
+    """In place: token i's K/V rows go to position L_i (logical page L_i // 16 through the page table, row L_i % 16),
+    then L_i += 1.  Returns the physical pages that became full (their landmarks are due, a1 'on page fill')."""
+    filled = []
+    for i in range(len(seq_lens)):
+        L = int(seq_lens[i])
+        page = int(page_table[i, L // page_size])
+        k_cache[page, :, L % page_size, :] = k_new[i]
+        v_cache[page, :, L % page_size, :] = v_new[i]
+        seq_lens[i] = L + 1
+        if (L + 1) % page_size == 0:
+            filled.append(page)
+    return filled
+
+
+def rollout(q_steps, k_steps, v_steps, k_cache, v_cache, page_table, seq_lens, sched: Optional[Schedule], sm_scale: float,
+            max_sel: Optional[int] = None):
+    """T decode steps: append the step's K/V, then O1..O8 (sched given) or dense attention (sched None) with the
+    step's query over the grown cache.  Inputs are not modified.  Returns one dict per step: sparse_step's result
+    (or {'out', 'lse'} for dense) plus 'seq_lens' and 'filled' (physical pages whose landmarks were (re)built)."""
+    q_steps, k_steps, v_steps = _u16(q_steps), _u16(k_steps), _u16(v_steps)
+    k_cache, v_cache = _u16(k_cache).copy(), _u16(v_cache).copy()
+    page_table, seq_lens = _i32(page_table), _i32(seq_lens).copy()
+    steps = []
+    for t in range(q_steps.shape[0]):
+        filled = append_step(k_cache, v_cache, page_table, seq_lens, k_steps[t], v_steps[t])
+        if sched is None:
+            out, lse = dense_step(q_steps[t], k_cache, v_cache, page_table, seq_lens, sm_scale)
+            res = dict(out=out, lse=lse)
+        else:
+            res = sparse_step(q_steps[t], k_cache, v_cache, page_table, seq_lens, sched, sm_scale, max_sel=max_sel)
+        res["seq_lens"] = seq_lens.copy()
+        res["filled"] = filled
+        steps.append(res)
+    return steps, k_cache, v_cache

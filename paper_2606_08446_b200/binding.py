@@ -61,6 +61,7 @@ _SIGS = {
     "sparrow_select": (C.c_int, [_vp, _vp, _vp, _vp, _SCH, _vp, _i32, _vp, _vp, _vp, _sz, _SHP, _vp]),
     "sparrow_sparse_decode": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _i32, _vp, _vp, _vp, _f, _vp, _sz, _SHP, _vp]),
     "sparrow_dense_decode": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _f, _vp, _sz, _SHP, _vp]),
+    "sparrow_append": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _SHP, _vp]),
     "sparrow_step": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _SCH, _vp, _i32, _vp, _vp, _vp, _vp, _f, _vp, _sz, _SHP, _vp]),
     "sparrow_step_workspace_bytes": (_sz, [_SHP, _i32]),
     "sparrow_step_host": (C.c_int, [_vp, _vp, _vp, _vp, _i64, _vp, _vp, _vp, _vp, _SCH, _i32, _f, _vp, _vp, _sz, _SHP, _vp]),
@@ -188,6 +189,14 @@ def sparrow_dense_decode(q, k_cache, v_cache, page_table, seq_lens, out, lse, sm
                                    0 if workspace is None else workspace.numel() * workspace.element_size(), _by(shape), _stream(stream))
     if check:
         _check(rc, "sparrow_dense_decode")
+    return rc
+
+
+def sparrow_append(k_new, v_new, k_cache, v_cache, summaries, page_table, seq_lens, shape, stream=None, *, check=True):
+    rc = _lib.sparrow_append(_ptr(k_new), _ptr(v_new), _ptr(k_cache), _ptr(v_cache), _ptr(summaries), _ptr(page_table),
+                             _ptr(seq_lens), _by(shape), _stream(stream))
+    if check:
+        _check(rc, "sparrow_append")
     return rc
 
 

@@ -8,6 +8,7 @@
 #include "select.cuh"
 #include "step.cuh"
 #include "summarize.cuh"
+#include "append.cuh"
 
 using namespace sparrow;
 
@@ -409,6 +410,24 @@ int sparrow_dense_decode(const void *q, const void *k_cache, const void *v_cache
         return SPARROW_ERR_INVALID_ARG;
     return launch_decode<true>(q, k_cache, v_cache, page_table, seq_lens, nullptr, 0, nullptr, out, lse, sm_scale,
                                workspace, workspace_bytes, shape, (cudaStream_t)stream);
+}
+
+int sparrow_append(const void *k_new, const void *v_new, void *k_cache, void *v_cache, void *summaries,
+                   const int32_t *page_table, int32_t *seq_lens, const sparrow_shape_t *shape, void *stream)
+{
+    g_launches = 0;
+    int rc = check_shape(shape);
+    if (rc) return rc;
+    if (!k_new || !v_new || !k_cache || !v_cache || !summaries || !page_table || !seq_lens) return SPARROW_ERR_INVALID_ARG;
+    if (!aligned16(k_new) || !aligned16(v_new) || !aligned16(k_cache) || !aligned16(v_cache) || !aligned16(summaries))
+        return SPARROW_ERR_INVALID_ARG;
+    if (shape->n_seq == 0) return SPARROW_OK;
+    const int warps = shape->n_kv_heads < kAppendMaxWarps ? shape->n_kv_heads : kAppendMaxWarps;
+    append_kernel<<<shape->n_seq, warps * 32, 0, (cudaStream_t)stream>>>(
+        (const uint16_t *)k_new, (const uint16_t *)v_new, (uint16_t *)k_cache, (uint16_t *)v_cache, (uint16_t *)summaries,
+        page_table, seq_lens, shape->n_kv_heads, shape->max_pages_per_seq);
+    SPARROW_CHECK_LAUNCH("append_kernel");
+    return SPARROW_OK;
 }
 
 size_t sparrow_step_workspace_bytes(const sparrow_shape_t *s, int32_t max_sel)

@@ -48,9 +48,10 @@ class SparrowEngine:
 
     def summarize_all(self, stream=None):
         """Post-prefill bulk call over every page the batch owns (partial last pages use n_valid)."""
-        ids, nv = full_page_updates(self.wl)
-        dev = self.wl.q.device
-        self._ids, self._nv = ids.to(dev), nv.to(dev)
+        if getattr(self, "_ids", None) is None:          # built once on the host; later calls only launch the kernel
+            ids, nv = full_page_updates(self.wl)
+            dev = self.wl.q.device
+            self._ids, self._nv = ids.to(dev), nv.to(dev)
         return self.summarize(self._ids, self._nv, stream=stream)
 
     # ---- a2-a5
@@ -60,17 +61,47 @@ class SparrowEngine:
                                 self.sel_pages, self.max_sel, self.sel_count, self.scores, self.select_ws, self.shape, stream)
 
     # ---- a6-a7
-    def sparse_decode(self, q=None, stream=None):
+    def sparse_decode(self, q=None, stream=None, out=None, lse=None):
         wl = self.wl
         return B.sparrow_sparse_decode(wl.q if q is None else q, wl.k_cache, wl.v_cache, wl.page_table, wl.seq_lens,
-                                       self.sel_pages, self.max_sel, self.sel_count, self.out, self.lse, wl.sm_scale,
-                                       self.sparse_ws, self.shape, stream)
+                                       self.sel_pages, self.max_sel, self.sel_count, self.out if out is None else out,
+                                       self.lse if lse is None else lse, wl.sm_scale, self.sparse_ws, self.shape, stream)
 
     # ---- a8
-    def dense_decode(self, q=None, stream=None):
+    def dense_decode(self, q=None, stream=None, out=None, lse=None):
         wl = self.wl
         return B.sparrow_dense_decode(wl.q if q is None else q, wl.k_cache, wl.v_cache, wl.page_table, wl.seq_lens,
-                                      self.out_dense, self.lse_dense, wl.sm_scale, self.dense_ws, self.shape, stream)
+                                      self.out_dense if out is None else out, self.lse_dense if lse is None else lse,
+                                      wl.sm_scale, self.dense_ws, self.shape, stream)
+
+    # ---- 8(f)-1: the rollout loop
+    def append(self, k_new, v_new, stream=None):
+        """Cache side of a rollout step: write the token's K/V at position L, L += 1, summarize the page if it filled."""
+        wl = self.wl
+        return B.sparrow_append(k_new, v_new, wl.k_cache, wl.v_cache, self.summaries, wl.page_table, wl.seq_lens, self.shape, stream)
+
+    def reserve(self, n_steps: int):
+        """Size the selection buffers for lengths up to the current maximum + n_steps (B(L) grows with L)."""
+        max_len = int(self.wl.seq_lens.max().item()) + n_steps
+        assert max_len <= self.wl.max_pages * PAGE, "the page table has no room for that many appended tokens"
+        dev = self.wl.q.device
+        self.max_sel = max(1, B.sparrow_max_sel_pages(self.sched, max_len))
+        self.sel_pages = torch.full((self.wl.n_seq, self.wl.Hkv, self.max_sel), -1, dtype=torch.int32, device=dev)
+        self.sparse_ws = torch.zeros((B.sparrow_decode_workspace_bytes(self.shape, self.max_sel),), dtype=torch.uint8, device=dev)
+        self.step_ws = torch.zeros((B.sparrow_step_workspace_bytes(self.shape, self.max_sel),), dtype=torch.uint8, device=dev)
+
+    def rollout(self, q_steps, k_steps, v_steps, out_steps, lse_steps=None, dense=False, stream=None):
+        """T decode steps back to back on one stream (capturable as ONE CUDA graph: the lengths live on the device
+        and every launch is asynchronous): append -> select -> sparse decode per step, or append -> dense decode."""
+        for t in range(q_steps.shape[0]):
+            self.append(k_steps[t], v_steps[t], stream)
+            lse = None if lse_steps is None else lse_steps[t]
+            if dense:
+                self.dense_decode(q_steps[t], stream, out=out_steps[t], lse=self.lse_dense if lse is None else lse)
+            else:
+                self.select(q_steps[t], stream)
+                self.sparse_decode(q_steps[t], stream, out=out_steps[t], lse=lse)
+        return out_steps
 
     # ---- a2-a7 in one launch
     def fused_step(self, q=None, stream=None):

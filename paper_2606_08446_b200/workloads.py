@@ -104,7 +104,7 @@ def draw_lengths(spec, n_seq: int, gen: torch.Generator) -> List[int]:
 def make_workload(name: str = "custom", *, n_seq: int, Hq: int, Hkv: int, lengths, schedule: dict,
                   plant: bool = False, seed: int = 0, device="cpu", spare_pages: int = 3,
                   poison_tail: bool = False, plant_scale: float = 3.0, plant_frac: float = 0.05,
-                  chunk_pages: int = 8192, **_ignored) -> Workload:
+                  chunk_pages: int = 8192, reserve_tokens: int = 0, **_ignored) -> Workload:
     """Draw one batch.  Lengths, page tables and planted pages come from a CPU generator (so they do
     not depend on the device); q/K/V values come from a generator on ``device``."""
     dev = torch.device(device)
@@ -115,7 +115,8 @@ def make_workload(name: str = "custom", *, n_seq: int, Hq: int, Hkv: int, length
     assert Hq == r * Hkv
 
     lens = draw_lengths(lengths, n_seq, cg)
-    n_pages = [-(-L // P) for L in lens]
+    # pages each sequence owns: its cached tokens plus room for `reserve_tokens` more (the rollout loop appends into them)
+    n_pages = [-(-(L + reserve_tokens) // P) for L in lens]
     max_pages = max(n_pages)
     n_phys = sum(n_pages) + spare_pages
     perm = torch.randperm(n_phys, generator=cg)          # scattered physical placement
@@ -165,7 +166,7 @@ def make_workload(name: str = "custom", *, n_seq: int, Hq: int, Hkv: int, length
         for i, L in enumerate(lens):
             tail = L % P
             if tail:
-                ph = int(page_table[i, n_pages[i] - 1])
+                ph = int(page_table[i, L // P])
                 k_cache[ph, :, tail:, :] = 1.0e4
                 v_cache[ph, :, tail:, :] = -1.0e4
 
@@ -208,3 +209,13 @@ def just_filled_updates(wl: Workload):
     pt = wl.page_table.cpu()
     ids = [int(pt[i, L // PAGE - 1]) for i, L in enumerate(lens) if L % PAGE == 0 and L > 0]
     return torch.tensor(ids, dtype=torch.int32), torch.full((len(ids),), PAGE, dtype=torch.int32)
+
+
+def make_rollout_inputs(wl: Workload, n_steps: int, seed: int = 0):
+    """Per-step inputs of a T-step rollout: q [T][n][Hq][128], k_new / v_new [T][n][Hkv][128],
+    bf16 ~ N(0,1) from a seeded generator on the workload's device.  No method arithmetic here."""
+    dev = wl.q.device
+    g = torch.Generator(device=dev).manual_seed(seed + 104729)
+    def draw(h):
+        return torch.randn((n_steps, wl.n_seq, h, HEAD_DIM), generator=g, device=dev, dtype=torch.float32).to(torch.bfloat16)
+    return draw(wl.Hq), draw(wl.Hkv), draw(wl.Hkv)

@@ -350,3 +350,81 @@ def test_oracle_rejects_undersized_max_sel():
     with pytest.raises(ValueError):
         oracle.sparse_step(h["q"], h["k_cache"], h["v_cache"], h["page_table"], h["seq_lens"],
                            oracle.Schedule.from_spec(wl.schedule), wl.sm_scale, max_sel=8)
+
+
+# ------------------------------------------------------------------ 8(f)-1: rollout loop (append + grow) ----
+def _rollout_case(T=40, reserve=64):
+    lens = [250, 1023, 15, 2040]
+    sched = W._sched("table", 16, 48, table_pages=(6, 9, 14), bin_tokens=512)      # budget steps up as L crosses 512, 1024
+    wl = W.make_workload(n_seq=len(lens), Hq=4, Hkv=2, lengths=("list", lens), schedule=sched, seed=21, device="cpu",
+                         reserve_tokens=reserve)
+    qs, ks, vs = W.make_rollout_inputs(wl, T, seed=5)
+    bits = lambda t: t.contiguous().view(torch.int16).numpy().view(np.uint16)
+    return wl, wl.host(), bits(qs), bits(ks), bits(vs), sched
+
+
+def test_rollout_append_places_tokens_by_position_bruteforce():
+    """After T appends token j of sequence i sits at (page_table[i][j // 16], row j % 16): checked token by token
+    against the step inputs with indexing written here, not the oracle's (the cache a decode grows)."""
+    T = 40
+    wl, h, qs, ks, vs, sched = _rollout_case(T)
+    steps, kc, vc = oracle.rollout(qs, ks, vs, h["k_cache"], h["v_cache"], h["page_table"], h["seq_lens"],
+                                   oracle.Schedule.from_spec(sched), wl.sm_scale)
+    for i, L0 in enumerate(h["seq_lens"].tolist()):
+        assert steps[-1]["seq_lens"][i] == L0 + T
+        for t in range(T):
+            j = L0 + t
+            page = h["page_table"][i, j // P]
+            assert np.array_equal(kc[page, :, j % P, :], ks[t, i]) and np.array_equal(vc[page, :, j % P, :], vs[t, i])
+        for j in range(0, L0, 97):       # old tokens untouched
+            page = h["page_table"][i, j // P]
+            assert np.array_equal(kc[page, :, j % P, :], h["k_cache"][page, :, j % P, :])
+    # pages reported as filled are exactly those whose last row was written at that step
+    for t, st in enumerate(steps):
+        want = sorted(int(h["page_table"][i, (L0 + t) // P]) for i, L0 in enumerate(h["seq_lens"].tolist()) if (L0 + t + 1) % P == 0)
+        assert sorted(st["filled"]) == want
+
+
+def test_rollout_step_equals_one_shot_on_the_grown_cache_and_budget_follows_length():
+    """Step t of the loop is O1..O8 on the cache as it stands after t + 1 appends (checked against a cache rebuilt
+    here from scratch), and the attended-token count per step is the closed form of the TABLE schedule in 512-token
+    bins -- the budget steps up when L crosses a bin edge and attention cost is O(B), not O(L)
+    (PAPER.md:140, :498)."""
+    T = 24
+    wl, h, qs, ks, vs, sched = _rollout_case(T)
+    osched = oracle.Schedule.from_spec(sched)
+    steps, _, _ = oracle.rollout(qs, ks, vs, h["k_cache"], h["v_cache"], h["page_table"], h["seq_lens"], osched, wl.sm_scale)
+    table, bins = sched["table_pages"], sched["bin_tokens"]
+    for t in (0, 7, T - 1):
+        kc, vc = h["k_cache"].copy(), h["v_cache"].copy()
+        lens = h["seq_lens"].copy()
+        for u in range(t + 1):
+            for i in range(wl.n_seq):
+                j = int(lens[i]); page = h["page_table"][i, j // P]
+                kc[page, :, j % P] = ks[u, i]; vc[page, :, j % P] = vs[u, i]
+                lens[i] += 1
+        one = oracle.sparse_step(qs[t], kc, vc, h["page_table"], lens, osched, wl.sm_scale)
+        assert np.array_equal(one["sel"], steps[t]["sel"]) and np.allclose(one["out"], steps[t]["out"], rtol=0, atol=1e-12)
+        for i in range(wl.n_seq):
+            L = int(lens[i]); n_pages = -(-L // P)
+            budget_pages = table[min((L - 1) // bins, len(table) - 1)]
+            n_forced = len(set(range(min(1, n_pages))) | set(range(max(L - 48, 0) // P, n_pages)))
+            want = n_pages if budget_pages >= n_pages else max(budget_pages, n_forced)
+            assert steps[t]["sel_count"][i] == want, (t, i, L)
+    # sequence 1 (L0 = 1023) crosses the 1024 bin edge after its second append: 9 -> 14 pages
+    assert steps[0]["sel_count"][1] == 9 and steps[1]["sel_count"][1] == 14
+
+
+def test_rollout_dense_branch_is_dense_attention_on_the_grown_cache():
+    T = 5
+    wl, h, qs, ks, vs, sched = _rollout_case(T)
+    steps, kc, vc = oracle.rollout(qs, ks, vs, h["k_cache"], h["v_cache"], h["page_table"], h["seq_lens"], None, wl.sm_scale)
+    i, L = 2, int(h["seq_lens"][2]) + T                      # the 15-token sequence: numpy softmax over its 20 tokens
+    keys = np.stack([f64(kc[h["page_table"][i, j // P], :, j % P, :]) for j in range(L)])      # [L][Hkv][D]
+    vals = np.stack([f64(vc[h["page_table"][i, j // P], :, j % P, :]) for j in range(L)])
+    q = f64(qs[T - 1, i])                                     # [Hq][D]
+    for hq in range(wl.Hq):
+        g = hq // (wl.Hq // wl.Hkv)
+        z = keys[:, g, :] @ q[hq] * wl.sm_scale
+        p = np.exp(z - z.max()); p /= p.sum()
+        assert np.allclose(p @ vals[:, g, :], steps[-1]["out"][i, hq], rtol=0, atol=1e-12)
