@@ -170,6 +170,26 @@ int sparrow_step_host(const void *q_host, const int32_t *seq_lens_host,
                       void *out_host, void *scratch, size_t scratch_bytes,
                       const sparrow_shape_t *shape, void *stream);
 
+/* ---- rollout cost model (SURVEY.md 8(f)-4; PAPER.md:129-145 Eq. 2-3, :474-498 App. F) -- host only ----------
+ * Equivalent-FLOP cost of a rollout: batch_size x n_samples responses of L_out tokens after a prompt of L_in,
+ * model of P parameters, K/V width D, GQA ratio r, hardware intensity I (flops per element moved; R18), KV budget K
+ * tokens, page size, c landmark vectors per page (1 = the paper's model, 2 = this library's min/max summaries, R1).
+ *   attention elements   H = (2 L_in + L_d) L_d + 2 K (L_out - L_d)+ ,  L_d = min(L_out, max(K - L_in, 0))   (App. F)
+ *   dense   comp = 2 P B N L_out + r B N (2 L_in + L_out) L_out D      mem = 2 P L_out + B N (2 L_in L_out + L_out^2) D
+ *   sparse  comp = 2 P B N L_out + r B N D H                           mem = 2 P L_out + B N D H
+ *   scoring (steps past the dense phase only; landmark visits S = sum over those steps of (L_in + t) / pagesize):
+ *           comp = 2 r B N D S                                         mem = c B N D S         (Eq. 3; reading R21)
+ *   total = comp + I * mem.  Returns SPARROW_ERR_INVALID_ARG for non-positive sizes. */
+typedef struct sparrow_cost_args {
+    double params, batch_size, n_samples, L_in, L_out, D, r, intensity, budget_tokens, page_size, landmarks_per_page;
+} sparrow_cost_args_t;
+typedef struct sparrow_cost {
+    double attn_elems_dense, attn_elems_sparse, landmark_visits;
+    double dense_comp, dense_mem, dense_total;
+    double sparse_comp, sparse_mem, scoring_comp, scoring_mem, sparse_total;
+} sparrow_cost_t;
+int sparrow_cost_model(const sparrow_cost_args_t *args, sparrow_cost_t *cost);
+
 /* ---- host helpers (no device work; callable without a GPU) ---------------------------------------- */
 size_t sparrow_select_workspace_bytes(const sparrow_shape_t *shape);
 size_t sparrow_decode_workspace_bytes(const sparrow_shape_t *shape, int32_t max_sel /* 0 = dense */);

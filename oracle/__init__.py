@@ -22,5 +22,6 @@ from .oracle import (  # noqa: F401
     dense_step,
     append_step,
     rollout,
+    cost_model,
     num_threads,
 )

@@ -313,3 +313,31 @@ def rollout(q_steps, k_steps, v_steps, k_cache, v_cache, page_table, seq_lens, s
         res["filled"] = filled
         steps.append(res)
     return steps, k_cache, v_cache
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# the paper's rollout cost model, restated from PAPER.md:129-145 (Eq. 2-3) and :474-498 (App. F)
+# in the paper's notation.  Plain Python floats (fp64).
+def cost_model(P, B, N, L_in, L_out, D, r, I, K, pagesize, c=1.0) -> dict:
+    """P parameters, B batch, N samples, L_in prompt, L_out response, D K/V width, r GQA ratio, I hardware intensity
+    (R18), K KV budget in tokens, c landmark vectors per page (1 in the paper's model; R1 uses 2).
+    App. F:  L_dense = min(L_out, K - L_in) (not below 0);  H = (2 L_in + L_dense) L_dense + 2 K (L_out - L_dense)+
+             C_comp = 2 P B N L_out + r B N (2 L_in + L_out) L_out D;  C_mem = 2 P L_out + B N (2 L_in L_out + L_out^2) D
+             sparse: the attention terms with H in place of (2 L_in + L_out) L_out.
+    Eq. 3 scoring (reading R21: one landmark visit per page of the context per decode step, only on the steps decoded
+    under the budget): visits S = sum over those steps of (L_in + t) / pagesize (continuous form, as the paper's
+    L_out^2 / 2 terms);  compute 2 r B N D S;  memory c B N D S.   C = C_comp + I C_mem."""
+    L_dense = min(L_out, max(K - L_in, 0.0))
+    H = (2 * L_in + L_dense) * L_dense + 2 * K * max(L_out - L_dense, 0.0)
+    H_dense = (2 * L_in + L_out) * L_out
+    S = ((L_in * L_out + L_out ** 2 / 2) - (L_in * L_dense + L_dense ** 2 / 2)) / pagesize
+    dense_comp = 2 * P * B * N * L_out + r * B * N * H_dense * D
+    dense_mem = 2 * P * L_out + B * N * H_dense * D
+    sparse_comp = 2 * P * B * N * L_out + r * B * N * D * H
+    sparse_mem = 2 * P * L_out + B * N * D * H
+    scoring_comp = 2 * r * B * N * D * S
+    scoring_mem = c * B * N * D * S
+    return dict(attn_elems_dense=H_dense, attn_elems_sparse=H, landmark_visits=S, dense_comp=dense_comp, dense_mem=dense_mem,
+                dense_total=dense_comp + I * dense_mem, sparse_comp=sparse_comp, sparse_mem=sparse_mem,
+                scoring_comp=scoring_comp, scoring_mem=scoring_mem,
+                sparse_total=sparse_comp + scoring_comp + I * (sparse_mem + scoring_mem))

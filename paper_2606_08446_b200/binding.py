@@ -39,6 +39,16 @@ class sparrow_schedule_t(C.Structure):
                 ("table_len", C.c_int32), ("bin_tokens", C.c_int32)]
 
 
+class sparrow_cost_args_t(C.Structure):
+    _fields_ = [(k, C.c_double) for k in ("params", "batch_size", "n_samples", "L_in", "L_out", "D", "r", "intensity",
+                                          "budget_tokens", "page_size", "landmarks_per_page")]
+
+
+class sparrow_cost_t(C.Structure):
+    _fields_ = [(k, C.c_double) for k in ("attn_elems_dense", "attn_elems_sparse", "landmark_visits", "dense_comp", "dense_mem",
+                                          "dense_total", "sparse_comp", "sparse_mem", "scoring_comp", "scoring_mem", "sparse_total")]
+
+
 def make_shape(n_seq, n_q_heads, n_kv_heads, max_pages_per_seq, n_phys_pages, head_dim=128, page_size=16):
     return sparrow_shape_t(n_seq, n_q_heads, n_kv_heads, head_dim, page_size, max_pages_per_seq, n_phys_pages)
 
@@ -68,6 +78,7 @@ _SIGS = {
     "sparrow_select_workspace_bytes": (_sz, [_SHP]),
     "sparrow_decode_workspace_bytes": (_sz, [_SHP, _i32]),
     "sparrow_step_scratch_bytes": (_sz, [_SHP, _i32]),
+    "sparrow_cost_model": (C.c_int, [C.POINTER(sparrow_cost_args_t), C.POINTER(sparrow_cost_t)]),
     "sparrow_budget_tokens": (_i64, [_SCH, _i64]),
     "sparrow_k_pages": (_i32, [_SCH, _i64]),
     "sparrow_forced_count": (_i32, [_SCH, _i64]),
@@ -133,6 +144,15 @@ def sparrow_step_workspace_bytes(shape, max_sel: int) -> int:
 
 def sparrow_step_scratch_bytes(shape, max_sel: int) -> int:
     return _lib.sparrow_step_scratch_bytes(_by(shape), max_sel)
+
+
+def sparrow_cost_model(*, check=True, **kw) -> dict:
+    """Eq. 2-3 / App. F of the paper; keyword arguments = the fields of sparrow_cost_args_t.  Returns a dict."""
+    args, cost = sparrow_cost_args_t(**{k: float(v) for k, v in kw.items()}), sparrow_cost_t()
+    rc = _lib.sparrow_cost_model(_by(args), _by(cost))
+    if check:
+        _check(rc, "sparrow_cost_model")
+    return {k: getattr(cost, k) for k, _ in sparrow_cost_t._fields_}
 
 
 def sparrow_budget_tokens(sched, L: int) -> int:

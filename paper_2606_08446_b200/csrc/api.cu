@@ -317,6 +317,31 @@ size_t sparrow_decode_workspace_bytes(const sparrow_shape_t *s, int32_t max_sel)
     return gm.bytes_ctr + gm.bytes_o + gm.bytes_ml;
 }
 
+int sparrow_cost_model(const sparrow_cost_args_t *a, sparrow_cost_t *c)
+{
+    if (!a || !c) return SPARROW_ERR_INVALID_ARG;
+    if (!(a->params >= 0) || !(a->batch_size > 0) || !(a->n_samples > 0) || !(a->L_in >= 0) || !(a->L_out > 0) || !(a->D > 0) ||
+        !(a->r >= 1) || !(a->intensity >= 0) || !(a->budget_tokens > 0) || !(a->page_size > 0) || !(a->landmarks_per_page >= 0))
+        return SPARROW_ERR_INVALID_ARG;
+    const double BN = a->batch_size * a->n_samples, Li = a->L_in, Lo = a->L_out, K = a->budget_tokens;
+    double Ld = K - Li;
+    Ld = Ld < 0 ? 0 : (Ld > Lo ? Lo : Ld);
+    const double rest = Lo - Ld;                                        // steps decoded under the budget
+    c->attn_elems_dense = (2 * Li + Lo) * Lo;
+    c->attn_elems_sparse = (2 * Li + Ld) * Ld + 2 * K * rest;
+    c->landmark_visits = ((Li * Lo + 0.5 * Lo * Lo) - (Li * Ld + 0.5 * Ld * Ld)) / a->page_size;
+    const double param_comp = 2 * a->params * BN * Lo, param_mem = 2 * a->params * Lo;
+    c->dense_comp = param_comp + a->r * BN * c->attn_elems_dense * a->D;
+    c->dense_mem = param_mem + BN * c->attn_elems_dense * a->D;
+    c->dense_total = c->dense_comp + a->intensity * c->dense_mem;
+    c->sparse_comp = param_comp + a->r * BN * a->D * c->attn_elems_sparse;
+    c->sparse_mem = param_mem + BN * a->D * c->attn_elems_sparse;
+    c->scoring_comp = 2 * a->r * BN * a->D * c->landmark_visits;
+    c->scoring_mem = a->landmarks_per_page * BN * a->D * c->landmark_visits;
+    c->sparse_total = c->sparse_comp + c->scoring_comp + a->intensity * (c->sparse_mem + c->scoring_mem);
+    return SPARROW_OK;
+}
+
 int64_t sparrow_budget_tokens(const sparrow_schedule_t *sched, int64_t L)
 {
     SchedDev sd;

@@ -105,3 +105,21 @@ def test_workspace_sizes_and_validation_without_a_gpu(B):
     badsched = B.make_schedule(W._sched("linear_frac", 0, 0, f0_ppm=1, f1_ppm=1, L0=5, L1=5))
     assert B.sparrow_budget_tokens(badsched, 100) == -1
     assert "workspace" in B.sparrow_strerror(-3) and B.sparrow_strerror(0) == "ok"
+
+
+def test_cost_model_helper_matches_the_oracle_restatement():
+    """sparrow_cost_model (host helper of the library) against oracle.cost_model, both written from PAPER.md Eq. 2-3 /
+    App. F independently; and invalid arguments are refused."""
+    import itertools
+    import oracle
+    from paper_2606_08446_b200 import binding as B
+    for L_in, L_out, K, ps, c in itertools.product((0.0, 900.0, 9000.0), (1.0, 700.0, 32000.0), (256.0, 2048.0, 65536.0), (16.0, 128.0), (1.0, 2.0)):
+        kw = dict(params=8.0e9, batch_size=2.0, n_samples=8.0, L_in=L_in, L_out=L_out, D=128.0, r=4.0, intensity=295.0,
+                  budget_tokens=K, page_size=ps, landmarks_per_page=c)
+        got = B.sparrow_cost_model(**kw)
+        want = oracle.cost_model(kw["params"], kw["batch_size"], kw["n_samples"], L_in, L_out, 128.0, 4.0, 295.0, K, ps, c=c)
+        for k, v in want.items():
+            assert abs(got[k] - v) <= 1e-12 * max(1.0, abs(v)), (k, got[k], v, kw)
+    with pytest.raises(B.SparrowError):
+        B.sparrow_cost_model(params=1.0, batch_size=0.0, n_samples=1.0, L_in=0.0, L_out=1.0, D=128.0, r=1.0, intensity=1.0,
+                             budget_tokens=16.0, page_size=16.0, landmarks_per_page=1.0)

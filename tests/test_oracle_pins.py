@@ -428,3 +428,38 @@ def test_rollout_dense_branch_is_dense_attention_on_the_grown_cache():
         z = keys[:, g, :] @ q[hq] * wl.sm_scale
         p = np.exp(z - z.max()); p /= p.sum()
         assert np.allclose(p @ vals[:, g, :], steps[-1]["out"][i, hq], rtol=0, atol=1e-12)
+
+
+# ------------------------------------------------------------------ 8(f)-4: the paper's cost model ----
+def test_cost_model_against_per_step_sums_and_limits():
+    """App. F's closed forms against the per-decode-step sums they stand for, written out here:
+    step t attends min(L_in + t, K) tokens (K and V: 2 elements x D each), and scores (L_in + t) / pagesize landmarks
+    when L_in + t > K.  The closed forms are the continuous versions: they differ from the sums by the O(L) terms."""
+    P_, B_, N_, D_, r_, I_, ps = 1.7e9, 4.0, 8.0, 128.0, 2.0, 300.0, 16.0
+    for L_in, L_out, K in [(1000.0, 30000.0, 4096.0), (0.0, 5000.0, 1024.0), (6000.0, 2000.0, 4096.0), (100.0, 500.0, 4096.0)]:
+        c = oracle.cost_model(P_, B_, N_, L_in, L_out, D_, r_, I_, K, ps, c=2.0)
+        steps = np.arange(1, int(L_out) + 1, dtype=np.float64)
+        ctx = L_in + steps
+        attn_sum = 2 * np.minimum(ctx, K).sum()                     # K and V tokens over the rollout
+        dense_sum = 2 * ctx.sum()
+        visits = (ctx[ctx > K] / ps).sum()
+        assert abs(c["attn_elems_dense"] - dense_sum) <= 2 * L_out
+        assert abs(c["attn_elems_sparse"] - attn_sum) <= 2 * L_out
+        assert abs(c["landmark_visits"] - visits) <= (L_in + L_out) / ps
+        # memory and compute terms are those element counts times D (and r, B, N) plus the parameter terms
+        assert math.isclose(c["sparse_mem"], 2 * P_ * L_out + B_ * N_ * D_ * c["attn_elems_sparse"], rel_tol=1e-15)
+        assert math.isclose(c["dense_comp"], 2 * P_ * B_ * N_ * L_out + r_ * B_ * N_ * D_ * c["attn_elems_dense"], rel_tol=1e-15)
+        assert math.isclose(c["scoring_mem"], 2.0 * B_ * N_ * D_ * c["landmark_visits"], rel_tol=1e-15)
+        assert math.isclose(c["sparse_total"], c["sparse_comp"] + c["scoring_comp"] + I_ * (c["sparse_mem"] + c["scoring_mem"]), rel_tol=1e-15)
+    # budget covers the whole context: sparse == dense, nothing is scored (PAPER.md:494-496)
+    c = oracle.cost_model(P_, B_, N_, 100.0, 500.0, D_, r_, I_, 4096.0, ps)
+    assert c["attn_elems_sparse"] == c["attn_elems_dense"] and c["landmark_visits"] == 0 and c["sparse_total"] == c["dense_total"]
+    # O(K L_out) instead of O(L_out^2) (PAPER.md:498): doubling L_out doubles the budgeted part, quadruples the dense one
+    a = oracle.cost_model(0, 1, 1, 0.0, 20000.0, D_, r_, I_, 1000.0, ps)
+    b = oracle.cost_model(0, 1, 1, 0.0, 40000.0, D_, r_, I_, 1000.0, ps)
+    assert math.isclose(b["attn_elems_dense"] / a["attn_elems_dense"], 4.0)
+    assert 2.0 < b["attn_elems_sparse"] / a["attn_elems_sparse"] < 2.06
+    # Table 4's configurations all have budget 1024 (PAPER.md:428-434): equal attention cost, scoring cost ~ 1/pagesize
+    base = [oracle.cost_model(0, 1, 1, 16384.0, 1.0, D_, r_, I_, ps_ * n_, ps_) for ps_, n_ in ((16., 64.), (32., 32.), (64., 16.), (128., 8.))]
+    assert len({x["attn_elems_sparse"] for x in base}) == 1
+    assert math.isclose(base[0]["landmark_visits"] / base[3]["landmark_visits"], 8.0)
