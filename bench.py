@@ -166,6 +166,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--workload", default="cfg2", choices=[c for c in W.CONFIGS if c != "cfg4"])
     ap.add_argument("--impl", default="sparrow", choices=["sparrow", "reference"])
+    ap.add_argument("--step-form", default="two-launches", choices=["two-launches", "fused"],
+                    help="select + sparse decode as two launches (default, measured faster) or as the one cooperative sparrow_step launch")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-check", action="store_true", help="skip the sampled oracle self-check before timing")
     args = ap.parse_args()
@@ -210,12 +212,24 @@ def main():
     else:
         chk = None
 
+    fused = args.step_form == "fused"
+
     def one_step():
         n = 0
         if upd[0].numel() > 0:
             eng.summarize(upd[0], upd[1], stream=st); n += B.sparrow_last_launch_count()
+        if fused:
+            return n
         eng.select(stream=st); n += B.sparrow_last_launch_count()
         return n
+
+    def attend():
+        """second half of the step: the sparse decode launch (or the whole fused select + decode launch)"""
+        if fused:
+            eng.fused_step(stream=st)
+        else:
+            eng.sparse_decode(stream=st)
+        return B.sparrow_last_launch_count()
 
     # ---- timed region: K steps, device-resident inputs, events on the launching stream ----
     # Region A (-> `value`): K whole steps back to back, one event before and one after, as a caller runs them.
@@ -227,7 +241,7 @@ def main():
     launches = 0
     with torch.cuda.stream(st):
         for _ in range(Wm):
-            one_step(); eng.sparse_decode(stream=st)
+            one_step(); attend()
         st.synchronize()
         D.barrier()
         torch.cuda.synchronize()
@@ -236,7 +250,7 @@ def main():
         t_beg.record(st)
         for k in range(K):
             launches += one_step()
-            eng.sparse_decode(stream=st); launches += B.sparrow_last_launch_count()
+            launches += attend()
         t_end.record(st)
         st.synchronize()
         torch.cuda.synchronize()
@@ -245,7 +259,7 @@ def main():
             ev[k][0].record(st)
             one_step()
             ev[k][1].record(st)
-            eng.sparse_decode(stream=st)
+            attend()
             ev[k][2].record(st)
         st.synchronize()
         clk = clocks.stop()
@@ -295,7 +309,10 @@ def main():
     cnt = eng.sel_count.cpu().numpy()
     ab = algorithmic_bytes(wl, eng, lens, cnt)
     peak, peak_src = measured_peaks()
-    dec_gbs = ab["decode"] / (dec_ms * 1e-3) / 1e9
+    roof_bytes = ab["decode"] + (ab["select"] if fused else 0)       # fused: one launch streams the summaries too
+    roof_kernel = ("step_kernel (one sparrow_step call: scoring + top-k + decode + LSE merge)" if fused else
+                   "decode_kernel<sparse> (one sparrow_sparse_decode call; LSE merge fused in the same launch)")
+    dec_gbs = roof_bytes / (dec_ms * 1e-3) / 1e9
     sel_gbs = ab["select"] / (sel_ms * 1e-3) / 1e9
     dense_gbs = ab["dense"] / (dense_ms * 1e-3) / 1e9
     traffic = None      # dram__bytes_read.sum + dram__bytes_write.sum of the decode kernel from the committed ncu capture
@@ -303,7 +320,7 @@ def main():
     if os.path.exists(tp):
         for ln in open(tp):
             f = ln.split()
-            if len(f) >= 3 and f[0] == args.workload and f[1] == "decode_kernel":
+            if len(f) >= 3 and f[0] == args.workload and f[1] == ("step_kernel" if fused else "decode_kernel"):
                 traffic = int(f[2])
 
     line = {
@@ -311,14 +328,14 @@ def main():
         "ms_per_step": t_max * 1e3 / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "bf16", "data": "synthetic",
         "config": {"workload": args.workload, "n_seq": wl.n_seq, "Hq": wl.Hq, "Hkv": wl.Hkv, "head_dim": 128, "page_size": 16,
-                   "len_min": int(lens.min()), "len_max": int(lens.max()), "schedule": wl.schedule["kind"],
+                   "len_min": int(lens.min()), "len_max": int(lens.max()), "schedule": wl.schedule["kind"], "step_form": args.step_form,
                    "sink_tokens": wl.schedule["sink_tokens"], "local_tokens": wl.schedule["local_tokens"],
                    "selected_pages_per_seq_mean": float(cnt.mean()), "parallelism": f"replicas x{world} (no collective)",
                    "l2": "inputs larger than L2: %.0f MB touched per step vs 126 MB L2" % ((ab["decode"] + ab["select"]) / 1e6),
                    "timing": "value: K steps back to back between two events; roofline/kernels: a second pass of K steps with an event between the calls"},
-        "roofline": {"bound": "hbm", "kernel": "decode_kernel<sparse> (one sparrow_sparse_decode call; LSE merge fused in the same launch)",
+        "roofline": {"bound": "hbm", "kernel": roof_kernel,
                      "achieved": dec_gbs, "peak": peak, "unit": "GB/s", "frac": dec_gbs / peak, "traffic": traffic,
-                     "peak_source": peak_src, "algorithmic_bytes_per_launch": ab["decode"], "avg_launch_ms": dec_ms,
+                     "peak_source": peak_src, "algorithmic_bytes_per_launch": roof_bytes, "avg_launch_ms": dec_ms,
                      "frac_of_8TBs_nominal": dec_gbs / 8000.0},
         "kernels": {"select": {"ms": sel_ms, "algorithmic_bytes": ab["select"], "achieved_GBs": sel_gbs, "frac": sel_gbs / peak},
                     "sparse_decode": {"ms": dec_ms, "algorithmic_bytes": ab["decode"], "achieved_GBs": dec_gbs, "frac": dec_gbs / peak},
