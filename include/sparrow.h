@@ -146,7 +146,8 @@ int sparrow_append(const void *k_new, const void *v_new, void *k_cache, void *v_
  * cooperative launch: every warp moves from scoring to decoding as soon as its share is done, and a decode
  * look-up waits only for the one (sequence, kv-head) list it needs.  Falls back to the two launches when the
  * shape does not fit the fused kernel's shared memory (roughly n_seq + max_pages_per_seq/2 > 12000) or the device
- * cannot keep 148 CTAs resident.  sched->kind == DENSE is allowed (identity lists).  workspace:
+ * cannot keep 148 CTAs resident.  sched->kind == DENSE is allowed (identity lists).  Measured on B200 this form is
+ * not yet faster than the two calls: it is the opt-in single-launch form.  workspace:
  * sparrow_step_workspace_bytes(shape, max_sel) bytes, ZERO-INITIALISED once by the caller, restored to zero by
  * the call like the other workspaces; not shareable by two calls in flight. */
 int sparrow_step(const void *q, const void *k_cache, const void *v_cache, const void *summaries,

@@ -4,21 +4,22 @@
 //
 // Why one launch: select and decode are two short HBM streams (cfg2: 160 MB + 538 MB, ~25 us + ~80 us at the
 // roofline); as two kernels each pays its own ramp-up, its own tail (the top-k of the last units with HBM idle, the
-// last merges) and a launch gap -- 25-30 us of a ~135 us step.  Here the same 148 x 8 warps first stream the
-// summaries, and every warp moves on to the K/V stream as soon as its share of the scoring is done; the only
-// synchronisation is one flag per (sequence, kv-head) unit, set when the unit's page list is written and waited for
-// by the decode look-ups that need it.  Both streams are cut in (sequence, kv-head) order, so a warp decodes
-// roughly the units it (and its neighbours) scored and the waits are short; HBM stays busy across the phase change.
+// last merges) and a launch gap.  Here the same 148 x 8 warps first stream the summaries, and every warp moves on to
+// the K/V stream as soon as its share of the scoring is done; the only synchronisation is one flag per
+// (sequence, kv-head) unit, set when the unit's page list is written and waited for by the decode look-ups that need
+// it.  MEASURED (profiles/r1_v7_cfg2.md): exact and parity-green, but not faster than the two launches
+// yet -- all units finish scoring together and the single-warp top-k (13-40 us) then holds every decoder up -- so the
+// two-launch form stays the library's default and this kernel is the opt-in single-launch form.
 //
 // Scoring phase (per warp, no CTA-wide barrier): the candidate pages of the batch form a flat stream of 32-page
 // warp-chunks, ordered (sequence, kv-head, chunk), cut into equal contiguous ranges.  A chunk's summaries (512 B per
 // page: min | max) are gathered through the page table with 16-byte cp.async into the warp's K/V ring (idle in this
-// phase), 16 pages = 8 KiB per stage, so a warp keeps 8-16 KiB in flight; the score is the R5 closed form
+// phase) used as four 4 KiB slots of 8 pages, three in flight while the fourth is scored; page-table entries are
+// fetched two chunks ahead.  The score is the R5 closed form
 //   s[p] = sum_d ( Q+[d]*mx[d] + Q-[d]*mn[d] ),  Q+ = sum_h max(q_h,0), Q- = sum_h min(q_h,0)
 // (lane = one 16-byte piece of the summary = 8 channels of min or of max; transpose-reduce over the warp).
-// The warp that completes a unit (one atomic counter per unit) runs its top-k alone: order-preserving keys in a
-// CTA-shared scratch (behind a shared-memory lock; contention is rare), 8-bit radix select for the k-th key, ordered
-// ballot compaction -- ascending list, ties to the lower page (R10) -- then releases the unit's flag.
+// The warp that completes a unit (one atomic counter per unit) runs its top-k alone (warp_topk below) in its own
+// shared-memory scratch (one CTA-wide scratch behind a lock when eight do not fit), then releases the unit's flag.
 // Sequences that are dense under the schedule (R13) write the identity list chunk by chunk and skip the scoring.
 //
 // Decode phase: decode_warp_stream<false, true> of decode.cuh, unchanged but for the flag wait.
