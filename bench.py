@@ -287,7 +287,8 @@ def run_cfg4(args, rank, local_rank, world, dev):
         "roofline": {"bound": "hbm", "kernel": "decode_kernel<sparse> (mean over the 34 sparse layers, events between the calls)",
                      "achieved": dec_gbs, "peak": peak, "unit": "GB/s", "frac": dec_gbs / peak, "traffic": None, "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": ab["decode"], "avg_launch_ms": dec_ms, "frac_of_8TBs_nominal": dec_gbs / 8000.0},
-        "kernels": {"select": {"ms": sel_ms, "algorithmic_bytes": ab["select"], "achieved_GBs": sel_gbs, "frac": sel_gbs / peak},
+        "kernels": {"summarize_step": {"ms": sum_ms, "pages": int(upd[0].numel())},
+                    "select": {"ms": sel_ms, "algorithmic_bytes": ab["select"], "achieved_GBs": sel_gbs, "frac": sel_gbs / peak},
                     "sparse_decode": {"ms": dec_ms, "algorithmic_bytes": ab["decode"], "achieved_GBs": dec_gbs, "frac": dec_gbs / peak},
                     "dense_decode_all_layers": {"ms": dense_ms_all, "achieved_GBs": n_layers * ab["dense"] / (dense_ms_all * 1e-3) / 1e9}},
         "graph_ms_per_step": graph_ms,
@@ -383,7 +384,7 @@ def main():
     # kernel's launch duration; the extra event records cost a few microseconds per step, so B is not the
     # throughput number.
     K, Wm = args.steps, args.warmup
-    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(K)]
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(K)]
     launches = 0
     with torch.cuda.stream(st):
         for _ in range(Wm):
@@ -402,14 +403,19 @@ def main():
         torch.cuda.synchronize()
         D.barrier()
         for k in range(K):
+            ev[k][3].record(st)
+            if upd[0].numel() > 0:
+                eng.summarize(upd[0], upd[1], stream=st)
             ev[k][0].record(st)
-            one_step()
+            if not fused:
+                eng.select(stream=st)
             ev[k][1].record(st)
             attend()
             ev[k][2].record(st)
         st.synchronize()
         clk = clocks.stop()
     total_ms = t_beg.elapsed_time(t_end)
+    sum_ms = float(np.mean([e[3].elapsed_time(e[0]) for e in ev]))
     sel_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in ev]))
     dec_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in ev]))
     value, t_max = D.whole_job_throughput(wl.n_seq * K, total_ms * 1e-3, device=dev)
@@ -483,7 +489,8 @@ def main():
                      "achieved": dec_gbs, "peak": peak, "unit": "GB/s", "frac": dec_gbs / peak, "traffic": traffic,
                      "peak_source": peak_src, "algorithmic_bytes_per_launch": roof_bytes, "avg_launch_ms": dec_ms,
                      "frac_of_8TBs_nominal": dec_gbs / 8000.0},
-        "kernels": {"select": {"ms": sel_ms, "algorithmic_bytes": ab["select"], "achieved_GBs": sel_gbs, "frac": sel_gbs / peak},
+        "kernels": {"summarize_step": {"ms": sum_ms, "pages": int(upd[0].numel())},
+                    "select": {"ms": sel_ms, "algorithmic_bytes": ab["select"], "achieved_GBs": sel_gbs, "frac": sel_gbs / peak},
                     "sparse_decode": {"ms": dec_ms, "algorithmic_bytes": ab["decode"], "achieved_GBs": dec_gbs, "frac": dec_gbs / peak},
                     "dense_decode": {"ms": dense_ms, "algorithmic_bytes": ab["dense"], "achieved_GBs": dense_gbs, "frac": dense_gbs / peak},
                     "bulk_summarize": {"ms": bulk_sum_ms, "pages": n_bulk,

@@ -18,7 +18,8 @@
  *     enqueued on `stream` (a cudaStream_t passed as void*, NULL = the legacy default stream) and the
  *     calls can be captured in a CUDA graph.  Device pointers must be 16-byte aligned.
  *   - bf16 tensors are raw 16-bit patterns.  Layouts (row-major, innermost last):
- *       k_cache, v_cache  [n_phys_pages][n_kv_heads][page_size=16][head_dim=128]   bf16  ("HND" pages)
+ *       k_cache, v_cache  [n_phys_pages][n_kv_heads][page_size][head_dim=128]      bf16  ("HND" pages; page_size 16,
+ *                                                      32, 64 or 128 -- a larger page is streamed as 16-token tiles)
  *       summaries         [n_phys_pages][n_kv_heads][2][128]                       bf16  ([0]=min, [1]=max)
  *       q, out            [n_seq][n_q_heads][128]                                  bf16
  *       lse               [n_seq][n_q_heads]                                       fp32  (natural log)
@@ -30,7 +31,7 @@
  *       sel_count         [n_seq]                                                  int32 (same for all kv heads)
  *     Query head h uses kv head h / r, r = n_q_heads / n_kv_heads (GQA; K/V are read once per group).
  *   - Return value: SPARROW_OK (0) or a negative sparrow_status; nothing throws, aborts or falls back to
- *     the CPU.  Supported: head_dim = 128, page_size = 16, 1 <= r <= 8, bf16; anything else returns
+ *     the CPU.  Supported: head_dim = 128, page_size in {16, 32, 64, 128}, 1 <= r <= 8, bf16; anything else returns
  *     SPARROW_ERR_UNSUPPORTED.
  */
 #ifndef SPARROW_H_
@@ -56,7 +57,7 @@ typedef struct sparrow_shape {
     int32_t n_q_heads;           /* Hq */
     int32_t n_kv_heads;          /* Hkv */
     int32_t head_dim;            /* D, must be 128 */
-    int32_t page_size;           /* P, must be 16 */
+    int32_t page_size;           /* P: 16 (the paper's choice) or 32 / 64 / 128 (Table 4) */
     int32_t max_pages_per_seq;   /* row stride of page_table */
     int64_t n_phys_pages;        /* pages in the K/V pools */
 } sparrow_shape_t;
@@ -88,6 +89,8 @@ typedef struct sparrow_schedule {
     const int32_t *table_pages;   /* HOST pointer, table_len <= SPARROW_MAX_TABLE_BINS entries; copied by value */
     int32_t table_len;
     int32_t bin_tokens;
+    int32_t page_size;            /* tokens per page that turns B(L) into pages: 16, 32, 64 or 128; 0 = 16.  The device
+                                     entry points use shape->page_size and refuse a non-zero value that differs */
 } sparrow_schedule_t;
 
 /* ---- a1: page summaries (north_star (a); "landmark") -------------------------------

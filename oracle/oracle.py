@@ -303,7 +303,7 @@ def rollout(q_steps, k_steps, v_steps, k_cache, v_cache, page_table, seq_lens, s
     page_table, seq_lens = _i32(page_table), _i32(seq_lens).copy()
     steps = []
     for t in range(q_steps.shape[0]):
-        filled = append_step(k_cache, v_cache, page_table, seq_lens, k_steps[t], v_steps[t])
+        filled = append_step(k_cache, v_cache, page_table, seq_lens, k_steps[t], v_steps[t], page_size=k_cache.shape[2])
         if sched is None:
             out, lse = dense_step(q_steps[t], k_cache, v_cache, page_table, seq_lens, sm_scale)
             res = dict(out=out, lse=lse)

@@ -36,7 +36,7 @@ class sparrow_schedule_t(C.Structure):
     _fields_ = [("kind", C.c_int32), ("sink_tokens", C.c_int32), ("local_tokens", C.c_int32),
                 ("fixed_tokens", C.c_int64), ("floor_tokens", C.c_int64), ("f0_ppm", C.c_int64), ("f1_ppm", C.c_int64),
                 ("L0", C.c_int64), ("L1", C.c_int64), ("table_pages", C.POINTER(C.c_int32)),
-                ("table_len", C.c_int32), ("bin_tokens", C.c_int32)]
+                ("table_len", C.c_int32), ("bin_tokens", C.c_int32), ("page_size", C.c_int32)]
 
 
 class sparrow_cost_args_t(C.Structure):
@@ -53,13 +53,14 @@ def make_shape(n_seq, n_q_heads, n_kv_heads, max_pages_per_seq, n_phys_pages, he
     return sparrow_shape_t(n_seq, n_q_heads, n_kv_heads, head_dim, page_size, max_pages_per_seq, n_phys_pages)
 
 
-def make_schedule(spec: dict) -> sparrow_schedule_t:
+def make_schedule(spec: dict, page_size: int = 0) -> sparrow_schedule_t:
     """From the plain-data schedule dict of ``workloads`` (kind, sink_tokens, ... table_pages, bin_tokens)."""
     tbl = (C.c_int32 * max(1, len(spec.get("table_pages", ()))))(*spec.get("table_pages", ()))
     s = sparrow_schedule_t(SCHED_KIND[spec["kind"]], spec.get("sink_tokens", 0), spec.get("local_tokens", 0),
                            spec.get("fixed_tokens", 0), spec.get("floor_tokens", 0), spec.get("f0_ppm", 0),
                            spec.get("f1_ppm", 0), spec.get("L0", 0), spec.get("L1", 1),
-                           C.cast(tbl, C.POINTER(C.c_int32)), len(spec.get("table_pages", ())), spec.get("bin_tokens", 2048))
+                           C.cast(tbl, C.POINTER(C.c_int32)), len(spec.get("table_pages", ())), spec.get("bin_tokens", 2048),
+                           spec.get("page_size", page_size))
     s._keep = tbl
     return s
 

@@ -37,7 +37,8 @@ int check_shape(const sparrow_shape_t *s)
     if (!s) return SPARROW_ERR_INVALID_ARG;
     if (s->n_seq < 0 || s->n_q_heads <= 0 || s->n_kv_heads <= 0 || s->max_pages_per_seq <= 0 || s->n_phys_pages < 0)
         return SPARROW_ERR_INVALID_ARG;
-    if (s->head_dim != kDim || s->page_size != kPage) return SPARROW_ERR_UNSUPPORTED;
+    if (s->head_dim != kDim) return SPARROW_ERR_UNSUPPORTED;
+    if (s->page_size != 16 && s->page_size != 32 && s->page_size != 64 && s->page_size != 128) return SPARROW_ERR_UNSUPPORTED;
     if (s->n_q_heads % s->n_kv_heads != 0) return SPARROW_ERR_UNSUPPORTED;
     const int r = s->n_q_heads / s->n_kv_heads;
     if (r < 1 || r > kMaxGroup) return SPARROW_ERR_UNSUPPORTED;
@@ -45,7 +46,8 @@ int check_shape(const sparrow_shape_t *s)
     return SPARROW_OK;
 }
 
-int to_dev_sched(const sparrow_schedule_t *in, SchedDev *out)
+// page_tokens: the shape's page size for the device entry points; 0 = take the schedule's own (host helpers), default 16
+int to_dev_sched(const sparrow_schedule_t *in, SchedDev *out, int page_tokens = 0)
 {
     if (!in) return SPARROW_ERR_INVALID_ARG;
     if (in->kind < SPARROW_SCHED_DENSE || in->kind > SPARROW_SCHED_TABLE) return SPARROW_ERR_INVALID_ARG;
@@ -61,6 +63,10 @@ int to_dev_sched(const sparrow_schedule_t *in, SchedDev *out)
     out->L0 = in->L0;
     out->L1 = in->L1;
     out->bin_tokens = in->bin_tokens;
+    if (in->page_size != 0 && in->page_size != 16 && in->page_size != 32 && in->page_size != 64 && in->page_size != 128)
+        return SPARROW_ERR_INVALID_ARG;
+    if (page_tokens != 0 && in->page_size != 0 && in->page_size != page_tokens) return SPARROW_ERR_INVALID_ARG;
+    out->page = page_tokens != 0 ? page_tokens : (in->page_size != 0 ? in->page_size : kPage);
     out->inv_den = 1.0;
     if (in->kind == SPARROW_SCHED_FIXED && in->fixed_tokens < 0) return SPARROW_ERR_INVALID_ARG;
     constexpr int64_t kPpmMax = 1000000;                 // keep fractions are in [0, 1]
@@ -94,7 +100,7 @@ DecodeGeom decode_geom(const sparrow_shape_t *s, int32_t max_sel /* 0 = dense */
     DecodeGeom gm;
     const size_t units = (size_t)s->n_seq * s->n_kv_heads;
     const int64_t max_cnt = (max_sel > 0 && max_sel < s->max_pages_per_seq) ? max_sel : s->max_pages_per_seq;
-    gm.max_rounds = decode_max_rounds((int64_t)units * max_cnt);
+    gm.max_rounds = decode_max_rounds((int64_t)units * max_cnt * (s->page_size / kPage));
     const size_t rows = (units + (size_t)kDecW * gm.max_rounds) * (s->n_q_heads / s->n_kv_heads);
     gm.bytes_o = (rows * kDim * sizeof(float) + 255) & ~(size_t)255;
     gm.bytes_ml = (rows * 2 * sizeof(float) + 255) & ~(size_t)255;
@@ -115,7 +121,8 @@ int launch_decode(const void *q, const void *k_cache, const void *v_cache, const
     if (s->n_seq > kDecMaxSeq) return SPARROW_ERR_UNSUPPORTED;
     {   // flat tile positions are 32-bit
         const int64_t max_cnt = kDense ? s->max_pages_per_seq : (max_sel < s->max_pages_per_seq ? max_sel : s->max_pages_per_seq);
-        if ((int64_t)s->n_seq * max_cnt * s->n_kv_heads >= (1LL << 31) || s->n_phys_pages * s->n_kv_heads >= (1LL << 31))
+        const int64_t tpp = s->page_size / kPage;
+        if ((int64_t)s->n_seq * max_cnt * s->n_kv_heads * tpp >= (1LL << 31) || s->n_phys_pages * s->n_kv_heads * tpp >= (1LL << 31))
             return SPARROW_ERR_UNSUPPORTED;
     }
     if (s->n_seq == 0) return SPARROW_OK;
@@ -140,6 +147,7 @@ int launch_decode(const void *q, const void *k_cache, const void *v_cache, const
     A.out = (uint16_t *)out; A.lse = lse; A.scale_log2 = scale_log2;
     A.n_seq = s->n_seq; A.n_q_heads = s->n_q_heads; A.n_kv_heads = s->n_kv_heads; A.max_pages = s->max_pages_per_seq;
     A.ready = nullptr;
+    A.tpp_log2 = s->page_size == 16 ? 0 : (s->page_size == 32 ? 1 : (s->page_size == 64 ? 2 : 3));
     decode_kernel<kDense><<<kDecGrid, kDecThreads, smem, st>>>(A, gm.max_rounds);
     SPARROW_CHECK_LAUNCH("decode_kernel");
     return SPARROW_OK;
@@ -153,7 +161,7 @@ int summarize_impl(const void *k_cache, void *summaries, const int32_t *page_ids
     const int64_t blocks = (tiles + kSumWarps - 1) / kSumWarps;
     if (blocks > 0x7fffffffLL) return SPARROW_ERR_UNSUPPORTED;
     summarize_kernel<<<(unsigned)blocks, kSumWarps * 32, 0, st>>>((const uint16_t *)k_cache, (uint16_t *)summaries,
-                                                                 page_ids, n_valid, n_update, s->n_kv_heads);
+                                                                 page_ids, n_valid, n_update, s->n_kv_heads, s->page_size);
     SPARROW_CHECK_LAUNCH("summarize_kernel");
     return SPARROW_OK;
 }
@@ -229,7 +237,7 @@ int step_impl(const void *q, const void *k_cache, const void *v_cache, const voi
     const bool per_warp = dyn_base + kDecWarps * keys * 4 <= kSmemBudget;
     const size_t dyn = dyn_base + (per_warp ? kDecWarps : 1) * keys * 4;
     static int fused_ok = -1;                    // -1 unknown, 0 the device cannot run the cooperative grid, 1 yes
-    bool fused = fused_ok != 0 && dyn <= kSmemBudget && s->n_seq <= kDecMaxSeq &&
+    bool fused = fused_ok != 0 && s->page_size == kPage && dyn <= kSmemBudget && s->n_seq <= kDecMaxSeq &&
                  s->n_phys_pages * s->n_kv_heads < (1LL << 27) &&
                  (int64_t)s->n_seq * s->max_pages_per_seq * s->n_kv_heads < (1LL << 31);
     if (fused && fused_ok < 0) {
@@ -260,6 +268,7 @@ int step_impl(const void *q, const void *k_cache, const void *v_cache, const voi
         A.out = (uint16_t *)out; A.lse = lse; A.scale_log2 = sm_scale * 1.4426950408889634f;
         A.n_seq = s->n_seq; A.n_q_heads = s->n_q_heads; A.n_kv_heads = s->n_kv_heads; A.max_pages = s->max_pages_per_seq;
         A.ready = reinterpret_cast<const int32_t *>(flags);
+        A.tpp_log2 = 0;
         S.summaries = (const uint16_t *)summaries;
         S.sel_pages = sel_pages; S.sel_count = sel_count;
         S.sel_counters = reinterpret_cast<int32_t *>(sel_ws);
@@ -296,7 +305,7 @@ const char *sparrow_strerror(int status)
     switch (status) {
     case SPARROW_OK: return "ok";
     case SPARROW_ERR_INVALID_ARG: return "invalid argument (null, negative or misaligned)";
-    case SPARROW_ERR_UNSUPPORTED: return "unsupported shape (need head_dim 128, page_size 16, 1 <= Hq/Hkv <= 8, bf16)";
+    case SPARROW_ERR_UNSUPPORTED: return "unsupported shape (need head_dim 128, page_size 16|32|64|128, 1 <= Hq/Hkv <= 8, bf16)";
     case SPARROW_ERR_WORKSPACE_TOO_SMALL: return "workspace too small";
     case SPARROW_ERR_CUDA: return g_errbuf[0] ? g_errbuf : "CUDA error";
     default: return "unknown status";
@@ -398,7 +407,7 @@ int sparrow_select(const void *q, const void *summaries, const int32_t *page_tab
     int rc = check_shape(shape);
     if (rc) return rc;
     SchedDev sd;
-    rc = to_dev_sched(sched, &sd);
+    rc = to_dev_sched(sched, &sd, shape->page_size);
     if (rc) return rc;
     if (!q || !summaries || !page_table || !seq_lens || !sel_pages || !sel_count || !workspace || max_sel <= 0)
         return SPARROW_ERR_INVALID_ARG;
@@ -450,7 +459,7 @@ int sparrow_append(const void *k_new, const void *v_new, void *k_cache, void *v_
     const int warps = shape->n_kv_heads < kAppendMaxWarps ? shape->n_kv_heads : kAppendMaxWarps;
     append_kernel<<<shape->n_seq, warps * 32, 0, (cudaStream_t)stream>>>(
         (const uint16_t *)k_new, (const uint16_t *)v_new, (uint16_t *)k_cache, (uint16_t *)v_cache, (uint16_t *)summaries,
-        page_table, seq_lens, shape->n_kv_heads, shape->max_pages_per_seq);
+        page_table, seq_lens, shape->n_kv_heads, shape->max_pages_per_seq, shape->page_size);
     SPARROW_CHECK_LAUNCH("append_kernel");
     return SPARROW_OK;
 }
@@ -471,7 +480,7 @@ int sparrow_step(const void *q, const void *k_cache, const void *v_cache, const 
     int rc = check_shape(shape);
     if (rc) return rc;
     SchedDev sd;
-    rc = to_dev_sched(sched, &sd);
+    rc = to_dev_sched(sched, &sd, shape->page_size);
     if (rc) return rc;
     if (!q || !k_cache || !v_cache || !summaries || !page_table || !seq_lens || !sel_pages || !sel_count || !out ||
         !workspace || max_sel <= 0)
@@ -529,7 +538,7 @@ int sparrow_step_host(const void *q_host, const int32_t *seq_lens_host, const in
     int rc = check_shape(s);
     if (rc) return rc;
     SchedDev sd;
-    rc = to_dev_sched(sched, &sd);
+    rc = to_dev_sched(sched, &sd, s->page_size);
     if (rc) return rc;
     if (!q_host || !seq_lens_host || !k_cache || !v_cache || !summaries || !page_table || !out_host || !scratch || max_sel <= 0)
         return SPARROW_ERR_INVALID_ARG;

@@ -10,7 +10,8 @@
 
 namespace sparrow {
 
-constexpr int kPage = 16;          // tokens per page
+constexpr int kPage = 16;          // tokens per TILE = the paper's page size; a larger page (32, 64, 128
+                                   // tokens: Table 4) is 2, 4 or 8 consecutive 16-token tiles
 constexpr int kDim = 128;          // head dim
 constexpr int kTileElems = kPage * kDim;        // one (page, kv-head) K or V tile: 2048 bf16 = 4 KiB
 constexpr int kTileBytes = kTileElems * 2;
@@ -19,6 +20,7 @@ constexpr int kSumElems = 2 * kDim;             // one (page, kv-head) summary: 
 // Schedule passed to kernels by value (no device memory, graph-capturable).
 struct SchedDev {
     int32_t kind, sink_tokens, local_tokens, table_len, bin_tokens;
+    int32_t page;                // tokens per page: 16, 32, 64 or 128
     int64_t fixed_tokens, floor_tokens, f0_ppm, f1_ppm, L0, L1;
     double inv_den;              // LINEAR_FRAC: 1.0 / (1e6 * (L1 - L0)), the quotient estimate's multiplier
     int32_t table[SPARROW_MAX_TABLE_BINS];
@@ -74,7 +76,7 @@ __host__ __device__ inline int64_t budget_tokens(const SchedDev &s, int64_t L)
 #endif
         if (b < 0) b = 0;
         if (b >= s.table_len) b = s.table_len - 1;
-        B = (int64_t)s.table[b] * kPage;
+        B = (int64_t)s.table[b] * s.page;
         break;
     }
     }
@@ -97,16 +99,16 @@ __host__ __device__ inline SeqPlan make_plan(const SchedDev &s, int64_t L)
 {
     SeqPlan pl;
     pl.L = (int32_t)L;
-    pl.n_pages = (int32_t)ceil_div64(L, kPage);
-    int64_t kp = ceil_div64(budget_tokens(s, L), kPage);                 // R4: ceil
+    pl.n_pages = (int32_t)ceil_div64(L, s.page);
+    int64_t kp = ceil_div64(budget_tokens(s, L), s.page);                // R4: ceil
     pl.k_pages = (int32_t)(kp < pl.n_pages ? kp : pl.n_pages);
-    int32_t ns = (int32_t)ceil_div64(s.sink_tokens, kPage);              // R8
+    int32_t ns = (int32_t)ceil_div64(s.sink_tokens, s.page);             // R8
     pl.n_sink = ns < pl.n_pages ? ns : pl.n_pages;
     int32_t t0 = pl.n_pages - 1;                                         // last page always kept (R9)
     if (s.local_tokens > 0) {
         int64_t lo = L - s.local_tokens;
         if (lo < 0) lo = 0;
-        int32_t fl = (int32_t)(lo / kPage);                              // R7: every page overlapping the window
+        int32_t fl = (int32_t)(lo / s.page);                             // R7: every page overlapping the window
         if (fl < t0) t0 = fl;
     }
     if (t0 < 0) t0 = 0;

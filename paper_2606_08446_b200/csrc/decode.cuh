@@ -166,6 +166,7 @@ struct DecodeArgs {
     float *lse;
     float scale_log2;
     int n_seq, n_q_heads, n_kv_heads, max_pages;
+    int tpp_log2;                // log2 of the 16-token tiles per page (page size 16, 32, 64, 128 -> 0, 1, 2, 3)
     const int32_t *ready;        // fused step only: per-unit flag, non-zero once the unit's page list is written
 };
 
@@ -214,9 +215,10 @@ __device__ __forceinline__ void decode_warp_stream(const DecodeArgs &A, const in
         int unit;        // stage A: sequence * Hkv + kv-head
         int info;        // stage A: bit 8 first tile of a segment, bit 9 last; stage B adds bits 0-4 = valid tokens
         int seq, logical, len, phys;
+        int sub;         // stage A: 16-token tile inside the page (pages larger than 16 tokens)
     };
     auto stage_a = [&](Lookup &m, int p, bool on, int ra, int rb) {
-        m.tile = 0; m.unit = 0; m.info = 0; m.seq = -1; m.logical = 0; m.len = 0; m.phys = 0;
+        m.tile = 0; m.unit = 0; m.info = 0; m.seq = -1; m.logical = 0; m.len = 0; m.phys = 0; m.sub = 0;
         if (on) {
             int lo = 0, hi = n_seq - 1;                          // last sequence whose first tile is <= p ...
             while (lo < hi) {
@@ -230,11 +232,13 @@ __device__ __forceinline__ void decode_warp_stream(const DecodeArgs &A, const in
             m.seq = seq;
             m.unit = seq * n_kv_heads + g;
             m.info = ((i == 0 || p == ra) ? kMetaFirst : 0) | ((i == c - 1 || p == rb - 1) ? kMetaLast : 0);
+            const int pi = i >> A.tpp_log2;                      // list position of the tile's page
+            m.sub = i - (pi << A.tpp_log2);
             if (kFused) {                                        // the list is written by this launch: wait for it
                 while (ld_acquire(A.ready + m.unit) == 0) __nanosleep(64);
-                m.logical = __ldcg(sel_pages + ((int64_t)m.unit) * max_sel + i);
+                m.logical = __ldcg(sel_pages + ((int64_t)m.unit) * max_sel + pi);
             } else {
-                m.logical = kDense ? i : __ldg(sel_pages + ((int64_t)m.unit) * max_sel + i);
+                m.logical = kDense ? pi : __ldg(sel_pages + ((int64_t)m.unit) * max_sel + pi);
             }
             m.len = __ldg(seq_lens + seq);
         }
@@ -242,12 +246,12 @@ __device__ __forceinline__ void decode_warp_stream(const DecodeArgs &A, const in
     auto stage_b = [&](Lookup &m) {
         if (m.seq >= 0) {
             m.phys = __ldg(page_table + (int64_t)m.seq * max_pages + m.logical);
-            int valid = m.len - m.logical * kPage;
+            int valid = m.len - ((m.logical << A.tpp_log2) + m.sub) * kPage;
             valid = valid < 0 ? 0 : (valid > kPage ? kPage : valid);
             m.info |= valid;
         }
     };
-    auto stage_c = [&](Lookup &m) { m.tile = m.phys * n_kv_heads + (m.unit - m.seq * n_kv_heads); };
+    auto stage_c = [&](Lookup &m) { m.tile = ((m.phys * n_kv_heads + (m.unit - m.seq * n_kv_heads)) << A.tpp_log2) + m.sub; };
 
     // ---- the warp's supply of ranges and windows ----
     int ra = 0, rb = 0, rp = 0;          // current range [ra, rb), next tile not yet in a window
@@ -556,7 +560,7 @@ __global__ void __launch_bounds__(kDecThreads, 1)
 decode_kernel(const DecodeArgs A, int max_rounds)
 {
     extern __shared__ __align__(1024) uint8_t smem[];
-    int32_t *s_prefix = reinterpret_cast<int32_t *>(smem + kDecRingBytes);     // [n_seq + 1] list entries before sequence i
+    int32_t *s_prefix = reinterpret_cast<int32_t *>(smem + kDecRingBytes);     // [n_seq + 1] tiles per kv-head before sequence i
     __shared__ int s_scan[kDecWarps];
     __shared__ DecSchedule s_sched;
 
@@ -573,9 +577,10 @@ decode_kernel(const DecodeArgs A, int max_rounds)
         const int s0 = min(tid * per, n_seq), s1 = min(s0 + per, n_seq);
         auto count_of = [&](int s) {
             int c;
-            if (kDense) c = (__ldg(seq_lens + s) + kPage - 1) / kPage;
+            const int page_tokens = kPage << A.tpp_log2;
+            if (kDense) c = (__ldg(seq_lens + s) + page_tokens - 1) / page_tokens;
             else { c = __ldg(A.sel_count + s); c = c < max_sel ? c : max_sel; }
-            return c > 0 ? c : 0;
+            return c > 0 ? c << A.tpp_log2 : 0;                  // in 16-token tiles
         };
         int sum = 0;
         for (int s = s0; s < s1; ++s) sum += count_of(s);

@@ -23,7 +23,7 @@ __device__ __forceinline__ uint32_t bf2_max(uint32_t a, uint32_t b)
 __global__ void __launch_bounds__(kSumWarps * 32)
 summarize_kernel(const uint16_t *__restrict__ k_cache, uint16_t *__restrict__ summaries,
                  const int32_t *__restrict__ page_ids, const int32_t *__restrict__ n_valid,
-                 int64_t n_update, int n_kv_heads)
+                 int64_t n_update, int n_kv_heads, int page_tokens)
 {
     const int lane = threadIdx.x & 31;
     const int64_t tile = (int64_t)blockIdx.x * kSumWarps + (threadIdx.x >> 5);   // (update, kv-head)
@@ -31,30 +31,32 @@ summarize_kernel(const uint16_t *__restrict__ k_cache, uint16_t *__restrict__ su
     const int64_t u = tile / n_kv_heads;
     const int g = (int)(tile % n_kv_heads);
     const int64_t page = page_ids ? (int64_t)page_ids[u] : u;
-    int valid = n_valid ? n_valid[u] : kPage;
-    valid = valid < 0 ? 0 : (valid > kPage ? kPage : valid);
+    int valid = n_valid ? n_valid[u] : page_tokens;
+    valid = valid < 0 ? 0 : (valid > page_tokens ? page_tokens : valid);
 
-    const uint16_t *src = k_cache + (page * n_kv_heads + g) * (int64_t)kTileElems;
+    const uint16_t *src = k_cache + (page * n_kv_heads + g) * (int64_t)page_tokens * kDim;     // page_tokens rows of 256 B
     const int half = lane >> 4;       // which of the two rows of this load
     const int c = lane & 15;          // 16-byte chunk (8 channels) of the row
 
     // +inf / -inf in both bf16 lanes: identity of min / max (a page with valid == 0 keeps them)
     uint32_t mn[4] = {0x7f807f80u, 0x7f807f80u, 0x7f807f80u, 0x7f807f80u};
     uint32_t mx[4] = {0xff80ff80u, 0xff80ff80u, 0xff80ff80u, 0xff80ff80u};
-    uint4 v[8];
+    for (int t0 = 0; t0 < valid; t0 += kPage) {      // one 16-token tile (4 KiB) at a time
+        uint4 v[8];
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {     // all loads first (8 x 16 B in flight per lane)
-        const int t = 2 * i + half;
-        if (t < valid) v[i] = ldg_stream16(src + t * kDim + c * 8);
-    }
+        for (int i = 0; i < 8; ++i) {     // all loads first (8 x 16 B in flight per lane)
+            const int t = t0 + 2 * i + half;
+            if (t < valid) v[i] = ldg_stream16(src + t * kDim + c * 8);
+        }
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
-        const int t = 2 * i + half;
-        if (t < valid) {
-            mn[0] = bf2_min(mn[0], v[i].x); mx[0] = bf2_max(mx[0], v[i].x);
-            mn[1] = bf2_min(mn[1], v[i].y); mx[1] = bf2_max(mx[1], v[i].y);
-            mn[2] = bf2_min(mn[2], v[i].z); mx[2] = bf2_max(mx[2], v[i].z);
-            mn[3] = bf2_min(mn[3], v[i].w); mx[3] = bf2_max(mx[3], v[i].w);
+        for (int i = 0; i < 8; ++i) {
+            const int t = t0 + 2 * i + half;
+            if (t < valid) {
+                mn[0] = bf2_min(mn[0], v[i].x); mx[0] = bf2_max(mx[0], v[i].x);
+                mn[1] = bf2_min(mn[1], v[i].y); mx[1] = bf2_max(mx[1], v[i].y);
+                mn[2] = bf2_min(mn[2], v[i].z); mx[2] = bf2_max(mx[2], v[i].z);
+                mn[3] = bf2_min(mn[3], v[i].w); mx[3] = bf2_max(mx[3], v[i].w);
+            }
         }
     }
 #pragma unroll

@@ -18,7 +18,7 @@ class SparrowEngine:
         assert wl.q.is_cuda, "the engine needs the workload on a CUDA device (no CPU fallback)"
         self.wl = wl
         dev = wl.q.device
-        self.shape = B.make_shape(wl.n_seq, wl.Hq, wl.Hkv, wl.max_pages, wl.n_phys)
+        self.shape = B.make_shape(wl.n_seq, wl.Hq, wl.Hkv, wl.max_pages, wl.n_phys, page_size=wl.page_size)
         self.set_schedule(schedule or wl.schedule)
         self.summaries = torch.zeros((wl.n_phys, wl.Hkv, 2, 128), dtype=torch.bfloat16, device=dev)
         self.sel_count = torch.zeros((wl.n_seq,), dtype=torch.int32, device=dev)
@@ -34,7 +34,7 @@ class SparrowEngine:
     def set_schedule(self, spec: dict):
         dev = self.wl.q.device
         self.sched_spec = dict(spec)
-        self.sched = B.make_schedule(spec)
+        self.sched = B.make_schedule(spec, page_size=self.wl.page_size)
         max_len = int(self.wl.seq_lens.max().item())
         self.max_sel = max(1, B.sparrow_max_sel_pages(self.sched, max_len))
         self.sel_pages = torch.full((self.wl.n_seq, self.wl.Hkv, self.max_sel), -1, dtype=torch.int32, device=dev)
@@ -83,7 +83,7 @@ class SparrowEngine:
     def reserve(self, n_steps: int):
         """Size the selection buffers for lengths up to the current maximum + n_steps (B(L) grows with L)."""
         max_len = int(self.wl.seq_lens.max().item()) + n_steps
-        assert max_len <= self.wl.max_pages * PAGE, "the page table has no room for that many appended tokens"
+        assert max_len <= self.wl.max_pages * self.wl.page_size, "the page table has no room for that many appended tokens"
         dev = self.wl.q.device
         self.max_sel = max(1, B.sparrow_max_sel_pages(self.sched, max_len))
         self.sel_pages = torch.full((self.wl.n_seq, self.wl.Hkv, self.max_sel), -1, dtype=torch.int32, device=dev)

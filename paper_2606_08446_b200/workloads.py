@@ -65,6 +65,7 @@ class Workload:
     planted: Optional[List[List[np.ndarray]]] = None   # [seq][kv-head] -> planted logical pages
     seed: int = 0
     meta: dict = field(default_factory=dict)
+    page_size: int = PAGE         # tokens per page: 16 (the paper's choice) or 32 / 64 / 128 (Table 4)
 
     @property
     def max_pages(self) -> int:
@@ -104,13 +105,14 @@ def draw_lengths(spec, n_seq: int, gen: torch.Generator) -> List[int]:
 def make_workload(name: str = "custom", *, n_seq: int, Hq: int, Hkv: int, lengths, schedule: dict,
                   plant: bool = False, seed: int = 0, device="cpu", spare_pages: int = 3,
                   poison_tail: bool = False, plant_scale: float = 3.0, plant_frac: float = 0.05,
-                  chunk_pages: int = 8192, reserve_tokens: int = 0, **_ignored) -> Workload:
+                  chunk_pages: int = 8192, reserve_tokens: int = 0, page_size: int = PAGE, **_ignored) -> Workload:
     """Draw one batch.  Lengths, page tables and planted pages come from a CPU generator (so they do
     not depend on the device); q/K/V values come from a generator on ``device``."""
     dev = torch.device(device)
     cg = torch.Generator(device="cpu").manual_seed(seed)
     dg = torch.Generator(device=dev).manual_seed(seed + 7919)
-    D, P = HEAD_DIM, PAGE
+    D, P = HEAD_DIM, page_size
+    chunk_pages = max(1, chunk_pages * PAGE // P)
     r = Hq // Hkv
     assert Hq == r * Hkv
 
@@ -175,7 +177,7 @@ def make_workload(name: str = "custom", *, n_seq: int, Hq: int, Hkv: int, length
         seq_lens=torch.tensor(lens, dtype=torch.int32, device=dev),
         page_table=page_table.to(dev), q=q, k_cache=k_cache, v_cache=v_cache,
         sm_scale=1.0 / math.sqrt(D), planted=planted, seed=seed,
-        meta=dict(lengths=lengths, n_pages_total=sum(n_pages), plant=plant),
+        meta=dict(lengths=lengths, n_pages_total=sum(n_pages), plant=plant), page_size=P,
     )
 
 
@@ -194,11 +196,12 @@ def full_page_updates(wl: Workload):
     pt = wl.page_table.cpu()
     ids, nv = [], []
     for i, L in enumerate(lens):
-        npg = -(-L // PAGE)
+        P = wl.page_size
+        npg = -(-L // P)
         ids.append(pt[i, :npg])
-        v = torch.full((npg,), PAGE, dtype=torch.int32)
-        if L % PAGE:
-            v[-1] = L % PAGE
+        v = torch.full((npg,), P, dtype=torch.int32)
+        if L % P:
+            v[-1] = L % P
         nv.append(v)
     return torch.cat(ids).to(torch.int32), torch.cat(nv)
 
@@ -207,8 +210,9 @@ def just_filled_updates(wl: Workload):
     """(page_ids, n_valid) of pages that became full at this decode step (L % 16 == 0)."""
     lens = wl.seq_lens.cpu().tolist()
     pt = wl.page_table.cpu()
-    ids = [int(pt[i, L // PAGE - 1]) for i, L in enumerate(lens) if L % PAGE == 0 and L > 0]
-    return torch.tensor(ids, dtype=torch.int32), torch.full((len(ids),), PAGE, dtype=torch.int32)
+    P = wl.page_size
+    ids = [int(pt[i, L // P - 1]) for i, L in enumerate(lens) if L % P == 0 and L > 0]
+    return torch.tensor(ids, dtype=torch.int32), torch.full((len(ids),), P, dtype=torch.int32)
 
 
 def make_rollout_inputs(wl: Workload, n_steps: int, seed: int = 0):

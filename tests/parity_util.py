@@ -44,13 +44,13 @@ def check_summaries(summ_gpu: torch.Tensor, h: dict, page_ids, n_valid):
     assert not bad.any(), f"summaries differ at {int(bad.sum())} of {bad.size} entries"
 
 
-def check_selection(res: dict, sel_gpu: np.ndarray, cnt_gpu: np.ndarray, seq_lens, scores_gpu=None) -> dict:
+def check_selection(res: dict, sel_gpu: np.ndarray, cnt_gpu: np.ndarray, seq_lens, scores_gpu=None, page_size: int = 16) -> dict:
     """res = oracle.sparse_step(...) for the same sequences.  Returns statistics."""
     n, Hkv, _ = sel_gpu.shape
     stats = dict(units=0, differing_units=0, band_pages=0)
     for i in range(n):
         L = int(seq_lens[i])
-        n_pages = -(-L // 16)
+        n_pages = -(-L // page_size)
         cnt = int(res["sel_count"][i])
         assert int(cnt_gpu[i]) == cnt, f"seq {i}: sel_count {int(cnt_gpu[i])} != oracle {cnt}"
         F = set(np.flatnonzero(res["forced"][i, :n_pages]).tolist())
@@ -109,14 +109,15 @@ def check_sparse_step(eng, wl, h=None, idx=None, check_summ=True) -> dict:
     sel_gpu = eng.sel_pages[tidx].cpu().numpy()
     cnt_gpu = eng.sel_count[tidx].cpu().numpy()
     scores_gpu = eng.scores[tidx].cpu().numpy() if eng.scores is not None else None
-    stats = check_selection(res, sel_gpu, cnt_gpu, hs["seq_lens"], scores_gpu)
+    P = getattr(wl, "page_size", 16)
+    stats = check_selection(res, sel_gpu, cnt_gpu, hs["seq_lens"], scores_gpu, page_size=P)
     if check_summ:
         # summaries of every page the checked sequences own
         ids, nv = [], []
         for i in range(len(idx)):
-            L = int(hs["seq_lens"][i]); npg = -(-L // 16)
-            ids.append(hs["page_table"][i, :npg]); v = np.full(npg, 16, np.int32)
-            if L % 16: v[-1] = L % 16
+            L = int(hs["seq_lens"][i]); npg = -(-L // P)
+            ids.append(hs["page_table"][i, :npg]); v = np.full(npg, P, np.int32)
+            if L % P: v[-1] = L % P
             nv.append(v)
         check_summaries(eng.summaries, h, np.concatenate(ids), np.concatenate(nv))
     if stats["differing_units"]:

@@ -222,3 +222,51 @@ def test_full_size_config_sampled_against_oracle(cfg, n_sample):
             rec += sum(p in row for p in pl); tot += min(len(pl), k)
     print(f"{cfg}: planted candidates recovered {rec}/{tot}")
     assert rec >= 0.8 * tot
+
+
+# ------------------------------------------------------------------ 8(f)-2: page sizes 32 / 64 / 128 ----
+@pytest.mark.parametrize("page", [32, 64, 128])
+@pytest.mark.parametrize("Hq,Hkv", [(8, 2), (5, 1)])
+def test_page_size_variants_match_oracle(page, Hq, Hkv):
+    """Table 4's page sizes: a page is streamed as page/16 tiles; summaries, selection, sparse and
+    dense attention against the oracle at that page size; ragged lengths around tile and page edges."""
+    lens = [1, 15, 16, 17, page - 1, page, page + 1, 3 * page + 5, 1000, 2049, 4099, 6000]
+    sched = W._sched("fixed", 16, 64, fixed_tokens=1024)          # Table 4's budget 1024: 32-32, 64-16, 128-8
+    wl = W.make_workload(n_seq=len(lens), Hq=Hq, Hkv=Hkv, lengths=("list", lens), schedule=sched, seed=page + Hq, device=DEV,
+                         poison_tail=True, plant=True, page_size=page)
+    eng = _run_sparse(wl, want_scores=True)                        # sparrow_step falls back to the two launches here
+    st = check_sparse_step(eng, wl)
+    assert eng.sel_count.cpu().tolist() == [min(-(-L // page), max(1024 // page, len(set([0]) | set(range(max(L - 64, 0) // page, -(-L // page)))))) for L in lens]
+    eng.dense_decode()
+    torch.cuda.synchronize()
+    check_dense(eng, wl)
+
+
+def test_rollout_with_page_size_64():
+    """append + summarize-on-fill + select + decode at page size 64: 70 steps cross a page edge for every sequence."""
+    from paper_2606_08446_b200.engine import SparrowEngine
+    T, lens = 70, [100, 1000, 4000]
+    sched = W._sched("clamp_frac", 64, 128, f0_ppm=250000, floor_tokens=512)
+    wl = W.make_workload(n_seq=3, Hq=8, Hkv=2, lengths=("list", lens), schedule=sched, seed=64, device=DEV, plant=True,
+                         page_size=64, reserve_tokens=T + 1)
+    eng = SparrowEngine(wl, want_scores=True)
+    eng.summarize_all(); eng.reserve(T)
+    qs, ks, vs = W.make_rollout_inputs(wl, T, seed=9)
+    bits = lambda t: t.contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
+    h0 = wl.host()
+    want, kc, vc = oracle.rollout(bits(qs), bits(ks), bits(vs), h0["k_cache"], h0["v_cache"], h0["page_table"], h0["seq_lens"],
+                                  oracle.Schedule.from_spec(sched), wl.sm_scale, max_sel=eng.max_sel)
+    out = torch.zeros((T, 3, 8, 128), dtype=torch.bfloat16, device=DEV)
+    lse = torch.zeros((T, 3, 8), dtype=torch.float32, device=DEV)
+    eng.rollout(qs, ks, vs, out, lse)
+    torch.cuda.synchronize()
+    assert np.array_equal(bits(wl.k_cache), kc) and np.array_equal(bits(wl.v_cache), vc)
+    filled = sorted(p for s in want for p in s["filled"])
+    assert len(filled) >= 3
+    check_summaries(eng.summaries, dict(k_cache=kc), np.array(filled), None)
+    from parity_util import check_selection
+    stats = check_selection(want[-1], eng.sel_pages.cpu().numpy(), eng.sel_count.cpu().numpy(), want[-1]["seq_lens"],
+                            eng.scores.cpu().numpy(), page_size=64)
+    if stats["differing_units"] == 0:
+        for t in (0, T // 2, T - 1):
+            check_outputs(out[t], lse[t], want[t]["out"], want[t]["lse"], f"page-64 rollout step {t}")

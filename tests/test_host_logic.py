@@ -92,11 +92,18 @@ def test_workspace_sizes_and_validation_without_a_gpu(B):
     assert 0 < sparse <= dense
     assert B.sparrow_step_scratch_bytes(shp, 128) > sparse + B.sparrow_select_workspace_bytes(shp)
     # unsupported shapes: status -2 before any pointer is touched; null pointers: -1.  No kernel is launched.
-    for bad in (B.make_shape(2, 4, 2, 64, 100, head_dim=64), B.make_shape(2, 4, 2, 64, 100, page_size=32),
+    for bad in (B.make_shape(2, 4, 2, 64, 100, head_dim=64), B.make_shape(2, 4, 2, 64, 100, page_size=48),
                 B.make_shape(2, 32, 2, 64, 100), B.make_shape(2, 5, 2, 64, 100)):
         assert B._lib.sparrow_summarize(None, None, None, None, 1, ctypes.byref(bad), None) == -2
         assert B.sparrow_decode_workspace_bytes(bad, 0) == 0
     ok = B.make_shape(2, 4, 2, 64, 100)
+    for page in (32, 64, 128):                                     # Table 4's page sizes are supported shapes
+        assert B.sparrow_decode_workspace_bytes(B.make_shape(2, 4, 2, 64, 100, page_size=page), 0) > 0
+    # the schedule's page size turns B(L) into pages: budget 1024 = 64 / 32 / 16 / 8 pages
+    for page, n in ((16, 64), (32, 32), (64, 16), (128, 8)):
+        sp = B.make_schedule(W._sched("fixed", 0, 0, fixed_tokens=1024), page_size=page)
+        assert B.sparrow_k_pages(sp, 20000) == n and B.sparrow_sel_count(sp, 20000) == n
+    assert B.sparrow_k_pages(B.make_schedule(W._sched("fixed", 0, 0, fixed_tokens=1024), page_size=48), 20000) == -1
     assert B._lib.sparrow_summarize(None, None, None, None, 1, ctypes.byref(ok), None) == -1
     assert B._lib.sparrow_summarize(None, None, None, None, 0, ctypes.byref(ok), None) == 0      # empty update: no-op
     s = B.make_schedule(W.CONFIGS["cfg1"]["schedule"])

@@ -463,3 +463,55 @@ def test_cost_model_against_per_step_sums_and_limits():
     base = [oracle.cost_model(0, 1, 1, 16384.0, 1.0, D_, r_, I_, ps_ * n_, ps_) for ps_, n_ in ((16., 64.), (32., 32.), (64., 16.), (128., 8.))]
     assert len({x["attn_elems_sparse"] for x in base}) == 1
     assert math.isclose(base[0]["landmark_visits"] / base[3]["landmark_visits"], 8.0)
+
+
+# ------------------------------------------------------------------ 8(f)-2: page sizes 32 / 64 / 128 (Table 4) ----
+@pytest.mark.parametrize("page", [32, 64, 128])
+def test_page_size_variants_whole_step_against_numpy_token_level(page):
+    """The oracle at page sizes other than 16 (16-64, 32-32, 64-16, 128-8 all mean budget 1024)
+    against a numpy restatement of the whole step written here at TOKEN level: summaries as min / max over each page's
+    valid tokens, score = sum over the group's heads and channels of max(q*mn, q*mx), forced = pages touching the
+    sink tokens, the last `W` tokens or the last token, top-k by (score desc, page asc), softmax over the valid tokens
+    of the kept pages."""
+    lens = [700, 129, 2000 + page // 2]
+    S, Wn, budget = 40, 200, 8 * page                      # budget in tokens: 8 pages whatever the page size
+    sched = W._sched("fixed", S, Wn, fixed_tokens=budget)
+    wl = W.make_workload(n_seq=3, Hq=4, Hkv=2, lengths=("list", lens), schedule=sched, seed=31 + page, device="cpu",
+                         page_size=page, plant=True)
+    h = wl.host()
+    assert h["k_cache"].shape[2] == page
+    res = oracle.sparse_step(h["q"], h["k_cache"], h["v_cache"], h["page_table"], h["seq_lens"], oracle.Schedule.from_spec(sched),
+                             wl.sm_scale)
+    Kf, Vf, Qf = f64(h["k_cache"]), f64(h["v_cache"]), f64(h["q"])
+    r = wl.Hq // wl.Hkv
+    for i, L in enumerate(lens):
+        n_pages = -(-L // page)
+        tok_page = np.arange(L) // page
+        forced = set(tok_page[:min(S, L)].tolist()) | set(tok_page[max(L - Wn, 0):].tolist()) | {int(tok_page[-1])}
+        K_pages = min(-(-min(budget, L) // page), n_pages)
+        want_cnt = n_pages if K_pages >= n_pages else max(K_pages, len(forced))
+        assert res["sel_count"][i] == want_cnt
+        for g in range(wl.Hkv):
+            keys = np.stack([Kf[h["page_table"][i, t // page], g, t % page] for t in range(L)])      # [L][D]
+            vals = np.stack([Vf[h["page_table"][i, t // page], g, t % page] for t in range(L)])
+            qg = Qf[i, g * r:(g + 1) * r]                                                              # [r][D]
+            score = np.full(n_pages, -np.inf)
+            for p in range(n_pages):
+                kp = keys[p * page:min((p + 1) * page, L)]
+                mn, mx = kp.min(0), kp.max(0)
+                score[p] = np.maximum(qg * mn, qg * mx).sum()
+            if K_pages >= n_pages:
+                keep = list(range(n_pages))
+            else:
+                cand = [p for p in range(n_pages) if p not in forced]
+                k = max(0, K_pages - len(forced))
+                order = sorted(cand, key=lambda p: (-score[p], p))[:k]
+                keep = sorted(forced | set(order))
+                assert np.allclose(res["scores"][i, g, cand], score[cand], rtol=1e-12, atol=1e-9)
+            assert res["sel"][i, g, :want_cnt].tolist() == keep
+            tok = np.concatenate([np.arange(p * page, min((p + 1) * page, L)) for p in keep])
+            for hh in range(r):
+                z = keys[tok] @ qg[hh] * wl.sm_scale
+                pr = np.exp(z - z.max()); pr /= pr.sum()
+                assert np.allclose(pr @ vals[tok], res["out"][i, g * r + hh], rtol=0, atol=1e-12)
+                assert abs(z.max() + math.log(np.exp(z - z.max()).sum()) - res["lse"][i, g * r + hh]) < 1e-12
