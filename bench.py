@@ -302,6 +302,47 @@ def run_cfg4(args, rank, local_rank, world, dev):
     print(json.dumps(line), flush=True)
 
 
+def run_table4(args, rank, dev):
+    """PAPER.md:426-434 (Table 4): sparse decode at KV budget 1024 tokens with page sizes 16 / 32 / 64 / 128 (configs
+    16-64, 32-32, 64-16, 128-8) and 16k / 24k / 32k tokens of past KV, Qwen3-1.7B attention shape, batch 16.  The paper
+    times a full-model decode pass on one H200 (4.1-5.4 ms, flat in the page size); this times the attention path of
+    ONE layer (select + sparse decode) on the B200, where the page size only changes the summary stream."""
+    if rank != 0:
+        return
+    from paper_2606_08446_b200.engine import SparrowEngine
+    rows = []
+    for past in (16384, 24576, 32768):
+        for page in (16, 32, 64, 128):
+            sched = W._sched("fixed", 64, 512, fixed_tokens=1024)
+            wl = W.make_workload("table4", n_seq=16, Hq=16, Hkv=8, lengths=("list", [past] * 16), schedule=sched, plant=True,
+                                 seed=4400 + page, device=dev, page_size=page)
+            eng = SparrowEngine(wl)
+            eng.summarize_all()
+            res = {}
+            for name, fn in (("select", eng.select), ("sparse_decode", eng.sparse_decode), ("dense_decode", eng.dense_decode)):
+                for _ in range(3):
+                    fn()
+                best = 1e9
+                for _ in range(3):
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    e0.record()
+                    for _ in range(args.steps):
+                        fn()
+                    e1.record(); torch.cuda.synchronize()
+                    best = min(best, e0.elapsed_time(e1) * 1e3 / args.steps)
+                res[name] = best
+            rows.append({"past_kv": past, "page_size": page, "pages_kept": int(eng.sel_count[0].item()),
+                         "select_us": res["select"], "sparse_decode_us": res["sparse_decode"],
+                         "sparse_us": res["select"] + res["sparse_decode"], "dense_decode_us": res["dense_decode"]})
+            del eng, wl
+            torch.cuda.empty_cache()
+    print(json.dumps({"table4": rows, "unit": "us per layer (attention path only)", "steps": args.steps,
+                      "config": {"workload": "table4", "n_seq": 16, "Hq": 16, "Hkv": 8, "budget_tokens": 1024, "sink_tokens": 64,
+                                 "local_tokens": 512},
+                      "paper_context": "Table 4 (PAPER.md:426-434): full-model decode pass 4.13-5.41 ms on 1xH200, flat in page size"}),
+          flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -312,6 +353,7 @@ def main():
     ap.add_argument("--impl", default="sparrow", choices=["sparrow", "reference"])
     ap.add_argument("--step-form", default="two-launches", choices=["two-launches", "fused"],
                     help="select + sparse decode as two launches (default, measured faster) or as the one cooperative sparrow_step launch")
+    ap.add_argument("--table4", action="store_true", help="page-size sweep at budget 1024 (PAPER.md Table 4) instead of the step benchmark")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-check", action="store_true", help="skip the sampled oracle self-check before timing")
     args = ap.parse_args()
@@ -325,6 +367,9 @@ def main():
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
     D.init("nccl")
+    if args.table4:
+        run_table4(args, rank, dev)
+        return
     if args.workload == "cfg4":
         run_cfg4(args, rank, local_rank, world, dev)
         return
