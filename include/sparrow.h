@@ -174,6 +174,21 @@ int sparrow_step_host(const void *q_host, const int32_t *seq_lens_host,
                       void *out_host, void *scratch, size_t scratch_bytes,
                       const sparrow_shape_t *shape, void *stream);
 
+/* ---- the paper's divergence statistic (SURVEY.md 8(f)-3; PAPER.md:76-79 Eq. 1, :95, :101, :119) -------------
+ * Per token position i < n_pos the dense policy P and the sparse policy Q each give their top_n (<= 32) tokens and
+ * natural-log probabilities: ids_p, logp_p, ids_q, logp_q are [n_pos][top_n].  alpha[i] = sum over the tokens present
+ * in BOTH lists of min(p, q) -- Eq. 1's sum_x min(p(x), q(x)) restricted to what the engine returns (reading R23; a
+ * token missing from one list adds nothing; ids are assumed distinct within a list).  Positions are grouped in bins
+ * b = min(positions[i] / bin_tokens, n_bins - 1) (2K-token bins in the paper); bin_count[b] = tokens in the bin and
+ * bin_quantile[b] = the nearest-rank `quantile` (0.05 in the paper) of alpha over the bin: the value of rank
+ * max(1, ceil(quantile * count)) in ascending order, NaN for an empty bin.  fp32 throughout; exact selection.
+ * workspace: sparrow_acceptance_workspace_bytes(n_bins) bytes, ZERO-INITIALISED once, restored by the call. */
+int sparrow_acceptance(const int32_t *ids_p, const float *logp_p, const int32_t *ids_q, const float *logp_q,
+                       const int32_t *positions, int64_t n_pos, int32_t top_n, int32_t bin_tokens, int32_t n_bins,
+                       float quantile, float *alpha, float *bin_quantile, int32_t *bin_count,
+                       void *workspace, size_t workspace_bytes, void *stream);
+size_t sparrow_acceptance_workspace_bytes(int32_t n_bins);
+
 /* ---- rollout cost model (SURVEY.md 8(f)-4; PAPER.md:129-145 Eq. 2-3, :474-498 App. F) -- host only ----------
  * Equivalent-FLOP cost of a rollout: batch_size x n_samples responses of L_out tokens after a prompt of L_in,
  * model of P parameters, K/V width D, GQA ratio r, hardware intensity I (flops per element moved; R18), KV budget K

@@ -23,5 +23,7 @@ from .oracle import (  # noqa: F401
     append_step,
     rollout,
     cost_model,
+    acceptance_rate,
+    binned_quantile,
     num_threads,
 )

@@ -6,6 +6,7 @@ bit patterns; everything the oracle returns is fp64 / integer numpy.
 from __future__ import annotations
 
 import ctypes as C
+import math
 import os
 import subprocess
 from dataclasses import dataclass, field
@@ -341,3 +342,37 @@ def cost_model(P, B, N, L_in, L_out, D, r, I, K, pagesize, c=1.0) -> dict:
                 dense_total=dense_comp + I * dense_mem, sparse_comp=sparse_comp, sparse_mem=sparse_mem,
                 scoring_comp=scoring_comp, scoring_mem=scoring_mem,
                 sparse_total=sparse_comp + scoring_comp + I * (sparse_mem + scoring_mem))
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# the paper's divergence statistic.  PAPER.md:76-79 (Eq. 1): alpha = E_{x~Q}[min(p(x)/q(x), 1)]
+# = sum_x min(p(x), q(x)); approximated from the top-20 tokens and logprobs per position; PAPER.md:101,
+# :119: tokens grouped by position in 2K bins, the statistic is the 5-percentile per bin.  fp64, plain loops.
+def acceptance_rate(ids_p, logp_p, ids_q, logp_q) -> np.ndarray:
+    """alpha per position from the two top-N lists ([n_pos][N] token ids and natural-log probabilities): the sum of
+    min(p, q) over the tokens present in both lists (reading R23: a token missing from a list adds nothing)."""
+    ids_p, ids_q = np.asarray(ids_p), np.asarray(ids_q)
+    p, q = np.exp(np.asarray(logp_p, dtype=np.float64)), np.exp(np.asarray(logp_q, dtype=np.float64))
+    alpha = np.zeros(len(ids_p), dtype=np.float64)
+    for i in range(len(ids_p)):
+        where_q = {int(t): j for j, t in enumerate(ids_q[i])}
+        for j, t in enumerate(ids_p[i]):
+            k = where_q.get(int(t))
+            if k is not None:
+                alpha[i] += min(p[i, j], q[i, k])
+    return alpha
+
+
+def binned_quantile(alpha, positions, bin_tokens: int, n_bins: int, quantile: float):
+    """Per length bin b = min(position // bin_tokens, n_bins - 1): (count, nearest-rank quantile) = the value of rank
+    max(1, ceil(quantile * count)) of the bin's alphas in ascending order; NaN for an empty bin."""
+    alpha, positions = np.asarray(alpha, dtype=np.float64), np.asarray(positions)
+    b = np.minimum(np.maximum(positions // bin_tokens, 0), n_bins - 1)
+    counts = np.zeros(n_bins, dtype=np.int64)
+    out = np.full(n_bins, np.nan)
+    for k in range(n_bins):
+        v = np.sort(alpha[b == k])
+        counts[k] = len(v)
+        if len(v):
+            out[k] = v[max(1, math.ceil(quantile * len(v))) - 1]
+    return counts, out

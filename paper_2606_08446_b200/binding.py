@@ -79,6 +79,8 @@ _SIGS = {
     "sparrow_select_workspace_bytes": (_sz, [_SHP]),
     "sparrow_decode_workspace_bytes": (_sz, [_SHP, _i32]),
     "sparrow_step_scratch_bytes": (_sz, [_SHP, _i32]),
+    "sparrow_acceptance": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _i64, _i32, _i32, _i32, _f, _vp, _vp, _vp, _vp, _sz, _vp]),
+    "sparrow_acceptance_workspace_bytes": (_sz, [_i32]),
     "sparrow_cost_model": (C.c_int, [C.POINTER(sparrow_cost_args_t), C.POINTER(sparrow_cost_t)]),
     "sparrow_budget_tokens": (_i64, [_SCH, _i64]),
     "sparrow_k_pages": (_i32, [_SCH, _i64]),
@@ -145,6 +147,21 @@ def sparrow_step_workspace_bytes(shape, max_sel: int) -> int:
 
 def sparrow_step_scratch_bytes(shape, max_sel: int) -> int:
     return _lib.sparrow_step_scratch_bytes(_by(shape), max_sel)
+
+
+def sparrow_acceptance_workspace_bytes(n_bins: int) -> int:
+    return _lib.sparrow_acceptance_workspace_bytes(n_bins)
+
+
+def sparrow_acceptance(ids_p, logp_p, ids_q, logp_q, positions, top_n: int, bin_tokens: int, n_bins: int, quantile: float,
+                       alpha, bin_quantile, bin_count, workspace, stream=None, *, check=True):
+    rc = _lib.sparrow_acceptance(_ptr(ids_p), _ptr(logp_p), _ptr(ids_q), _ptr(logp_q), _ptr(positions), int(positions.numel()),
+                                 top_n, bin_tokens, n_bins, quantile, _ptr(alpha), _ptr(bin_quantile), _ptr(bin_count),
+                                 _ptr(workspace), 0 if workspace is None else workspace.numel() * workspace.element_size(),
+                                 _stream(stream))
+    if check:
+        _check(rc, "sparrow_acceptance")
+    return rc
 
 
 def sparrow_cost_model(*, check=True, **kw) -> dict:

@@ -9,6 +9,7 @@
 #include "step.cuh"
 #include "summarize.cuh"
 #include "append.cuh"
+#include "accept.cuh"
 
 using namespace sparrow;
 
@@ -461,6 +462,50 @@ int sparrow_append(const void *k_new, const void *v_new, void *k_cache, void *v_
         (const uint16_t *)k_new, (const uint16_t *)v_new, (uint16_t *)k_cache, (uint16_t *)v_cache, (uint16_t *)summaries,
         page_table, seq_lens, shape->n_kv_heads, shape->max_pages_per_seq, shape->page_size);
     SPARROW_CHECK_LAUNCH("append_kernel");
+    return SPARROW_OK;
+}
+
+size_t sparrow_acceptance_workspace_bytes(int32_t n_bins)
+{
+    if (n_bins <= 0) return 0;
+    return align256((size_t)n_bins * kAccDigits * sizeof(int32_t)) + align256((size_t)n_bins * 4 * sizeof(uint32_t));
+}
+
+int sparrow_acceptance(const int32_t *ids_p, const float *logp_p, const int32_t *ids_q, const float *logp_q,
+                       const int32_t *positions, int64_t n_pos, int32_t top_n, int32_t bin_tokens, int32_t n_bins,
+                       float quantile, float *alpha, float *bin_quantile, int32_t *bin_count, void *workspace,
+                       size_t workspace_bytes, void *stream)
+{
+    g_launches = 0;
+    if (n_pos < 0 || top_n < 1 || top_n > 32 || bin_tokens <= 0 || n_bins <= 0 || n_bins > 65535 || !(quantile > 0.f) || !(quantile <= 1.f))
+        return SPARROW_ERR_INVALID_ARG;
+    if (!bin_quantile || !bin_count || !workspace) return SPARROW_ERR_INVALID_ARG;
+    if (n_pos > 0 && (!ids_p || !logp_p || !ids_q || !logp_q || !positions || !alpha)) return SPARROW_ERR_INVALID_ARG;
+    if (workspace_bytes < sparrow_acceptance_workspace_bytes(n_bins)) return SPARROW_ERR_WORKSPACE_TOO_SMALL;
+    cudaStream_t st = (cudaStream_t)stream;
+    int32_t *hist = reinterpret_cast<int32_t *>(workspace);
+    uint32_t *state = reinterpret_cast<uint32_t *>(reinterpret_cast<uint8_t *>(workspace) +
+                                                   align256((size_t)n_bins * kAccDigits * sizeof(int32_t)));
+    cudaError_t e = cudaMemsetAsync(state, 0, (size_t)n_bins * 4 * sizeof(uint32_t), st);
+    if (e != cudaSuccess) return cuda_fail(e, "memset(acceptance state)");
+    if (n_pos > 0) {
+        const int64_t blocks = (n_pos + kAccThreads / 32 - 1) / (kAccThreads / 32);
+        if (blocks > 0x7fffffffLL) return SPARROW_ERR_UNSUPPORTED;
+        accept_alpha_kernel<<<(unsigned)blocks, kAccThreads, 0, st>>>(ids_p, logp_p, ids_q, logp_q, n_pos, top_n, alpha);
+        SPARROW_CHECK_LAUNCH("accept_alpha_kernel");
+    }
+    // 3-pass radix select per bin over the fp32 bit patterns: bits 31..21, 20..10, 9..0
+    const int shifts[3] = {21, 10, 0}, bits[3] = {11, 11, 10};
+    int64_t gx = (n_pos + kAccThreads * 8 - 1) / (kAccThreads * 8);
+    gx = gx < 1 ? 1 : (gx > 4 * kNumSmsB200 ? 4 * kNumSmsB200 : gx);
+    for (int pass = 0; pass < 3; ++pass) {
+        accept_hist_kernel<<<dim3((unsigned)gx, (unsigned)n_bins), kAccThreads, 0, st>>>(alpha, positions, n_pos, bin_tokens, n_bins,
+                                                                                         shifts[pass], bits[pass], state, hist);
+        SPARROW_CHECK_LAUNCH("accept_hist_kernel");
+        accept_scan_kernel<<<n_bins, kAccThreads, 0, st>>>(hist, state, shifts[pass], bits[pass], pass == 0, quantile, pass == 2,
+                                                           bin_quantile, bin_count);
+        SPARROW_CHECK_LAUNCH("accept_scan_kernel");
+    }
     return SPARROW_OK;
 }
 

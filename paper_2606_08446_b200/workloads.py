@@ -223,3 +223,26 @@ def make_rollout_inputs(wl: Workload, n_steps: int, seed: int = 0):
     def draw(h):
         return torch.randn((n_steps, wl.n_seq, h, HEAD_DIM), generator=g, device=dev, dtype=torch.float32).to(torch.bfloat16)
     return draw(wl.Hq), draw(wl.Hkv), draw(wl.Hkv)
+
+
+def make_acceptance_inputs(n_traj: int, max_len: int, top_n: int = 20, vocab: int = 2048, seed: int = 0, device="cpu"):
+    """Synthetic stand-in for what the inference engine returns for the paper's divergence study: per
+    generated token the top-N token ids and log-probabilities under the dense policy P and the sparse policy Q.
+    Logits P ~ N(0, 2^2); Q = P + noise whose scale grows with the token position (the mismatch grows with length,
+    PAPER.md:99-103).  Trajectory lengths uniform in [max_len / 4, max_len].  Input generation only."""
+    dev = torch.device(device)
+    cg = torch.Generator(device="cpu").manual_seed(seed)
+    dg = torch.Generator(device=dev).manual_seed(seed + 15485863)
+    lens = torch.randint(max(1, max_len // 4), max_len + 1, (n_traj,), generator=cg)
+    positions = torch.cat([torch.arange(int(L), dtype=torch.int32) for L in lens]).to(dev)
+    n_pos = int(positions.numel())
+    out = {k: [] for k in ("ids_p", "logp_p", "ids_q", "logp_q")}
+    for a in range(0, n_pos, 16384):
+        pos = positions[a:a + 16384].float()
+        lp = 2.0 * torch.randn((len(pos), vocab), generator=dg, device=dev)
+        lq = lp + (0.05 + 0.6 * pos / max_len).unsqueeze(1) * torch.randn((len(pos), vocab), generator=dg, device=dev)
+        for name, logits in (("p", lp), ("q", lq)):
+            lsm = torch.log_softmax(logits, dim=-1)
+            val, idx = lsm.topk(top_n, dim=-1)
+            out["ids_" + name].append(idx.to(torch.int32)); out["logp_" + name].append(val.float())
+    return {k: torch.cat(v).contiguous() for k, v in out.items()} | {"positions": positions, "lens": lens}

@@ -515,3 +515,44 @@ def test_page_size_variants_whole_step_against_numpy_token_level(page):
                 pr = np.exp(z - z.max()); pr /= pr.sum()
                 assert np.allclose(pr @ vals[tok], res["out"][i, g * r + hh], rtol=0, atol=1e-12)
                 assert abs(z.max() + math.log(np.exp(z - z.max()).sum()) - res["lse"][i, g * r + hh]) < 1e-12
+
+
+# ------------------------------------------------------------------ 8(f)-3: acceptance rate (Eq. 1) and its tail ----
+def test_acceptance_rate_eq1_identity_and_special_cases():
+    """PAPER.md:76-79 Eq. 1: with the lists covering the whole vocabulary, alpha = sum_x min(p, q) must equal the
+    expectation form E_{x~Q}[min(p/q, 1)] and 1 - total-variation distance, both computed here from the definitions;
+    identical policies give 1, disjoint supports give 0; list order does not matter."""
+    rng = np.random.default_rng(3)
+    V, n = 50, 40
+    lp = rng.normal(size=(n, V)); lq = lp + 0.7 * rng.normal(size=(n, V))
+    lp -= np.log(np.exp(lp).sum(1, keepdims=True)); lq -= np.log(np.exp(lq).sum(1, keepdims=True))
+    ids = np.tile(np.arange(V), (n, 1))
+    perm = np.stack([rng.permutation(V) for _ in range(n)])
+    a = oracle.acceptance_rate(ids, lp, np.take_along_axis(ids, perm, 1), np.take_along_axis(lq, perm, 1))
+    p, q = np.exp(lp), np.exp(lq)
+    assert np.allclose(a, (q * np.minimum(p / q, 1.0)).sum(1), rtol=0, atol=1e-14)           # expectation under Q
+    assert np.allclose(a, 1.0 - 0.5 * np.abs(p - q).sum(1), rtol=0, atol=1e-14)             # 1 - TV distance
+    assert np.allclose(oracle.acceptance_rate(ids, lp, ids, lp), 1.0, atol=1e-14)
+    assert np.all(oracle.acceptance_rate(ids[:, :20], lp[:, :20], ids[:, 25:45], lq[:, 25:45]) == 0.0)
+    # truncated lists: only shared tokens count (R23): here exactly tokens 10..19
+    got = oracle.acceptance_rate(ids[:, :20], lp[:, :20], ids[:, 10:30], lq[:, 10:30])
+    assert np.allclose(got, np.minimum(p[:, 10:20], q[:, 10:20]).sum(1), atol=1e-15)
+
+
+def test_binned_quantile_is_the_nearest_rank_quantile():
+    """The 5-percentile per 2K-position bin against numpy's own inverted-CDF quantile, and the
+    bin edges / empty bins by hand."""
+    rng = np.random.default_rng(4)
+    pos = rng.integers(0, 9000, size=5000)
+    alpha = rng.beta(8, 1, size=5000)
+    counts, qv = oracle.binned_quantile(alpha, pos, 2048, 6, 0.05)
+    for b in range(6):
+        sel = alpha[np.minimum(pos // 2048, 5) == b]
+        assert counts[b] == len(sel)
+        if len(sel):
+            assert qv[b] == np.quantile(sel, 0.05, method="inverted_cdf")
+        else:
+            assert np.isnan(qv[b])
+    assert counts[5] == 0 and counts[4] == (pos >= 8192).sum()
+    c, v = oracle.binned_quantile([0.5, 0.1, 0.9, 0.3], [0, 2047, 2048, 5000], 2048, 2, 0.5)
+    assert c.tolist() == [2, 2] and v.tolist() == [0.1, 0.3]                                  # rank ceil(0.5 * 2) = 1
