@@ -31,6 +31,25 @@ int cuda_fail(cudaError_t e, const char *where)
         ++g_launches;                                       \
     } while (0)
 
+// Launch of a kernel of the step chain with programmatic stream serialization (see chain_entry() in common.cuh).
+template <typename... KArgs, typename... Args>
+cudaError_t launch_chain(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args &&...args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+#ifndef SPARROW_NO_PDL
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+#endif
+    return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
 bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 int check_shape(const sparrow_shape_t *s)
@@ -149,7 +168,7 @@ int launch_decode(const void *q, const void *k_cache, const void *v_cache, const
     A.n_seq = s->n_seq; A.n_q_heads = s->n_q_heads; A.n_kv_heads = s->n_kv_heads; A.max_pages = s->max_pages_per_seq;
     A.ready = nullptr;
     A.tpp_log2 = s->page_size == 16 ? 0 : (s->page_size == 32 ? 1 : (s->page_size == 64 ? 2 : 3));
-    decode_kernel<kDense><<<kDecGrid, kDecThreads, smem, st>>>(A, gm.max_rounds);
+    launch_chain(decode_kernel<kDense>, dim3(kDecGrid), dim3(kDecThreads), smem, st, A, gm.max_rounds);
     SPARROW_CHECK_LAUNCH("decode_kernel");
     return SPARROW_OK;
 }
@@ -161,8 +180,8 @@ int summarize_impl(const void *k_cache, void *summaries, const int32_t *page_ids
     const int64_t tiles = n_update * s->n_kv_heads;
     const int64_t blocks = (tiles + kSumWarps - 1) / kSumWarps;
     if (blocks > 0x7fffffffLL) return SPARROW_ERR_UNSUPPORTED;
-    summarize_kernel<<<(unsigned)blocks, kSumWarps * 32, 0, st>>>((const uint16_t *)k_cache, (uint16_t *)summaries,
-                                                                 page_ids, n_valid, n_update, s->n_kv_heads, s->page_size);
+    launch_chain(summarize_kernel, dim3((unsigned)blocks), dim3(kSumWarps * 32), 0, st, (const uint16_t *)k_cache,
+                 (uint16_t *)summaries, page_ids, n_valid, n_update, s->n_kv_heads, s->page_size);
     SPARROW_CHECK_LAUNCH("summarize_kernel");
     return SPARROW_OK;
 }
@@ -196,9 +215,9 @@ int select_impl(const void *q, const void *summaries, const int32_t *page_table,
         dyn_set = dyn;
     }
     dim3 grid((s->max_pages_per_seq + pages_per_cta - 1) / pages_per_cta, s->n_kv_heads, s->n_seq);
-    select_kernel<<<grid, kSelThreads, dyn, st>>>((const uint16_t *)q, (const uint16_t *)summaries, page_table, seq_lens,
-                                                  sd, sel_pages, max_sel, sel_count, scores_ws, counters, scores_dbg,
-                                                  s->n_q_heads, s->n_kv_heads, s->max_pages_per_seq, pages_per_cta);
+    launch_chain(select_kernel, grid, dim3(kSelThreads), dyn, st, (const uint16_t *)q, (const uint16_t *)summaries, page_table,
+                 seq_lens, sd, sel_pages, max_sel, sel_count, scores_ws, counters, scores_dbg, s->n_q_heads, s->n_kv_heads,
+                 s->max_pages_per_seq, pages_per_cta);
     SPARROW_CHECK_LAUNCH("select_kernel");
     return SPARROW_OK;
 }
@@ -458,9 +477,9 @@ int sparrow_append(const void *k_new, const void *v_new, void *k_cache, void *v_
         return SPARROW_ERR_INVALID_ARG;
     if (shape->n_seq == 0) return SPARROW_OK;
     const int warps = shape->n_kv_heads < kAppendMaxWarps ? shape->n_kv_heads : kAppendMaxWarps;
-    append_kernel<<<shape->n_seq, warps * 32, 0, (cudaStream_t)stream>>>(
-        (const uint16_t *)k_new, (const uint16_t *)v_new, (uint16_t *)k_cache, (uint16_t *)v_cache, (uint16_t *)summaries,
-        page_table, seq_lens, shape->n_kv_heads, shape->max_pages_per_seq, shape->page_size);
+    launch_chain(append_kernel, dim3(shape->n_seq), dim3(warps * 32), 0, (cudaStream_t)stream, (const uint16_t *)k_new,
+                 (const uint16_t *)v_new, (uint16_t *)k_cache, (uint16_t *)v_cache, (uint16_t *)summaries, page_table, seq_lens,
+                 shape->n_kv_heads, shape->max_pages_per_seq, shape->page_size);
     SPARROW_CHECK_LAUNCH("append_kernel");
     return SPARROW_OK;
 }

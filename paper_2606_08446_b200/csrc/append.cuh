@@ -17,6 +17,7 @@ append_kernel(const uint16_t *__restrict__ k_new, const uint16_t *__restrict__ v
               uint16_t *__restrict__ v_cache, uint16_t *__restrict__ summaries, const int32_t *__restrict__ page_table,
               int32_t *__restrict__ seq_lens, int n_kv_heads, int max_pages, int page_tokens)
 {
+    chain_entry();
     const int seq = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int L = seq_lens[seq];                         // tokens cached before this step
     __syncthreads();                                     // every warp has read L

@@ -136,6 +136,18 @@ __device__ __forceinline__ uint4 ldg_stream16(const void *p)
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
+// ---- programmatic dependent launch: the step's kernels (summarize / append -> select -> decode) are launched with
+// cudaLaunchAttributeProgrammaticStreamSerialization, so the next kernel's CTAs can be brought up while this one
+// drains.  Every kernel calls this first: it lets its dependents start launching and then waits until everything
+// before it in the stream has completed and is visible -- nothing is read or written before that point.
+__device__ __forceinline__ void chain_entry()
+{
+#ifndef SPARROW_NO_PDL
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+#endif
+}
+
 // ---- mbarrier + bulk-copy (TMA) primitives; shared-memory operands are 32-bit shared::cta addresses ----
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
 {

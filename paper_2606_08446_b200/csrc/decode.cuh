@@ -559,6 +559,7 @@ template <bool kDense>
 __global__ void __launch_bounds__(kDecThreads, 1)
 decode_kernel(const DecodeArgs A, int max_rounds)
 {
+    chain_entry();
     extern __shared__ __align__(1024) uint8_t smem[];
     int32_t *s_prefix = reinterpret_cast<int32_t *>(smem + kDecRingBytes);     // [n_seq + 1] tiles per kv-head before sequence i
     __shared__ int s_scan[kDecWarps];

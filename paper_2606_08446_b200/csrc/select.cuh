@@ -28,7 +28,10 @@ constexpr int kSelThreads = 256;
 constexpr int kSelWarps = kSelThreads / 32;
 constexpr int kSelPagesPerWarp = 32;                    // one warp-chunk: one lane per page-table entry
 constexpr int kSelBatch = 8;                            // summaries in flight per warp
-constexpr int kSelMinBlocks = 4;                        // CTAs / SM the register budget is held to
+#ifndef SPARROW_SEL_MIN_BLOCKS
+#define SPARROW_SEL_MIN_BLOCKS 4
+#endif
+constexpr int kSelMinBlocks = SPARROW_SEL_MIN_BLOCKS;   // CTAs / SM the register budget is held to
 constexpr int kSelCtaPagesMin = kSelWarps * kSelPagesPerWarp;                // pages_per_cta is a multiple of this
 constexpr int kSelMaxPages = 16384;  // keys of one unit live in shared memory (64 KiB): 262144 tokens
 
@@ -79,6 +82,7 @@ select_kernel(const uint16_t *__restrict__ q, const uint16_t *__restrict__ summa
               float *__restrict__ scores_ws, int32_t *__restrict__ counters, float *__restrict__ scores_dbg,
               int n_q_heads, int n_kv_heads, int max_pages, int pages_per_cta)
 {
+    chain_entry();
     extern __shared__ uint32_t s_keys[];                 // [n_pages] (phase B only)
     __shared__ float s_q[2][kDim];                       // [0] = Q- (pairs with min), [1] = Q+ (pairs with max)
     __shared__ int s_hist[256];

@@ -279,6 +279,7 @@ struct ChunkDesc {
 __global__ void __launch_bounds__(kDecThreads, 1)
 step_kernel(const StepArgs S, const SchedDev sched)
 {
+    chain_entry();
     extern __shared__ __align__(1024) uint8_t smem[];
     const DecodeArgs &A = S.dec;
     const int n_seq = A.n_seq, n_kv_heads = A.n_kv_heads, max_sel = A.max_sel, max_pages = A.max_pages;

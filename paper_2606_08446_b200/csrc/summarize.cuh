@@ -25,6 +25,7 @@ summarize_kernel(const uint16_t *__restrict__ k_cache, uint16_t *__restrict__ su
                  const int32_t *__restrict__ page_ids, const int32_t *__restrict__ n_valid,
                  int64_t n_update, int n_kv_heads, int page_tokens)
 {
+    chain_entry();
     const int lane = threadIdx.x & 31;
     const int64_t tile = (int64_t)blockIdx.x * kSumWarps + (threadIdx.x >> 5);   // (update, kv-head)
     if (tile >= n_update * n_kv_heads) return;
