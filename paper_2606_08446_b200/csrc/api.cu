@@ -508,18 +508,30 @@ int sparrow_acceptance(const int32_t *ids_p, const float *logp_p, const int32_t 
     cudaError_t e = cudaMemsetAsync(state, 0, (size_t)n_bins * 4 * sizeof(uint32_t), st);
     if (e != cudaSuccess) return cuda_fail(e, "memset(acceptance state)");
     if (n_pos > 0) {
-        const int64_t blocks = (n_pos + kAccThreads / 32 - 1) / (kAccThreads / 32);
+        const int64_t per_block = (int64_t)(kAccThreads / 32) * kAccPosPerWarp;
+        const int64_t blocks = (n_pos + per_block - 1) / per_block;
         if (blocks > 0x7fffffffLL) return SPARROW_ERR_UNSUPPORTED;
         accept_alpha_kernel<<<(unsigned)blocks, kAccThreads, 0, st>>>(ids_p, logp_p, ids_q, logp_q, n_pos, top_n, alpha);
         SPARROW_CHECK_LAUNCH("accept_alpha_kernel");
     }
     // 3-pass radix select per bin over the fp32 bit patterns: bits 31..21, 20..10, 9..0
     const int shifts[3] = {21, 10, 0}, bits[3] = {11, 11, 10};
+    // bins per histogram block: as many 8 KiB histograms as fit in 200 KiB of shared memory (one CTA per SM then)
+    const int bins_per_group = n_bins < 25 ? n_bins : 25;
+    const int groups = (n_bins + bins_per_group - 1) / bins_per_group;
+    const size_t hsmem = (size_t)bins_per_group * kAccDigits * sizeof(int);
+    static size_t hsmem_set = 0;
+    if (hsmem > 48 * 1024 && hsmem > hsmem_set) {
+        e = cudaFuncSetAttribute(accept_hist_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)hsmem);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(accept_hist_kernel)");
+        hsmem_set = hsmem;
+    }
     int64_t gx = (n_pos + kAccThreads * 8 - 1) / (kAccThreads * 8);
-    gx = gx < 1 ? 1 : (gx > 4 * kNumSmsB200 ? 4 * kNumSmsB200 : gx);
+    const int64_t gmax = (hsmem > 100 * 1024 ? 1 : 2) * kNumSmsB200;
+    gx = gx < 1 ? 1 : (gx > gmax ? gmax : gx);
     for (int pass = 0; pass < 3; ++pass) {
-        accept_hist_kernel<<<dim3((unsigned)gx, (unsigned)n_bins), kAccThreads, 0, st>>>(alpha, positions, n_pos, bin_tokens, n_bins,
-                                                                                         shifts[pass], bits[pass], state, hist);
+        accept_hist_kernel<<<dim3((unsigned)gx, (unsigned)groups), kAccThreads, hsmem, st>>>(
+            alpha, positions, n_pos, bin_tokens, n_bins, bins_per_group, shifts[pass], bits[pass], state, hist);
         SPARROW_CHECK_LAUNCH("accept_hist_kernel");
         accept_scan_kernel<<<n_bins, kAccThreads, 0, st>>>(hist, state, shifts[pass], bits[pass], pass == 0, quantile, pass == 2,
                                                            bin_quantile, bin_count);
