@@ -126,6 +126,16 @@ def time_oracle_sample(wl, h, budget_s=12.0):
         if len(idx) >= wl.n_seq or dt * 2.2 > budget_s:
             break
         n_try = min(wl.n_seq, max(n_try + 1, int(n_try * min(4.0, budget_s / max(dt, 1e-3) / 2.2))))
+    # the whole batch fits the budget many times over: repeat the step for ~10 s of CPU work and take the mean
+    if best[0] >= wl.n_seq and best[1] < budget_s / 4:
+        reps = int(min(200, max(2, (budget_s * 0.8) // max(best[1], 1e-3))))
+        idx = np.arange(wl.n_seq)
+        sub = (np.ascontiguousarray(h["q"][idx]), h["k_cache"], h["v_cache"], np.ascontiguousarray(h["page_table"][idx]),
+               np.ascontiguousarray(h["seq_lens"][idx]))
+        t0 = time.perf_counter()
+        for _ in range(reps):
+            oracle.sparse_step(*sub, sched, wl.sm_scale)
+        best = (wl.n_seq, (time.perf_counter() - t0) / reps)
     return best[0], best[1], oracle.num_threads()
 
 
@@ -600,7 +610,7 @@ def main():
         h = h or wl.host()
         n_s, dt, cores = time_oracle_sample(wl, h)
         line["cpu_baseline"] = {"value": n_s / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                "sample": f"first {n_s} of {wl.n_seq} sequences of {args.workload}: one full select + sparse-attention step in {dt:.2f} s"}
+                                "sample": f"first {n_s} of {wl.n_seq} sequences of {args.workload}: full select + sparse-attention steps, {dt:.3f} s each (mean over ~10 s of CPU work when one step is short)"}
     print(json.dumps(line), flush=True)
 
 
