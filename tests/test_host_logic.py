@@ -64,15 +64,17 @@ def test_host_schedule_agrees_with_oracle_on_random_lengths(B):
     specs += [W._sched("table", 40, 300, table_pages=(8, 16, 64, 100, 128), bin_tokens=2048),
               W._sched("dense", 0, 0), W._sched("fixed", 0, 0, fixed_tokens=1), W._sched("fixed", 1000, 5, fixed_tokens=100)]
     for spec in specs:
-        s, so = B.make_schedule(spec), oracle.Schedule.from_spec(spec)
-        for L in [1, 2, 15, 16, 17, 31, 32, 33] + rng.integers(1, 45000, 300).tolist():
-            assert B.sparrow_budget_tokens(s, L) == oracle.budget_tokens(so, L), (spec, L)
-            K = oracle.k_pages(so, L)
-            assert B.sparrow_k_pages(s, L) == K
-            F = int(oracle.forced_pages(L, so.sink_tokens, so.local_tokens).sum())
-            assert B.sparrow_forced_count(s, L) == F
-            n_pages = -(-L // 16)
-            assert B.sparrow_sel_count(s, L) == (n_pages if K >= n_pages else max(K, F))
+        for page in (16, 32, 64, 128):                           # Table 4's page sizes
+            s, so = B.make_schedule(spec, page_size=page), oracle.Schedule.from_spec(spec)
+            lens = [1, 2, 15, 16, 17, 31, 32, 33, 127, 128, 129] + rng.integers(1, 45000, 300 if page == 16 else 80).tolist()
+            for L in lens:
+                assert B.sparrow_budget_tokens(s, L) == oracle.budget_tokens(so, L, page), (spec, L, page)
+                K = oracle.k_pages(so, L, page)
+                assert B.sparrow_k_pages(s, L) == K
+                F = int(oracle.forced_pages(L, so.sink_tokens, so.local_tokens, page).sum())
+                assert B.sparrow_forced_count(s, L) == F
+                n_pages = -(-L // page)
+                assert B.sparrow_sel_count(s, L) == (n_pages if K >= n_pages else max(K, F))
 
 
 def test_max_sel_pages_bounds_every_length(B):
