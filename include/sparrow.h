@@ -60,7 +60,17 @@ typedef struct sparrow_shape {
     int32_t page_size;           /* P: 16 (the paper's choice) or 32 / 64 / 128 (Table 4) */
     int32_t max_pages_per_seq;   /* row stride of page_table */
     int64_t n_phys_pages;        /* pages in the K/V pools */
+    int32_t landmark;            /* SPARROW_LANDMARK_MINMAX (0, north_star's default) or SPARROW_LANDMARK_MEAN (1) */
 } sparrow_shape_t;
+
+/* Form of the page landmark (PAPER.md:147 leaves it open; reading R1):
+ *   MINMAX  per-channel min and max of the page's keys, summaries [n_phys_pages][n_kv_heads][2][128] (512 B), score =
+ *           sum_{h in group} sum_d max(q*min, q*max) -- an upper bound of q.k over the page (north_star's default)
+ *   MEAN    the mean key, summaries [n_phys_pages][n_kv_heads][128] (256 B), score = sum_{h in group} q_h . mean -- the
+ *           one-vector-per-page landmark that the paper's cost model charges.  mean = fp32 sum of the
+ *           valid tokens in token order, divided by their number, rounded once to bf16.
+ * Everything else (budget, forced pages, top-k, attention) is the same.  sparrow_step uses the two launches for MEAN. */
+enum { SPARROW_LANDMARK_MINMAX = 0, SPARROW_LANDMARK_MEAN = 1 };
 
 /* Dynamic sparsity schedule B(L) in EXACT integer arithmetic (R3), so that host, device and any checker
  * agree bit for bit.  Fractions are parts per million in [0, 1000000] (L1 - L0 < 2^31); anything else is

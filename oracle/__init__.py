@@ -25,5 +25,7 @@ from .oracle import (  # noqa: F401
     cost_model,
     acceptance_rate,
     binned_quantile,
+    summarize_mean,
+    sparse_step_mean,
     num_threads,
 )

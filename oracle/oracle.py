@@ -376,3 +376,70 @@ def binned_quantile(alpha, positions, bin_tokens: int, n_bins: int, quantile: fl
         if len(v):
             out[k] = v[max(1, math.ceil(quantile * len(v))) - 1]
     return counts, out
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# SURVEY.md 8(f)-2, landmark variant: ONE vector per page, the mean key -- the landmark the paper's cost model charges
+# (D elements per page; the form itself is left open at :147, reading R1).  The landmark is a stored
+# bf16 code, so it is computed in the precision that decides the code (the kernel's): fp32 accumulation over the
+# page's valid tokens in token order, one fp32 division, one rounding to bf16 (nearest even).  Everything after it
+# (score, top-k, attention) is fp64 as in O5..O8.
+def _bf16_round_bits(x32: np.ndarray) -> np.ndarray:
+    u = x32.astype(np.float32).view(np.uint32).astype(np.uint64)
+    return (((u + 0x7FFF + ((u >> 16) & 1)) >> 16) & 0xFFFF).astype(np.uint16)
+
+
+def summarize_mean(k_cache, page_ids, n_valid=None) -> np.ndarray:
+    """k_cache [n_phys][Hkv][P][D] uint16 (bf16 bits) -> mean-key landmarks [n_update][Hkv][D] as bf16 BITS (uint16)."""
+    k_cache = _u16(k_cache)
+    P = k_cache.shape[2]
+    out = np.zeros((len(page_ids), k_cache.shape[1], k_cache.shape[3]), dtype=np.uint16)
+    for u, page in enumerate(page_ids):
+        valid = P if n_valid is None else int(n_valid[u])
+        rows = (k_cache[int(page)].astype(np.uint32) << 16).view(np.float32)          # [Hkv][P][D] exact fp32
+        acc = np.zeros((rows.shape[0], rows.shape[2]), dtype=np.float32)
+        for t in range(valid):
+            acc = (acc + rows[:, t, :]).astype(np.float32)
+        out[u] = _bf16_round_bits(acc / np.float32(max(valid, 1)))
+    return out
+
+
+def sparse_step_mean(q, k_cache, v_cache, page_table, seq_lens, sched: Schedule, sm_scale: float, max_sel: Optional[int] = None) -> dict:
+    """O1..O8 with the mean-key landmark: score s[p] = sum_{h in group} q_h . mean[p] (fp64 over the bf16 landmark);
+    budget, forced pages, top-k (ties to the lower page) and attention exactly as sparse_step."""
+    q, k_cache, v_cache = _u16(q), _u16(k_cache), _u16(v_cache)
+    page_table, seq_lens = _i32(page_table), _i32(seq_lens)
+    n, Hq, D = q.shape
+    _, Hkv, P, _ = k_cache.shape
+    r = Hq // Hkv
+    max_pages = page_table.shape[1]
+    max_sel = max_pages if max_sel is None else max_sel
+    qf = (q.astype(np.uint32) << 16).view(np.float32).astype(np.float64)
+    res = dict(k_pages=np.zeros(n, np.int64), sel_count=np.zeros(n, np.int64), forced=np.zeros((n, max_pages), np.uint8),
+               scores=np.zeros((n, Hkv, max_pages)), tau=np.full((n, Hkv), np.nan), sel=np.zeros((n, Hkv, max_sel), np.int32))
+    for i in range(n):
+        L = int(seq_lens[i]); n_pages = -(-L // P)
+        K = k_pages(sched, L, P)
+        F = forced_pages(L, sched.sink_tokens, sched.local_tokens, P)
+        res["k_pages"][i] = K
+        res["forced"][i, :n_pages] = F
+        nv = np.full(n_pages, P, np.int32)
+        if L % P:
+            nv[-1] = L % P
+        lm = (summarize_mean(k_cache, page_table[i, :n_pages], nv).astype(np.uint32) << 16).view(np.float32).astype(np.float64)
+        for g in range(Hkv):
+            s = lm[:, g, :] @ qf[i, g * r:(g + 1) * r].sum(0)
+            res["scores"][i, g, :n_pages] = s
+            if K >= n_pages:
+                sel = np.arange(n_pages)
+            else:
+                cand = np.flatnonzero(F == 0)
+                k = max(0, K - int(F.sum()))
+                order = sorted(cand.tolist(), key=lambda p: (-s[p], p))[:k]
+                if k > 0:
+                    res["tau"][i, g] = s[order[-1]]
+                sel = np.sort(np.concatenate([np.flatnonzero(F), np.array(order, dtype=np.int64)]))
+            res["sel_count"][i] = len(sel)
+            res["sel"][i, g, :len(sel)] = sel
+    res["out"], res["lse"] = attention_on_sets(q, k_cache, v_cache, page_table, seq_lens, res["sel"], res["sel_count"], sm_scale)
+    return res

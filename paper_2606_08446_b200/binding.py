@@ -29,7 +29,7 @@ class SparrowError(RuntimeError):
 
 class sparrow_shape_t(C.Structure):
     _fields_ = [("n_seq", C.c_int32), ("n_q_heads", C.c_int32), ("n_kv_heads", C.c_int32), ("head_dim", C.c_int32),
-                ("page_size", C.c_int32), ("max_pages_per_seq", C.c_int32), ("n_phys_pages", C.c_int64)]
+                ("page_size", C.c_int32), ("max_pages_per_seq", C.c_int32), ("n_phys_pages", C.c_int64), ("landmark", C.c_int32)]
 
 
 class sparrow_schedule_t(C.Structure):
@@ -49,8 +49,11 @@ class sparrow_cost_t(C.Structure):
                                           "dense_total", "sparse_comp", "sparse_mem", "scoring_comp", "scoring_mem", "sparse_total")]
 
 
-def make_shape(n_seq, n_q_heads, n_kv_heads, max_pages_per_seq, n_phys_pages, head_dim=128, page_size=16):
-    return sparrow_shape_t(n_seq, n_q_heads, n_kv_heads, head_dim, page_size, max_pages_per_seq, n_phys_pages)
+LANDMARK = {"minmax": 0, "mean": 1}
+
+
+def make_shape(n_seq, n_q_heads, n_kv_heads, max_pages_per_seq, n_phys_pages, head_dim=128, page_size=16, landmark="minmax"):
+    return sparrow_shape_t(n_seq, n_q_heads, n_kv_heads, head_dim, page_size, max_pages_per_seq, n_phys_pages, LANDMARK[landmark])
 
 
 def make_schedule(spec: dict, page_size: int = 0) -> sparrow_schedule_t:

@@ -63,6 +63,7 @@ int check_shape(const sparrow_shape_t *s)
     const int r = s->n_q_heads / s->n_kv_heads;
     if (r < 1 || r > kMaxGroup) return SPARROW_ERR_UNSUPPORTED;
     if (s->n_kv_heads > 65535 || s->n_seq > 65535) return SPARROW_ERR_UNSUPPORTED;     // grid.y / grid.z
+    if (s->landmark != SPARROW_LANDMARK_MINMAX && s->landmark != SPARROW_LANDMARK_MEAN) return SPARROW_ERR_INVALID_ARG;
     return SPARROW_OK;
 }
 
@@ -180,8 +181,12 @@ int summarize_impl(const void *k_cache, void *summaries, const int32_t *page_ids
     const int64_t tiles = n_update * s->n_kv_heads;
     const int64_t blocks = (tiles + kSumWarps - 1) / kSumWarps;
     if (blocks > 0x7fffffffLL) return SPARROW_ERR_UNSUPPORTED;
-    launch_chain(summarize_kernel, dim3((unsigned)blocks), dim3(kSumWarps * 32), 0, st, (const uint16_t *)k_cache,
-                 (uint16_t *)summaries, page_ids, n_valid, n_update, s->n_kv_heads, s->page_size);
+    if (s->landmark == SPARROW_LANDMARK_MEAN)
+        launch_chain(summarize_mean_kernel, dim3((unsigned)blocks), dim3(kSumWarps * 32), 0, st, (const uint16_t *)k_cache,
+                     (uint16_t *)summaries, page_ids, n_valid, n_update, s->n_kv_heads, s->page_size);
+    else
+        launch_chain(summarize_kernel, dim3((unsigned)blocks), dim3(kSumWarps * 32), 0, st, (const uint16_t *)k_cache,
+                     (uint16_t *)summaries, page_ids, n_valid, n_update, s->n_kv_heads, s->page_size);
     SPARROW_CHECK_LAUNCH("summarize_kernel");
     return SPARROW_OK;
 }
@@ -208,16 +213,23 @@ int select_impl(const void *q, const void *summaries, const int32_t *page_table,
     pages_per_cta = SPARROW_SEL_PPC_FIXED;
 #endif
     const size_t dyn = (size_t)s->max_pages_per_seq * sizeof(uint32_t);
-    static size_t dyn_set = 0;
-    if (dyn > 48 * 1024 && dyn > dyn_set) {
-        cudaError_t e = cudaFuncSetAttribute(select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
+    const bool mean = s->landmark == SPARROW_LANDMARK_MEAN;
+    static size_t dyn_set[2] = {0, 0};
+    if (dyn > 48 * 1024 && dyn > dyn_set[mean]) {
+        cudaError_t e = mean ? cudaFuncSetAttribute(select_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn)
+                             : cudaFuncSetAttribute(select_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
         if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(select_kernel)");
-        dyn_set = dyn;
+        dyn_set[mean] = dyn;
     }
     dim3 grid((s->max_pages_per_seq + pages_per_cta - 1) / pages_per_cta, s->n_kv_heads, s->n_seq);
-    launch_chain(select_kernel, grid, dim3(kSelThreads), dyn, st, (const uint16_t *)q, (const uint16_t *)summaries, page_table,
-                 seq_lens, sd, sel_pages, max_sel, sel_count, scores_ws, counters, scores_dbg, s->n_q_heads, s->n_kv_heads,
-                 s->max_pages_per_seq, pages_per_cta);
+    if (mean)
+        launch_chain(select_kernel<true>, grid, dim3(kSelThreads), dyn, st, (const uint16_t *)q, (const uint16_t *)summaries,
+                     page_table, seq_lens, sd, sel_pages, max_sel, sel_count, scores_ws, counters, scores_dbg, s->n_q_heads,
+                     s->n_kv_heads, s->max_pages_per_seq, pages_per_cta);
+    else
+        launch_chain(select_kernel<false>, grid, dim3(kSelThreads), dyn, st, (const uint16_t *)q, (const uint16_t *)summaries,
+                     page_table, seq_lens, sd, sel_pages, max_sel, sel_count, scores_ws, counters, scores_dbg, s->n_q_heads,
+                     s->n_kv_heads, s->max_pages_per_seq, pages_per_cta);
     SPARROW_CHECK_LAUNCH("select_kernel");
     return SPARROW_OK;
 }
@@ -257,7 +269,7 @@ int step_impl(const void *q, const void *k_cache, const void *v_cache, const voi
     const bool per_warp = dyn_base + kDecWarps * keys * 4 <= kSmemBudget;
     const size_t dyn = dyn_base + (per_warp ? kDecWarps : 1) * keys * 4;
     static int fused_ok = -1;                    // -1 unknown, 0 the device cannot run the cooperative grid, 1 yes
-    bool fused = fused_ok != 0 && s->page_size == kPage && dyn <= kSmemBudget && s->n_seq <= kDecMaxSeq &&
+    bool fused = fused_ok != 0 && s->page_size == kPage && s->landmark == SPARROW_LANDMARK_MINMAX && dyn <= kSmemBudget && s->n_seq <= kDecMaxSeq &&
                  s->n_phys_pages * s->n_kv_heads < (1LL << 27) &&
                  (int64_t)s->n_seq * s->max_pages_per_seq * s->n_kv_heads < (1LL << 31);
     if (fused && fused_ok < 0) {
@@ -479,7 +491,7 @@ int sparrow_append(const void *k_new, const void *v_new, void *k_cache, void *v_
     const int warps = shape->n_kv_heads < kAppendMaxWarps ? shape->n_kv_heads : kAppendMaxWarps;
     launch_chain(append_kernel, dim3(shape->n_seq), dim3(warps * 32), 0, (cudaStream_t)stream, (const uint16_t *)k_new,
                  (const uint16_t *)v_new, (uint16_t *)k_cache, (uint16_t *)v_cache, (uint16_t *)summaries, page_table, seq_lens,
-                 shape->n_kv_heads, shape->max_pages_per_seq, shape->page_size);
+                 shape->n_kv_heads, shape->max_pages_per_seq, shape->page_size, shape->landmark);
     SPARROW_CHECK_LAUNCH("append_kernel");
     return SPARROW_OK;
 }

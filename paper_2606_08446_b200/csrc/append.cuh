@@ -10,12 +10,12 @@
 
 namespace sparrow {
 
-constexpr int kAppendMaxWarps = 32;
+constexpr int kAppendMaxWarps = 8;                 // warps per CTA; more kv-heads than that are looped over
 
 __global__ void __launch_bounds__(kAppendMaxWarps * 32)
 append_kernel(const uint16_t *__restrict__ k_new, const uint16_t *__restrict__ v_new, uint16_t *__restrict__ k_cache,
               uint16_t *__restrict__ v_cache, uint16_t *__restrict__ summaries, const int32_t *__restrict__ page_table,
-              int32_t *__restrict__ seq_lens, int n_kv_heads, int max_pages, int page_tokens)
+              int32_t *__restrict__ seq_lens, int n_kv_heads, int max_pages, int page_tokens, int landmark)
 {
     chain_entry();
     const int seq = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -34,6 +34,10 @@ append_kernel(const uint16_t *__restrict__ k_new, const uint16_t *__restrict__ v
         *reinterpret_cast<uint4 *>((lane < 16 ? k_cache : v_cache) + tile + row * kDim + c * 8) = val;
         if (row != page_tokens - 1) continue;            // the page is not full yet
         __syncwarp();                                    // the new key row is visible to the whole warp
+        if (landmark == SPARROW_LANDMARK_MEAN) {         // mean-key landmark: same device function as summarize_mean_kernel
+            mean_of_page(k_cache + tile, page_tokens, lane, summaries + (page * n_kv_heads + g) * (int64_t)kDim, true);
+            continue;
+        }
         const int half = lane >> 4;
         uint32_t mn[4] = {0x7f807f80u, 0x7f807f80u, 0x7f807f80u, 0x7f807f80u};
         uint32_t mx[4] = {0xff80ff80u, 0xff80ff80u, 0xff80ff80u, 0xff80ff80u};

@@ -75,6 +75,9 @@ __device__ __forceinline__ float dot8(const float (&qr)[8], const uint4 v, float
     return acc;
 }
 
+// kMean: the landmark is one vector per page, the mean key (256 B), scored as (sum_h q_h) . mean -- the form the paper's
+// cost model charges (D elements per page); otherwise the min/max pair of north_star (512 B).
+template <bool kMean>
 __global__ void __launch_bounds__(kSelThreads, kSelMinBlocks)
 select_kernel(const uint16_t *__restrict__ q, const uint16_t *__restrict__ summaries,
               const int32_t *__restrict__ page_table, const int32_t *__restrict__ seq_lens,
@@ -117,7 +120,7 @@ select_kernel(const uint16_t *__restrict__ q, const uint16_t *__restrict__ summa
     // B(L) and the forced-page rule are exact integer arithmetic: one thread evaluates them for the CTA.
     if (tid == 0) s_plan = make_plan(sched, L);
     if (tid < kDim) {
-        s_q[0][tid] = qm;
+        s_q[0][tid] = kMean ? qp + qm : qm;              // mean landmark: the group's summed query
         s_q[1][tid] = qp;
     }
     __syncthreads();
@@ -137,7 +140,7 @@ select_kernel(const uint16_t *__restrict__ q, const uint16_t *__restrict__ summa
     // ---------------------------------------------------------------- phase A: score this CTA's pages ----
     float qr[8];                                         // lane = 16-byte chunk of the summary: 8 channels of min or max
 #pragma unroll
-    for (int e = 0; e < 8; ++e) qr[e] = (&s_q[0][0])[lane * 8 + e];
+    for (int e = 0; e < 8; ++e) qr[e] = (&s_q[0][0])[(kMean ? (lane & 15) : lane) * 8 + e];
 
     const int cta_pages = min(pages_per_cta, pl.n_pages - cta_page0);
     const int n_wc_cta = (cta_pages + kSelPagesPerWarp - 1) / kSelPagesPerWarp;
@@ -150,7 +153,7 @@ select_kernel(const uint16_t *__restrict__ q, const uint16_t *__restrict__ summa
         const bool my_cand = my_page < pl.n_pages && !pl.forced(my_page);
         const uint32_t cand_mask = __ballot_sync(0xffffffffu, my_cand);  // bit j: page chunk base + j is a candidate
         // offset of this lane's page summary in 16-byte units (< 2^32: up to 64 GiB of summaries)
-        uint32_t my_off16 = ((uint32_t)phys_cur * (uint32_t)n_kv_heads + (uint32_t)g) * 32u;
+        uint32_t my_off16 = ((uint32_t)phys_cur * (uint32_t)n_kv_heads + (uint32_t)g) * (kMean ? 16u : 32u);
         // Pages that are not candidates (forced, or past the end) read the first candidate's summary instead (an L2
         // hit) and their score is never stored: every load of a batch is then unconditional, which keeps the loads
         // independent of one another (a predicated load is compiled as load-to-temporary + copy, which serialises).
@@ -164,6 +167,7 @@ select_kernel(const uint16_t *__restrict__ q, const uint16_t *__restrict__ summa
             phys_nxt = (i + 2 < n_wc && p2 < pl.n_pages) ? __ldg(pt + p2) : 0;
         }
         float my_score = 0.f;                            // score of page chunk base + lane, gathered below
+        if constexpr (!kMean) {
 #pragma unroll 1
         for (int b0 = 0; b0 < kSelPagesPerWarp; b0 += kSelBatch) {
             const uint32_t bm = (cand_mask >> b0) & ((1u << kSelBatch) - 1u);
@@ -203,6 +207,46 @@ select_kernel(const uint16_t *__restrict__ q, const uint16_t *__restrict__ summa
             const int src = ((j >> 2) & 1) * 16 + ((j >> 1) & 1) * 8 + (j & 1) * 4;
             const float got = __shfl_sync(0xffffffffu, z, src & 31);
             if (j >= 0 && j < kSelBatch) my_score = got;
+        }
+        } else {
+            // 256-byte landmarks: one load instruction covers TWO pages (lanes 0-15 | 16-31), a batch of 8 loads 16 pages
+#pragma unroll 1
+            for (int b0 = 0; b0 < kSelPagesPerWarp; b0 += 2 * kSelBatch) {
+                const uint32_t bm = (cand_mask >> b0) & 0xffffu;
+                if (bm == 0) continue;                   // warp-uniform
+                const int half = lane >> 4;
+                uint4 v[kSelBatch];
+#pragma unroll
+                for (int j = 0; j < kSelBatch; ++j) {
+                    const uint32_t off = __shfl_sync(0xffffffffu, my_off16, b0 + 2 * j + half) + (lane & 15);
+                    v[j] = ldg_stream16(sum16 + off);
+                }
+                float a[kSelBatch];
+#pragma unroll
+                for (int j = 0; j < kSelBatch; ++j) a[j] = dot8(qr, v[j], 0.f);
+                // transpose-reduce inside each 16-lane half: lane l ends with value j = 4*bit3 + 2*bit2 + bit1 of l
+                const bool h8 = lane & 8;
+                float k0 = h8 ? a[4] : a[0], k1 = h8 ? a[5] : a[1], k2 = h8 ? a[6] : a[2], k3 = h8 ? a[7] : a[3];
+                float s0 = h8 ? a[0] : a[4], s1 = h8 ? a[1] : a[5], s2 = h8 ? a[2] : a[6], s3 = h8 ? a[3] : a[7];
+                k0 += __shfl_xor_sync(0xffffffffu, s0, 8);
+                k1 += __shfl_xor_sync(0xffffffffu, s1, 8);
+                k2 += __shfl_xor_sync(0xffffffffu, s2, 8);
+                k3 += __shfl_xor_sync(0xffffffffu, s3, 8);
+                const bool h4 = lane & 4;
+                float m0 = h4 ? k2 : k0, m1 = h4 ? k3 : k1;
+                float t0 = h4 ? k0 : k2, t1 = h4 ? k1 : k3;
+                m0 += __shfl_xor_sync(0xffffffffu, t0, 4);
+                m1 += __shfl_xor_sync(0xffffffffu, t1, 4);
+                const bool h2 = lane & 2;
+                float z = h2 ? m1 : m0, y = h2 ? m0 : m1;
+                z += __shfl_xor_sync(0xffffffffu, y, 2);
+                z += __shfl_xor_sync(0xffffffffu, z, 1);
+                // page b0 + 2j + half is owned by lane b0 + 2j + half: fetch its total from lane 16*half + 8*(j>>2) + 4*((j>>1)&1) + 2*(j&1)
+                const int o = lane - b0, jo = o >> 1, ho = o & 1;
+                const int src = ho * 16 + ((jo >> 2) & 1) * 8 + ((jo >> 1) & 1) * 4 + (jo & 1) * 2;
+                const float got = __shfl_sync(0xffffffffu, z, src & 31);
+                if (o >= 0 && o < 2 * kSelBatch) my_score = got;
+            }
         }
         if (my_cand) {                                   // one coalesced 128-byte store per warp
             ws[my_page] = my_score;

@@ -71,4 +71,53 @@ summarize_kernel(const uint16_t *__restrict__ k_cache, uint16_t *__restrict__ su
     *reinterpret_cast<uint4 *>(dst) = o;
 }
 
+// Mean-key landmark (the single vector per page of the paper's cost model): mean[d] = (sum over the
+// page's valid tokens of K[t][d]) / valid, accumulated in fp32 in token order t = 0, 1, ... and rounded to bf16 once
+// (round to nearest even) -- the order is part of the definition, so the result is reproducible bit for bit.
+// One warp per (page, kv-head); lane = 4 channels (8 bytes), so a row is one coalesced 256-byte load.
+__device__ __forceinline__ void mean_of_page(const uint16_t *__restrict__ src, int valid, int lane, uint16_t *__restrict__ dst,
+                                             bool coherent)
+{
+    float acc[4] = {0.f, 0.f, 0.f, 0.f};
+    for (int t0 = 0; t0 < valid; t0 += kPage) {
+        uint2 v[kPage];
+#pragma unroll
+        for (int i = 0; i < kPage; ++i) {                // all loads of the tile first
+            const uint2 *p = reinterpret_cast<const uint2 *>(src + (t0 + i) * kDim + lane * 4);
+            if (t0 + i < valid) v[i] = coherent ? __ldcg(p) : __ldg(p);
+        }
+#pragma unroll
+        for (int i = 0; i < kPage; ++i) {                // then the adds, in token order
+            if (t0 + i < valid) {
+                acc[0] += bf16_lo(v[i].x); acc[1] += bf16_hi(v[i].x);
+                acc[2] += bf16_lo(v[i].y); acc[3] += bf16_hi(v[i].y);
+            }
+        }
+    }
+    const float n = valid > 0 ? (float)valid : 1.f;
+    __nv_bfloat162 lo = __floats2bfloat162_rn(acc[0] / n, acc[1] / n), hi = __floats2bfloat162_rn(acc[2] / n, acc[3] / n);
+    uint2 o;
+    o.x = *reinterpret_cast<uint32_t *>(&lo);
+    o.y = *reinterpret_cast<uint32_t *>(&hi);
+    *reinterpret_cast<uint2 *>(dst + lane * 4) = o;
+}
+
+__global__ void __launch_bounds__(kSumWarps * 32)
+summarize_mean_kernel(const uint16_t *__restrict__ k_cache, uint16_t *__restrict__ summaries,
+                      const int32_t *__restrict__ page_ids, const int32_t *__restrict__ n_valid,
+                      int64_t n_update, int n_kv_heads, int page_tokens)
+{
+    chain_entry();
+    const int lane = threadIdx.x & 31;
+    const int64_t tile = (int64_t)blockIdx.x * kSumWarps + (threadIdx.x >> 5);   // (update, kv-head)
+    if (tile >= n_update * n_kv_heads) return;
+    const int64_t u = tile / n_kv_heads;
+    const int g = (int)(tile % n_kv_heads);
+    const int64_t page = page_ids ? (int64_t)page_ids[u] : u;
+    int valid = n_valid ? n_valid[u] : page_tokens;
+    valid = valid < 0 ? 0 : (valid > page_tokens ? page_tokens : valid);
+    mean_of_page(k_cache + (page * n_kv_heads + g) * (int64_t)page_tokens * kDim, valid, lane,
+                 summaries + (page * n_kv_heads + g) * (int64_t)kDim, false);
+}
+
 }  // namespace sparrow

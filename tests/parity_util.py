@@ -37,6 +37,12 @@ def sub_host(h: dict, idx) -> dict:
 
 
 def check_summaries(summ_gpu: torch.Tensor, h: dict, page_ids, n_valid):
+    if summ_gpu.dim() == 3:         # mean-key landmark [n_phys][Hkv][128]: a stored bf16 code, compared bit for bit
+        want = oracle.summarize_mean(h["k_cache"], np.asarray(page_ids, np.int32), None if n_valid is None else np.asarray(n_valid, np.int32))
+        got = summ_gpu[torch.as_tensor(np.asarray(page_ids)).long().to(summ_gpu.device)].contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
+        bad = got != want
+        assert not bad.any(), f"mean landmarks differ at {int(bad.sum())} of {bad.size} entries"
+        return
     want = oracle.summarize(h["k_cache"], np.asarray(page_ids, np.int32), None if n_valid is None else np.asarray(n_valid, np.int32))
     got = bf16_to_f64(summ_gpu[torch.as_tensor(np.asarray(page_ids)).long().to(summ_gpu.device)])
     assert got.shape == want.shape
@@ -103,8 +109,8 @@ def check_sparse_step(eng, wl, h=None, idx=None, check_summ=True) -> dict:
     idx = np.arange(n) if idx is None else np.asarray(idx)
     hs = sub_host(h, idx)
     sched = oracle.Schedule.from_spec(eng.sched_spec)
-    res = oracle.sparse_step(hs["q"], hs["k_cache"], hs["v_cache"], hs["page_table"], hs["seq_lens"], sched, wl.sm_scale,
-                             max_sel=eng.max_sel)
+    step_fn = oracle.sparse_step_mean if getattr(eng, "landmark", "minmax") == "mean" else oracle.sparse_step
+    res = step_fn(hs["q"], hs["k_cache"], hs["v_cache"], hs["page_table"], hs["seq_lens"], sched, wl.sm_scale, max_sel=eng.max_sel)
     tidx = torch.as_tensor(idx).long().to(eng.out.device)
     sel_gpu = eng.sel_pages[tidx].cpu().numpy()
     cnt_gpu = eng.sel_count[tidx].cpu().numpy()

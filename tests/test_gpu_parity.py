@@ -270,3 +270,41 @@ def test_rollout_with_page_size_64():
     if stats["differing_units"] == 0:
         for t in (0, T // 2, T - 1):
             check_outputs(out[t], lse[t], want[t]["out"], want[t]["lse"], f"page-64 rollout step {t}")
+
+
+# ------------------------------------------------------------------ 8(f)-2: the mean-key landmark ----
+@pytest.mark.parametrize("Hq,Hkv,page", [(8, 2, 16), (5, 1, 16), (16, 8, 16), (8, 2, 64)])
+def test_mean_landmark_matches_oracle(Hq, Hkv, page):
+    """One vector per page (the paper's cost model): landmarks bit for bit (fp32 sum in token order ->
+    bf16), scores, selection (band rule) and attention against oracle.sparse_step_mean; ragged lengths, partial pages."""
+    lens = [1, 15, 16, 17, 33, 250, 256, 257, 1000, 2049, 4099, 9000]
+    sched = W._sched("fixed", 16, 64, fixed_tokens=320)
+    wl = W.make_workload(n_seq=len(lens), Hq=Hq, Hkv=Hkv, lengths=("list", lens), schedule=sched, seed=Hq * 10 + page, device=DEV,
+                         poison_tail=True, plant=True, page_size=page)
+    eng = _run_sparse(wl, want_scores=True, landmark="mean")       # sparrow_step takes the two launches for this landmark
+    assert eng.summaries.shape == (wl.n_phys, Hkv, 128)
+    check_sparse_step(eng, wl)
+
+
+def test_mean_landmark_rollout_summarizes_on_fill():
+    from paper_2606_08446_b200.engine import SparrowEngine
+    T, lens = 40, [100, 1000, 4090]
+    sched = W._sched("clamp_frac", 32, 96, f0_ppm=125000, floor_tokens=256)
+    wl = W.make_workload(n_seq=3, Hq=8, Hkv=2, lengths=("list", lens), schedule=sched, seed=8, device=DEV, plant=True, reserve_tokens=T + 1)
+    eng = SparrowEngine(wl, want_scores=True, landmark="mean")
+    eng.summarize_all(); eng.reserve(T)
+    qs, ks, vs = W.make_rollout_inputs(wl, T, seed=2)
+    out = torch.zeros((T, 3, 8, 128), dtype=torch.bfloat16, device=DEV)
+    eng.rollout(qs, ks, vs, out)
+    torch.cuda.synchronize()
+    # after the rollout the engine state is a plain step on the grown cache: landmarks (incl. pages filled on the way),
+    # selection and the last step's attention all checked against the oracle on the final cache
+    wl.q = qs[T - 1].contiguous()
+    eng.out.copy_(out[T - 1])
+    eng.sparse_decode(wl.q)                                          # refresh lse for the checker
+    torch.cuda.synchronize()
+    assert wl.seq_lens.cpu().tolist() == [L + T for L in lens]
+    h = wl.host()
+    ids = np.concatenate([h["page_table"][i, :(L + T) // 16] for i, L in enumerate(lens)])      # every FULL page
+    check_summaries(eng.summaries, h, ids, None)
+    check_sparse_step(eng, wl, h=h, check_summ=False)

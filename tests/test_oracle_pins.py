@@ -556,3 +556,68 @@ def test_binned_quantile_is_the_nearest_rank_quantile():
     assert counts[5] == 0 and counts[4] == (pos >= 8192).sum()
     c, v = oracle.binned_quantile([0.5, 0.1, 0.9, 0.3], [0, 2047, 2048, 5000], 2048, 2, 0.5)
     assert c.tolist() == [2, 2] and v.tolist() == [0.1, 0.3]                                  # rank ceil(0.5 * 2) = 1
+
+
+# ------------------------------------------------------------------ 8(f)-2: the mean-key landmark ----
+def test_mean_landmark_against_torch_and_exact_mean():
+    """summarize_mean = fp32 running sum in token order / count -> bf16 (nearest even).  Pinned with torch's own fp32
+    cumsum and bf16 rounding (a library routine, not a retyping), against the exact mean (never more than one bf16
+    step away), and on the special cases: one valid token -> that key; identical keys -> that key."""
+    wl = W.make_workload(n_seq=2, Hq=4, Hkv=2, lengths=("list", [100, 37]), schedule=W._sched("dense", 0, 0), seed=77, device="cpu")
+    h = wl.host()
+    ids = np.array([0, 3, 5, 2], np.int32)
+    nv = np.array([16, 1, 9, 16], np.int32)
+    got = oracle.summarize_mean(h["k_cache"], ids, nv)
+    for u, (pg, v) in enumerate(zip(ids, nv)):
+        rows = wl.k_cache[int(pg)].float()[:, :v, :]                                     # [Hkv][v][D] fp32 (exact)
+        want = (rows.cumsum(1)[:, -1, :] / float(v)).to(torch.bfloat16)
+        assert np.array_equal(got[u], want.view(torch.int16).numpy().view(np.uint16))
+        exact = f64(h["k_cache"][pg])[:, :v, :].mean(1)
+        step = np.maximum(np.abs(exact), 2.0 ** -126) * 2.0 ** -7                        # one bf16 step at that magnitude
+        assert (np.abs(f64(got[u]) - exact) <= step).all()
+    assert np.array_equal(got[1], h["k_cache"][3][:, 0, :])                              # one valid token
+    kc = h["k_cache"].copy(); kc[7, :, :, :] = kc[7, :, :1, :]
+    assert np.array_equal(oracle.summarize_mean(kc, np.array([7], np.int32))[0], kc[7][:, 0, :])
+
+
+def test_mean_landmark_step_against_numpy_token_level():
+    """The whole step with the mean-key landmark (PAPER.md:142's one vector per page) against a restatement written
+    here: torch fp32 mean per page, score = (sum of the group's queries) . mean, top-k by (score desc, page asc) among the
+    non-forced pages, softmax over the kept pages' valid tokens; plus planted pages recovered and B >= L == dense."""
+    lens = [700, 129, 2050]
+    S, Wn, budget = 40, 200, 256
+    sched = W._sched("fixed", S, Wn, fixed_tokens=budget)
+    wl = W.make_workload(n_seq=3, Hq=4, Hkv=2, lengths=("list", lens), schedule=sched, seed=91, device="cpu", plant=True, plant_scale=6.0)
+    h = wl.host()
+    res = oracle.sparse_step_mean(h["q"], h["k_cache"], h["v_cache"], h["page_table"], h["seq_lens"], oracle.Schedule.from_spec(sched), wl.sm_scale)
+    Kf, Vf, Qf = f64(h["k_cache"]), f64(h["v_cache"]), f64(h["q"])
+    r = wl.Hq // wl.Hkv
+    for i, L in enumerate(lens):
+        n_pages = -(-L // P)
+        forced = set(range(min(3, n_pages))) | set(range(max(L - Wn, 0) // P, n_pages))  # 40 sink tokens = 3 pages
+        dense_seq = budget // P >= n_pages
+        assert res["sel_count"][i] == (n_pages if dense_seq else max(budget // P, len(forced)))
+        for g in range(wl.Hkv):
+            qsum = Qf[i, g * r:(g + 1) * r].sum(0)
+            score = np.zeros(n_pages)
+            for p in range(n_pages):
+                v = min(P, L - p * P)
+                m = (wl.k_cache[int(h["page_table"][i, p]), g, :v].float().cumsum(0)[-1] / float(v)).to(torch.bfloat16).double().numpy()
+                score[p] = m @ qsum
+            cand = [p for p in range(n_pages) if p not in forced]
+            keep = list(range(n_pages)) if dense_seq else sorted(forced | set(sorted(cand, key=lambda p: (-score[p], p))[:max(0, budget // P - len(forced))]))
+            assert res["sel"][i, g, :len(keep)].tolist() == keep
+            planted = [p for p in wl.planted[i][g].tolist() if p not in forced]
+            if not dense_seq:
+                assert len(set(planted) & set(keep)) >= min(len(planted), max(0, budget // P - len(forced))) - 1
+            tok = np.concatenate([np.arange(p * P, min((p + 1) * P, L)) for p in keep])
+            keys = np.stack([Kf[h["page_table"][i, t // P], g, t % P] for t in tok])
+            vals = np.stack([Vf[h["page_table"][i, t // P], g, t % P] for t in tok])
+            for hh in range(r):
+                z = keys @ Qf[i, g * r + hh] * wl.sm_scale
+                pr = np.exp(z - z.max()); pr /= pr.sum()
+                assert np.allclose(pr @ vals, res["out"][i, g * r + hh], rtol=0, atol=1e-12)
+    big = oracle.sparse_step_mean(h["q"], h["k_cache"], h["v_cache"], h["page_table"], h["seq_lens"],
+                                  oracle.Schedule.from_spec(W._sched("fixed", S, Wn, fixed_tokens=4096)), wl.sm_scale)
+    dense_out, dense_lse = oracle.dense_step(h["q"], h["k_cache"], h["v_cache"], h["page_table"], h["seq_lens"], wl.sm_scale)
+    assert np.allclose(big["out"], dense_out, rtol=0, atol=1e-12) and np.allclose(big["lse"], dense_lse, rtol=0, atol=1e-12)
