@@ -101,7 +101,7 @@ def algorithmic_bytes(wl, eng, lens, cnt):
     cand = np.where(dense_seq, 0, n_pages - forced)
     qo = wl.n_seq * wl.Hq * 128 * 2
     decode = int(cnt.sum()) * wl.Hkv * KV_TILE_BYTES + int(cnt.sum()) * wl.Hkv * 4 + int(cnt.sum()) * 4 + 2 * qo
-    select = int(cand.sum()) * wl.Hkv * SUMMARY_BYTES + int(cand.sum()) * 4 + int(cnt.sum()) * wl.Hkv * 4 + qo
+    select = int(cand.sum()) * wl.Hkv * (SUMMARY_BYTES if getattr(eng, "landmark", "minmax") == "minmax" else SUMMARY_BYTES // 2) + int(cand.sum()) * 4 + int(cnt.sum()) * wl.Hkv * 4 + qo
     dense = int(n_pages.sum()) * wl.Hkv * KV_TILE_BYTES + int(n_pages.sum()) * 4 + 2 * qo
     return dict(decode=decode, select=select, dense=dense, sel_tiles=int(cnt.sum()) * wl.Hkv, cand_tiles=int(cand.sum()) * wl.Hkv)
 
@@ -397,10 +397,14 @@ def main():
                     help="select + sparse decode as two launches (default, measured faster) or as the one cooperative sparrow_step launch")
     ap.add_argument("--table4", action="store_true", help="page-size sweep at budget 1024 (PAPER.md Table 4) instead of the step benchmark")
     ap.add_argument("--acceptance", action="store_true", help="time sparrow_acceptance (SURVEY 8(f)-3) instead of the step benchmark")
+    ap.add_argument("--landmark", default="minmax", choices=["minmax", "mean"],
+                    help="page landmark: per-channel min/max (north_star's default, 512 B) or the mean key (the paper's cost model, 256 B)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-check", action="store_true", help="skip the sampled oracle self-check before timing")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
+    if args.landmark == "mean":
+        args.no_cpu_baseline = True      # the timed CPU baseline is the default (min/max) path's oracle
 
     rank, local_rank, world = D.env_world()
     if args.impl == "reference":
@@ -424,7 +428,7 @@ def main():
 
     base_seed = 1000 * int("".join(ch for ch in args.workload if ch.isdigit()) or 0)
     wl = W.make_config(args.workload, seed=D.replica_seed(base_seed, rank), device=dev)
-    eng = SparrowEngine(wl)
+    eng = SparrowEngine(wl, landmark=args.landmark)
     st = torch.cuda.Stream(device=dev)
     upd = tuple(t.to(dev) for t in W.just_filled_updates(wl))
     with torch.cuda.stream(st):
@@ -579,7 +583,7 @@ def main():
         "ms_per_step": t_max * 1e3 / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "bf16", "data": "synthetic",
         "config": {"workload": args.workload, "n_seq": wl.n_seq, "Hq": wl.Hq, "Hkv": wl.Hkv, "head_dim": 128, "page_size": 16,
-                   "len_min": int(lens.min()), "len_max": int(lens.max()), "schedule": wl.schedule["kind"], "step_form": args.step_form,
+                   "len_min": int(lens.min()), "len_max": int(lens.max()), "schedule": wl.schedule["kind"], "step_form": args.step_form, "landmark": args.landmark,
                    "sink_tokens": wl.schedule["sink_tokens"], "local_tokens": wl.schedule["local_tokens"],
                    "selected_pages_per_seq_mean": float(cnt.mean()), "parallelism": f"replicas x{world} (no collective)",
                    "l2": "inputs larger than L2: %.0f MB touched per step vs 126 MB L2" % ((ab["decode"] + ab["select"]) / 1e6),
