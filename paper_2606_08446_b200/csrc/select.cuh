@@ -168,46 +168,52 @@ select_kernel(const uint16_t *__restrict__ q, const uint16_t *__restrict__ summa
         }
         float my_score = 0.f;                            // score of page chunk base + lane, gathered below
         if constexpr (!kMean) {
+            auto load_batch = [&](uint4 (&v)[kSelBatch], int b0) {   // the 8 summaries of pages b0 .. b0 + 7: 8 x 512 B
+#pragma unroll
+                for (int j = 0; j < kSelBatch; ++j) {
+                    const uint32_t off = __shfl_sync(0xffffffffu, my_off16, b0 + j) + lane;
+                    v[j] = ldg_stream16(sum16 + off);
+                }
+            };
+            auto reduce_batch = [&](const uint4 (&v)[kSelBatch], int b0) {
+                float a[kSelBatch];
+#pragma unroll
+                for (int j = 0; j < kSelBatch; ++j) a[j] = dot8(qr, v[j], 0.f);
+                // transpose-reduce: after the three halving steps lane l holds page j = 4*b4 + 2*b3 + b2 (bits of l),
+                // summed over the lanes that differ from l in bits 4, 3, 2; two more butterflies finish the sum.
+                static_assert(kSelBatch == 8, "transpose-reduce is written for 8 pages per batch");
+                const bool hi = lane & 16;
+                float k0 = hi ? a[4] : a[0], k1 = hi ? a[5] : a[1], k2 = hi ? a[6] : a[2], k3 = hi ? a[7] : a[3];
+                float s0 = hi ? a[0] : a[4], s1 = hi ? a[1] : a[5], s2 = hi ? a[2] : a[6], s3 = hi ? a[3] : a[7];
+                k0 += __shfl_xor_sync(0xffffffffu, s0, 16);
+                k1 += __shfl_xor_sync(0xffffffffu, s1, 16);
+                k2 += __shfl_xor_sync(0xffffffffu, s2, 16);
+                k3 += __shfl_xor_sync(0xffffffffu, s3, 16);
+                const bool h8 = lane & 8;
+                float m0 = h8 ? k2 : k0, m1 = h8 ? k3 : k1;
+                float t0 = h8 ? k0 : k2, t1 = h8 ? k1 : k3;
+                m0 += __shfl_xor_sync(0xffffffffu, t0, 8);
+                m1 += __shfl_xor_sync(0xffffffffu, t1, 8);
+                const bool h4 = lane & 4;
+                float z = h4 ? m1 : m0, y = h4 ? m0 : m1;
+                z += __shfl_xor_sync(0xffffffffu, y, 4);
+                z += __shfl_xor_sync(0xffffffffu, z, 2);
+                z += __shfl_xor_sync(0xffffffffu, z, 1);
+                // lane l now holds the score of batch page j(l) = ((l>>4)&1)*4 + ((l>>3)&1)*2 + ((l>>2)&1); hand it to
+                // the lane that owns that page's table entry (lane b0 + j): source lane for j is 16*(j>>2) + 8*((j>>1)&1) + 4*(j&1).
+                const int j = lane - b0;
+                const int src = ((j >> 2) & 1) * 16 + ((j >> 1) & 1) * 8 + (j & 1) * 4;
+                const float got = __shfl_sync(0xffffffffu, z, src & 31);
+                if (j >= 0 && j < kSelBatch) my_score = got;
+            };
 #pragma unroll 1
-        for (int b0 = 0; b0 < kSelPagesPerWarp; b0 += kSelBatch) {
-            const uint32_t bm = (cand_mask >> b0) & ((1u << kSelBatch) - 1u);
-            if (bm == 0) continue;                       // warp-uniform
-            uint4 v[kSelBatch];
-#pragma unroll
-            for (int j = 0; j < kSelBatch; ++j) {        // all loads of the batch first
-                const uint32_t off = __shfl_sync(0xffffffffu, my_off16, b0 + j) + lane;
-                v[j] = ldg_stream16(sum16 + off);
+            for (int b0 = 0; b0 < kSelPagesPerWarp; b0 += kSelBatch) {
+                const uint32_t bm = (cand_mask >> b0) & ((1u << kSelBatch) - 1u);
+                if (bm == 0) continue;                   // warp-uniform
+                uint4 v[kSelBatch];
+                load_batch(v, b0);
+                reduce_batch(v, b0);
             }
-            float a[kSelBatch];
-#pragma unroll
-            for (int j = 0; j < kSelBatch; ++j) a[j] = dot8(qr, v[j], 0.f);
-            // transpose-reduce: after the three halving steps lane l holds page j = 4*b4 + 2*b3 + b2 (bits of l),
-            // summed over the lanes that differ from l in bits 4, 3, 2; two more butterflies finish the sum.
-            static_assert(kSelBatch == 8, "transpose-reduce is written for 8 pages per batch");
-            const bool hi = lane & 16;
-            float k0 = hi ? a[4] : a[0], k1 = hi ? a[5] : a[1], k2 = hi ? a[6] : a[2], k3 = hi ? a[7] : a[3];
-            float s0 = hi ? a[0] : a[4], s1 = hi ? a[1] : a[5], s2 = hi ? a[2] : a[6], s3 = hi ? a[3] : a[7];
-            k0 += __shfl_xor_sync(0xffffffffu, s0, 16);
-            k1 += __shfl_xor_sync(0xffffffffu, s1, 16);
-            k2 += __shfl_xor_sync(0xffffffffu, s2, 16);
-            k3 += __shfl_xor_sync(0xffffffffu, s3, 16);
-            const bool h8 = lane & 8;
-            float m0 = h8 ? k2 : k0, m1 = h8 ? k3 : k1;
-            float t0 = h8 ? k0 : k2, t1 = h8 ? k1 : k3;
-            m0 += __shfl_xor_sync(0xffffffffu, t0, 8);
-            m1 += __shfl_xor_sync(0xffffffffu, t1, 8);
-            const bool h4 = lane & 4;
-            float z = h4 ? m1 : m0, y = h4 ? m0 : m1;
-            z += __shfl_xor_sync(0xffffffffu, y, 4);
-            z += __shfl_xor_sync(0xffffffffu, z, 2);
-            z += __shfl_xor_sync(0xffffffffu, z, 1);
-            // lane l now holds the score of batch page j(l) = ((l>>4)&1)*4 + ((l>>3)&1)*2 + ((l>>2)&1); hand it to
-            // the lane that owns that page's table entry (lane b0 + j): source lane for j is 16*(j>>2) + 8*((j>>1)&1) + 4*(j&1).
-            const int j = lane - b0;
-            const int src = ((j >> 2) & 1) * 16 + ((j >> 1) & 1) * 8 + (j & 1) * 4;
-            const float got = __shfl_sync(0xffffffffu, z, src & 31);
-            if (j >= 0 && j < kSelBatch) my_score = got;
-        }
         } else {
             // 256-byte landmarks: one load instruction covers TWO pages (lanes 0-15 | 16-31), a batch of 8 loads 16 pages
 #pragma unroll 1
