@@ -438,14 +438,16 @@ __device__ __forceinline__ void decode_warp_stream(const DecodeArgs &A, const in
                     if ((lane & 3) == 0) *reinterpret_cast<float2 *>(ws_ml + (slot * r + hrow) * 2) = make_float2(m_run, l_tot);
                 }
             }
-            __threadfence();
+            // release / acquire through ONE atomic of lane 0 (no fence per lane): the warp barrier orders the lanes'
+            // partial stores before lane 0's acq_rel atomic (cumulative at gpu scope), and the shuffle that hands its
+            // result round orders that acquire before the other lanes' reads of the slots (ld.global.cg below)
             __syncwarp();
             int old = 0;
-            if (lane == 0) old = atomicAdd(counters + unit, 1);
+            if (lane == 0)
+                asm volatile("atom.acq_rel.gpu.global.add.s32 %0, [%1], 1;" : "=r"(old) : "l"(counters + unit) : "memory");
             old = __shfl_sync(kFull, old, 0);
             if (old != w1 - w0) continue;                            // not the last segment to arrive
             if (lane == 0) counters[unit] = 0;                       // restore the zero for the next call
-            __threadfence();
             const int nseg = w1 - w0 + 1;
             const int64_t row0 = ((int64_t)unit + w0) * r;           // slot row of segment s, head h: row0 + s * r + h
             // Every dependent round trip costs 1-2 us while the K/V stream saturates HBM, so the merge is written for

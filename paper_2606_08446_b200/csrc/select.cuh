@@ -261,18 +261,20 @@ select_kernel(const uint16_t *__restrict__ q, const uint16_t *__restrict__ summa
     }
 
     // ------------------------------------------------ last CTA of this (sequence, kv-head)? --------
-    __threadfence();
+    // Release / acquire through ONE atomic of thread 0 instead of a fence by every thread: the CTA barrier orders the
+    // warps' score stores before thread 0's acq_rel atomic (cumulative at gpu scope), and in the last CTA the barrier
+    // after it orders that acquire before the other threads' reads of the scores (ld.global.cg below).
     __syncthreads();
     if (tid == 0) {
         int32_t *ctr = counters + seq * n_kv_heads + g;
-        const int old = atomicAdd(ctr, 1);
+        int old;
+        asm volatile("atom.acq_rel.gpu.global.add.s32 %0, [%1], 1;" : "=r"(old) : "l"(ctr) : "memory");
         const int last = (old == n_chunks - 1);
         if (last) *ctr = 0;                              // restore the zero for the next call
         s_bcast[0][0] = last;
     }
     __syncthreads();
     if (!s_bcast[0][0]) return;
-    __threadfence();
 
     // ---------------------------------------------------------------- phase B: top-k of the unit ----
     const int n_pages = pl.n_pages;
