@@ -88,6 +88,7 @@ int to_dev_sched(const sparrow_schedule_t *in, SchedDev *out, int page_tokens = 
         return SPARROW_ERR_INVALID_ARG;
     if (page_tokens != 0 && in->page_size != 0 && in->page_size != page_tokens) return SPARROW_ERR_INVALID_ARG;
     out->page = page_tokens != 0 ? page_tokens : (in->page_size != 0 ? in->page_size : kPage);
+    out->page_log2 = out->page == 16 ? 4 : (out->page == 32 ? 5 : (out->page == 64 ? 6 : 7));
     out->inv_den = 1.0;
     if (in->kind == SPARROW_SCHED_FIXED && in->fixed_tokens < 0) return SPARROW_ERR_INVALID_ARG;
     constexpr int64_t kPpmMax = 1000000;                 // keep fractions are in [0, 1]

@@ -21,6 +21,7 @@ constexpr int kSumElems = 2 * kDim;             // one (page, kv-head) summary: 
 struct SchedDev {
     int32_t kind, sink_tokens, local_tokens, table_len, bin_tokens;
     int32_t page;                // tokens per page: 16, 32, 64 or 128
+    int32_t page_log2;           // its log2: every division by the page size in the plan is a shift
     int64_t fixed_tokens, floor_tokens, f0_ppm, f1_ppm, L0, L1;
     double inv_den;              // LINEAR_FRAC: 1.0 / (1e6 * (L1 - L0)), the quotient estimate's multiplier
     int32_t table[SPARROW_MAX_TABLE_BINS];
@@ -99,16 +100,18 @@ __host__ __device__ inline SeqPlan make_plan(const SchedDev &s, int64_t L)
 {
     SeqPlan pl;
     pl.L = (int32_t)L;
-    pl.n_pages = (int32_t)ceil_div64(L, s.page);
-    int64_t kp = ceil_div64(budget_tokens(s, L), s.page);                // R4: ceil
+    const int sh = s.page_log2;
+    const int64_t pm = s.page - 1;
+    pl.n_pages = (int32_t)((L + pm) >> sh);
+    int64_t kp = (budget_tokens(s, L) + pm) >> sh;                       // R4: ceil
     pl.k_pages = (int32_t)(kp < pl.n_pages ? kp : pl.n_pages);
-    int32_t ns = (int32_t)ceil_div64(s.sink_tokens, s.page);             // R8
+    int32_t ns = (int32_t)((s.sink_tokens + pm) >> sh);                  // R8
     pl.n_sink = ns < pl.n_pages ? ns : pl.n_pages;
     int32_t t0 = pl.n_pages - 1;                                         // last page always kept (R9)
     if (s.local_tokens > 0) {
         int64_t lo = L - s.local_tokens;
         if (lo < 0) lo = 0;
-        int32_t fl = (int32_t)(lo / s.page);                             // R7: every page overlapping the window
+        int32_t fl = (int32_t)(lo >> sh);                                // R7: every page overlapping the window
         if (fl < t0) t0 = fl;
     }
     if (t0 < 0) t0 = 0;
