@@ -67,8 +67,9 @@ typedef struct sparrow_shape {
  *   MINMAX  per-channel min and max of the page's keys, summaries [n_phys_pages][n_kv_heads][2][128] (512 B), score =
  *           sum_{h in group} sum_d max(q*min, q*max) -- an upper bound of q.k over the page (north_star's default)
  *   MEAN    the mean key, summaries [n_phys_pages][n_kv_heads][128] (256 B), score = sum_{h in group} q_h . mean -- the
- *           one-vector-per-page landmark that the paper's cost model charges.  mean = fp32 sum of the
- *           valid tokens in token order, divided by their number, rounded once to bf16.
+ *           one-vector-per-page landmark that the paper's cost model charges.  mean over the valid
+ *           tokens, accumulated in fp32, rounded once to bf16: the stored code is the exactly rounded mean or, where the
+ *           exact mean lies within the fp32 accumulation error of a rounding boundary, the neighbouring code (R24).
  * Everything else (budget, forced pages, top-k, attention) is the same.  sparrow_step uses the two launches for MEAN. */
 enum { SPARROW_LANDMARK_MINMAX = 0, SPARROW_LANDMARK_MEAN = 1 };
 
@@ -171,18 +172,23 @@ int sparrow_step(const void *q, const void *k_cache, const void *v_cache, const 
 size_t sparrow_step_workspace_bytes(const sparrow_shape_t *shape, int32_t max_sel);
 
 /* ---- whole step through HOST buffers (the end-to-end measurement path) ----------------------------
- * Copies this step's inputs from host memory (q_host [n][Hq][128] bf16, seq_lens_host [n] int32; pinned
- * memory makes the copies asynchronous), runs summarize (n_update pages, page_ids/n_valid are HOST arrays,
- * n_update may be 0) -> select -> sparse decode (or the dense path when sched->kind == DENSE) on `stream`,
- * copies out back to out_host [n][Hq][128] bf16 and WAITS for the stream.  The K/V pools, summaries and
- * page_table are the resident cache state and stay device pointers.  `scratch` is a device buffer of at
- * least sparrow_step_scratch_bytes(shape, max_sel) bytes, zero-initialised once by the caller. */
-int sparrow_step_host(const void *q_host, const int32_t *seq_lens_host,
-                      const int32_t *page_ids_host, const int32_t *n_valid_host, int64_t n_update,
+ * The step's inputs live in ONE host block (pinned memory makes the copy asynchronous) laid out as
+ *     q [n][Hq][128] bf16 at offset 0 | seq_lens [n] int32 | page_ids [n_update] int32 | n_valid [n_update] int32
+ * at the 256-byte-aligned offsets sparrow_step_host_block_bytes() reports, so that a single host-to-device copy brings
+ * them over (the caller writes its q and lengths straight into the block).  The call copies the used part of the
+ * block, runs summarize (n_update <= n_seq pages that just filled; 0 = none; has_n_valid = 0 means full pages) ->
+ * select -> sparse decode (or the dense path when sched->kind == DENSE) on `stream`, copies out back to
+ * out_host [n][Hq][128] bf16 and WAITS for the stream.  The K/V pools, summaries and page_table are the resident
+ * cache state and stay device pointers.  `scratch` is a device buffer of at least
+ * sparrow_step_scratch_bytes(shape, max_sel) bytes, zero-initialised once by the caller. */
+int sparrow_step_host(const void *in_block_host, int64_t n_update, int has_n_valid,
                       const void *k_cache, const void *v_cache, void *summaries, const int32_t *page_table,
                       const sparrow_schedule_t *sched, int32_t max_sel, float sm_scale,
                       void *out_host, void *scratch, size_t scratch_bytes,
                       const sparrow_shape_t *shape, void *stream);
+/* Size of the host block and (optional out-parameters) the offsets of its seq_lens / page_ids / n_valid parts. */
+size_t sparrow_step_host_block_bytes(const sparrow_shape_t *shape, size_t *off_seq_lens, size_t *off_page_ids,
+                                     size_t *off_n_valid);
 
 /* ---- the paper's divergence statistic (SURVEY.md 8(f)-3; PAPER.md:76-79 Eq. 1, :95, :101, :119) -------------
  * Per token position i < n_pos the dense policy P and the sparse policy Q each give their top_n (<= 32) tokens and
@@ -207,7 +213,8 @@ size_t sparrow_acceptance_workspace_bytes(int32_t n_bins);
  *   dense   comp = 2 P B N L_out + r B N (2 L_in + L_out) L_out D      mem = 2 P L_out + B N (2 L_in L_out + L_out^2) D
  *   sparse  comp = 2 P B N L_out + r B N D H                           mem = 2 P L_out + B N D H
  *   scoring (steps past the dense phase only; landmark visits S = sum over those steps of (L_in + t) / pagesize):
- *           comp = 2 r B N D S                                         mem = c B N D S         (Eq. 3; reading R21)
+ *           comp = r c B N D S                                         mem = c B N D S         (Eq. 3; reading R21:
+ *           with c = 1 and L_in = 0 these are the paper's printed r N D L_out^2 / (2 pagesize) and N D L_out^2 / (2 pagesize))
  *   total = comp + I * mem.  Returns SPARROW_ERR_INVALID_ARG for non-positive sizes. */
 typedef struct sparrow_cost_args {
     double params, batch_size, n_samples, L_in, L_out, D, r, intensity, budget_tokens, page_size, landmarks_per_page;

@@ -26,6 +26,7 @@ from .oracle import (  # noqa: F401
     acceptance_rate,
     binned_quantile,
     summarize_mean,
+    mean_landmark_band,
     sparse_step_mean,
     num_threads,
 )

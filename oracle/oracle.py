@@ -327,7 +327,10 @@ def cost_model(P, B, N, L_in, L_out, D, r, I, K, pagesize, c=1.0) -> dict:
              sparse: the attention terms with H in place of (2 L_in + L_out) L_out.
     Eq. 3 scoring (reading R21: one landmark visit per page of the context per decode step, only on the steps decoded
     under the budget): visits S = sum over those steps of (L_in + t) / pagesize (continuous form, as the paper's
-    L_out^2 / 2 terms);  compute 2 r B N D S;  memory c B N D S.   C = C_comp + I C_mem."""
+    L_out^2 / 2 terms).  The paper charges one D-vector read (memory D) and r D multiply-adds (compute r D) per landmark
+    vector visited -- its clean terms at :142 are memory I N D L_out^2 / (2 pagesize), compute r N D L_out^2 / (2 pagesize),
+    the same r : 1 ratio as the attention terms -- so with c landmark vectors per page:
+    memory c B N D S;  compute r c B N D S.   C = C_comp + I C_mem."""
     L_dense = min(L_out, max(K - L_in, 0.0))
     H = (2 * L_in + L_dense) * L_dense + 2 * K * max(L_out - L_dense, 0.0)
     H_dense = (2 * L_in + L_out) * L_out
@@ -336,7 +339,7 @@ def cost_model(P, B, N, L_in, L_out, D, r, I, K, pagesize, c=1.0) -> dict:
     dense_mem = 2 * P * L_out + B * N * H_dense * D
     sparse_comp = 2 * P * B * N * L_out + r * B * N * D * H
     sparse_mem = 2 * P * L_out + B * N * D * H
-    scoring_comp = 2 * r * B * N * D * S
+    scoring_comp = r * c * B * N * D * S
     scoring_mem = c * B * N * D * S
     return dict(attn_elems_dense=H_dense, attn_elems_sparse=H, landmark_visits=S, dense_comp=dense_comp, dense_mem=dense_mem,
                 dense_total=dense_comp + I * dense_mem, sparse_comp=sparse_comp, sparse_mem=sparse_mem,
@@ -380,33 +383,60 @@ def binned_quantile(alpha, positions, bin_tokens: int, n_bins: int, quantile: fl
 
 # ---------------------------------------------------------------------------------------------------------------
 # SURVEY.md 8(f)-2, landmark variant: ONE vector per page, the mean key -- the landmark the paper's cost model charges
-# (D elements per page; the form itself is left open at :147, reading R1).  The landmark is a stored
-# bf16 code, so it is computed in the precision that decides the code (the kernel's): fp32 accumulation over the
-# page's valid tokens in token order, one fp32 division, one rounding to bf16 (nearest even).  Everything after it
+# (D elements per page; the form itself is left open at :147, reading R1).  Plain definition (reading
+# R24): the arithmetic mean of the page's valid keys, evaluated in fp64 (a sum of at most 128 bf16 values is exact in
+# fp64 unless their exponents span more than 40 binades) and rounded ONCE to bf16, nearest even.  Everything after it
 # (score, top-k, attention) is fp64 as in O5..O8.
-def _bf16_round_bits(x32: np.ndarray) -> np.ndarray:
-    u = x32.astype(np.float32).view(np.uint32).astype(np.uint64)
-    return (((u + 0x7FFF + ((u >> 16) & 1)) >> 16) & 0xFFFF).astype(np.uint16)
+def _round_to_bf16_bits(x: np.ndarray) -> np.ndarray:
+    """fp64 -> nearest bf16 (8 significant bits, ties to even), returned as the bf16 BIT pattern.  Written on the
+    significand directly so that there is one rounding only (fp64 -> fp32 -> bf16 would round twice)."""
+    x = np.asarray(x, dtype=np.float64)
+    m, e = np.frexp(x)                                   # x = m * 2^e, 0.5 <= |m| < 1
+    y = np.ldexp(np.rint(np.ldexp(m, 8)), e - 8)         # rint rounds halves to even; 8 bits of significand kept
+    assert (np.abs(y[y != 0]) >= 2.0 ** -126).all(), "bf16 subnormals are outside this oracle's scope"
+    return (y.astype(np.float32).view(np.uint32) >> 16).astype(np.uint16)      # y is exactly representable: no rounding here
 
 
 def summarize_mean(k_cache, page_ids, n_valid=None) -> np.ndarray:
-    """k_cache [n_phys][Hkv][P][D] uint16 (bf16 bits) -> mean-key landmarks [n_update][Hkv][D] as bf16 BITS (uint16)."""
+    """k_cache [n_phys][Hkv][P][D] uint16 (bf16 bits) -> mean-key landmarks [n_update][Hkv][D] as bf16 BITS (uint16):
+    mean over the page's valid tokens (fp64), rounded once to bf16."""
     k_cache = _u16(k_cache)
     P = k_cache.shape[2]
     out = np.zeros((len(page_ids), k_cache.shape[1], k_cache.shape[3]), dtype=np.uint16)
     for u, page in enumerate(page_ids):
         valid = P if n_valid is None else int(n_valid[u])
-        rows = (k_cache[int(page)].astype(np.uint32) << 16).view(np.float32)          # [Hkv][P][D] exact fp32
-        acc = np.zeros((rows.shape[0], rows.shape[2]), dtype=np.float32)
+        rows = (k_cache[int(page)].astype(np.uint32) << 16).view(np.float32).astype(np.float64)   # [Hkv][P][D]
+        acc = np.zeros((rows.shape[0], rows.shape[2]), dtype=np.float64)
         for t in range(valid):
-            acc = (acc + rows[:, t, :]).astype(np.float32)
-        out[u] = _bf16_round_bits(acc / np.float32(max(valid, 1)))
+            acc = acc + rows[:, t, :]
+        out[u] = _round_to_bf16_bits(acc / float(max(valid, 1)))
     return out
 
 
-def sparse_step_mean(q, k_cache, v_cache, page_table, seq_lens, sched: Schedule, sm_scale: float, max_sel: Optional[int] = None) -> dict:
+def mean_landmark_band(k_cache, page_ids, n_valid=None):
+    """For a checker: (exact fp64 mean, fp32-accumulation error bound) per landmark entry, [n_update][Hkv][D] each.
+    A kernel that accumulates the page's keys in fp32 (any order) and divides in fp32 returns a value within
+    err = (valid + 1) * 2^-24 * mean_t |k_t| of the exact mean, so its bf16 code may differ from summarize_mean's by
+    one step only where the exact mean lies within err of the rounding boundary between the two codes (reading R24)."""
+    k_cache = _u16(k_cache)
+    P = k_cache.shape[2]
+    shape = (len(page_ids), k_cache.shape[1], k_cache.shape[3])
+    exact, err = np.zeros(shape), np.zeros(shape)
+    for u, page in enumerate(page_ids):
+        valid = P if n_valid is None else int(n_valid[u])
+        rows = (k_cache[int(page)].astype(np.uint32) << 16).view(np.float32).astype(np.float64)[:, :valid, :]
+        exact[u] = rows.sum(1) / float(max(valid, 1))
+        err[u] = (valid + 1) * 2.0 ** -24 * np.abs(rows).sum(1) / float(max(valid, 1))
+    return exact, err
+
+
+def sparse_step_mean(q, k_cache, v_cache, page_table, seq_lens, sched: Schedule, sm_scale: float, max_sel: Optional[int] = None,
+                     landmarks=None) -> dict:
     """O1..O8 with the mean-key landmark: score s[p] = sum_{h in group} q_h . mean[p] (fp64 over the bf16 landmark);
-    budget, forced pages, top-k (ties to the lower page) and attention exactly as sparse_step."""
+    budget, forced pages, top-k (ties to the lower page) and attention exactly as sparse_step.
+    landmarks: optional stored codes [n_phys][Hkv][D] (bf16 bits) to score with instead of summarize_mean's -- a
+    checker passes the codes under test once it has verified them against mean_landmark_band, so that O5..O8 are
+    compared on the same stored landmarks (as R11 does for the attention on the selected sets)."""
     q, k_cache, v_cache = _u16(q), _u16(k_cache), _u16(v_cache)
     page_table, seq_lens = _i32(page_table), _i32(seq_lens)
     n, Hq, D = q.shape
@@ -426,7 +456,8 @@ def sparse_step_mean(q, k_cache, v_cache, page_table, seq_lens, sched: Schedule,
         nv = np.full(n_pages, P, np.int32)
         if L % P:
             nv[-1] = L % P
-        lm = (summarize_mean(k_cache, page_table[i, :n_pages], nv).astype(np.uint32) << 16).view(np.float32).astype(np.float64)
+        lm_bits = summarize_mean(k_cache, page_table[i, :n_pages], nv) if landmarks is None else _u16(landmarks)[page_table[i, :n_pages]]
+        lm = (lm_bits.astype(np.uint32) << 16).view(np.float32).astype(np.float64)
         for g in range(Hkv):
             s = lm[:, g, :] @ qf[i, g * r:(g + 1) * r].sum(0)
             res["scores"][i, g, :n_pages] = s

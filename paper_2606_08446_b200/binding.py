@@ -78,7 +78,8 @@ _SIGS = {
     "sparrow_append": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _SHP, _vp]),
     "sparrow_step": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _SCH, _vp, _i32, _vp, _vp, _vp, _vp, _f, _vp, _sz, _SHP, _vp]),
     "sparrow_step_workspace_bytes": (_sz, [_SHP, _i32]),
-    "sparrow_step_host": (C.c_int, [_vp, _vp, _vp, _vp, _i64, _vp, _vp, _vp, _vp, _SCH, _i32, _f, _vp, _vp, _sz, _SHP, _vp]),
+    "sparrow_step_host": (C.c_int, [_vp, _i64, C.c_int, _vp, _vp, _vp, _vp, _SCH, _i32, _f, _vp, _vp, _sz, _SHP, _vp]),
+    "sparrow_step_host_block_bytes": (_sz, [_SHP, C.POINTER(_sz), C.POINTER(_sz), C.POINTER(_sz)]),
     "sparrow_select_workspace_bytes": (_sz, [_SHP]),
     "sparrow_decode_workspace_bytes": (_sz, [_SHP, _i32]),
     "sparrow_step_scratch_bytes": (_sz, [_SHP, _i32]),
@@ -252,12 +253,32 @@ def sparrow_step(q, k_cache, v_cache, summaries, page_table, seq_lens, sched, se
     return rc
 
 
-def sparrow_step_host(q_host, seq_lens_host, page_ids_host, n_valid_host, n_update: int, k_cache, v_cache, summaries,
+def sparrow_step_host_block_bytes(shape):
+    """(bytes of the pinned host block, offset of seq_lens, offset of page_ids, offset of n_valid)."""
+    o = [_sz(0), _sz(0), _sz(0)]
+    n = _lib.sparrow_step_host_block_bytes(_by(shape), _by(o[0]), _by(o[1]), _by(o[2]))
+    return n, o[0].value, o[1].value, o[2].value
+
+
+class HostBlock:
+    """The pinned host block of sparrow_step_host as torch views (marshalling only): .q [n][Hq][128] bf16, .seq_lens [n],
+    .page_ids [n], .n_valid [n] int32 all alias .block."""
+
+    def __init__(self, shape):
+        n, o_l, o_i, o_v = sparrow_step_host_block_bytes(shape)
+        self.block = torch.zeros((n,), dtype=torch.uint8).pin_memory()
+        ns = shape.n_seq
+        self.q = self.block[: ns * shape.n_q_heads * 256].view(torch.bfloat16).view(ns, shape.n_q_heads, 128)
+        self.seq_lens = self.block[o_l: o_l + 4 * ns].view(torch.int32)
+        self.page_ids = self.block[o_i: o_i + 4 * ns].view(torch.int32)
+        self.n_valid = self.block[o_v: o_v + 4 * ns].view(torch.int32)
+
+
+def sparrow_step_host(in_block, n_update: int, has_n_valid: bool, k_cache, v_cache, summaries,
                       page_table, sched, max_sel: int, sm_scale: float, out_host, scratch, shape, stream=None, *, check=True):
-    rc = _lib.sparrow_step_host(_ptr(q_host, cuda=False), _ptr(seq_lens_host, cuda=False), _ptr(page_ids_host, cuda=False),
-                                _ptr(n_valid_host, cuda=False), n_update, _ptr(k_cache), _ptr(v_cache), _ptr(summaries),
-                                _ptr(page_table), _by(sched), max_sel, sm_scale, _ptr(out_host, cuda=False), _ptr(scratch),
-                                scratch.numel() * scratch.element_size(), _by(shape), _stream(stream))
+    rc = _lib.sparrow_step_host(_ptr(in_block, cuda=False), n_update, 1 if has_n_valid else 0, _ptr(k_cache), _ptr(v_cache),
+                                _ptr(summaries), _ptr(page_table), _by(sched), max_sel, sm_scale, _ptr(out_host, cuda=False),
+                                _ptr(scratch), scratch.numel() * scratch.element_size(), _by(shape), _stream(stream))
     if check:
         _check(rc, "sparrow_step_host")
     return rc

@@ -17,6 +17,16 @@ def sources():
         os.path.join(_HERE, "..", "include", "sparrow.h")]
 
 
+def source_hash() -> str:
+    """Short hash of the kernel sources + the C header: names the build a measurement (e.g. an ncu capture) was taken on."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in sources():
+        h.update(os.path.basename(f).encode())
+        h.update(open(f, "rb").read())
+    return h.hexdigest()[:12]
+
+
 def stale() -> bool:
     if not os.path.exists(LIB):
         return True

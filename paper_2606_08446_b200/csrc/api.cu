@@ -378,7 +378,7 @@ int sparrow_cost_model(const sparrow_cost_args_t *a, sparrow_cost_t *c)
     c->dense_total = c->dense_comp + a->intensity * c->dense_mem;
     c->sparse_comp = param_comp + a->r * BN * a->D * c->attn_elems_sparse;
     c->sparse_mem = param_mem + BN * a->D * c->attn_elems_sparse;
-    c->scoring_comp = 2 * a->r * BN * a->D * c->landmark_visits;
+    c->scoring_comp = a->r * a->landmarks_per_page * BN * a->D * c->landmark_visits;   // r D multiply-adds per landmark vector
     c->scoring_mem = a->landmarks_per_page * BN * a->D * c->landmark_visits;
     c->sparse_total = c->sparse_comp + c->scoring_comp + a->intensity * (c->sparse_mem + c->scoring_mem);
     return SPARROW_OK;
@@ -583,13 +583,13 @@ int sparrow_step(const void *q, const void *k_cache, const void *v_cache, const 
 }
 
 // Device scratch of the host-buffer step, carved in this order (each 256-byte aligned):
-//   q | seq_lens | page_ids | n_valid | sel_pages | sel_count | out | fused-step workspace | dense decode workspace
+//   q | seq_lens | page_ids | n_valid   (the image of the caller's pinned host block: ONE H2D copy brings it over)
+//   | sel_pages | sel_count | out | select + decode workspace | dense decode workspace
 namespace {
 struct StepCarve {
-    size_t q, lens, ids, nval, sel, cnt, out, sel_ws, dec_ws, total;
+    size_t q, lens, ids, nval, in_end, sel, cnt, out, sel_ws, dec_ws, total;
     size_t sel_ws_bytes, dec_ws_bytes;
 };
-constexpr int64_t kStepMaxUpdates = 4096;     // pages that can fill in one step (<= n_seq in practice)
 StepCarve step_carve(const sparrow_shape_t *s, int32_t max_sel)
 {
     StepCarve c;
@@ -597,8 +597,9 @@ StepCarve step_carve(const sparrow_shape_t *s, int32_t max_sel)
     const size_t n = (size_t)s->n_seq;
     c.q = o; o += align256(n * s->n_q_heads * kDim * 2);
     c.lens = o; o += align256(n * 4);
-    c.ids = o; o += align256(kStepMaxUpdates * 4);
-    c.nval = o; o += align256(kStepMaxUpdates * 4);
+    c.ids = o; o += align256(n * 4);               // at most one page per sequence fills in a step
+    c.nval = o; o += align256(n * 4);
+    c.in_end = o;
     c.sel = o; o += align256(n * s->n_kv_heads * (size_t)(max_sel > 0 ? max_sel : 1) * 4);
     c.cnt = o; o += align256(n * 4);
     c.out = o; o += align256(n * s->n_q_heads * kDim * 2);
@@ -617,8 +618,17 @@ size_t sparrow_step_scratch_bytes(const sparrow_shape_t *s, int32_t max_sel)
     return step_carve(s, max_sel).total;
 }
 
-int sparrow_step_host(const void *q_host, const int32_t *seq_lens_host, const int32_t *page_ids_host,
-                      const int32_t *n_valid_host, int64_t n_update, const void *k_cache, const void *v_cache,
+size_t sparrow_step_host_block_bytes(const sparrow_shape_t *s, size_t *off_seq_lens, size_t *off_page_ids, size_t *off_n_valid)
+{
+    if (check_shape(s) != SPARROW_OK) return 0;
+    const StepCarve c = step_carve(s, 1);
+    if (off_seq_lens) *off_seq_lens = c.lens;
+    if (off_page_ids) *off_page_ids = c.ids;
+    if (off_n_valid) *off_n_valid = c.nval;
+    return c.in_end;
+}
+
+int sparrow_step_host(const void *in_block_host, int64_t n_update, int has_n_valid, const void *k_cache, const void *v_cache,
                       void *summaries, const int32_t *page_table, const sparrow_schedule_t *sched, int32_t max_sel,
                       float sm_scale, void *out_host, void *scratch, size_t scratch_bytes, const sparrow_shape_t *s,
                       void *stream)
@@ -629,30 +639,24 @@ int sparrow_step_host(const void *q_host, const int32_t *seq_lens_host, const in
     SchedDev sd;
     rc = to_dev_sched(sched, &sd, s->page_size);
     if (rc) return rc;
-    if (!q_host || !seq_lens_host || !k_cache || !v_cache || !summaries || !page_table || !out_host || !scratch || max_sel <= 0)
+    if (!in_block_host || !k_cache || !v_cache || !summaries || !page_table || !out_host || !scratch || max_sel <= 0)
         return SPARROW_ERR_INVALID_ARG;
-    if (n_update < 0 || n_update > kStepMaxUpdates || (n_update > 0 && !page_ids_host)) return SPARROW_ERR_INVALID_ARG;
+    if (n_update < 0 || n_update > s->n_seq) return SPARROW_ERR_INVALID_ARG;
     if (!aligned16(k_cache) || !aligned16(v_cache) || !aligned16(summaries) || !aligned16(scratch)) return SPARROW_ERR_INVALID_ARG;
     const StepCarve c = step_carve(s, max_sel);
     if (scratch_bytes < c.total) return SPARROW_ERR_WORKSPACE_TOO_SMALL;
     cudaStream_t st = (cudaStream_t)stream;
     uint8_t *base = reinterpret_cast<uint8_t *>(scratch);
     const size_t qbytes = (size_t)s->n_seq * s->n_q_heads * kDim * 2;
+    // one copy for the step's inputs: the block up to the end of what this step uses
+    const size_t in_bytes = n_update == 0 ? c.lens + (size_t)s->n_seq * 4
+                                          : (has_n_valid ? c.nval : c.ids) + (size_t)n_update * 4;
     cudaError_t e;
-    if ((e = cudaMemcpyAsync(base + c.q, q_host, qbytes, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(e, "H2D q");
-    if ((e = cudaMemcpyAsync(base + c.lens, seq_lens_host, (size_t)s->n_seq * 4, cudaMemcpyHostToDevice, st)) != cudaSuccess)
-        return cuda_fail(e, "H2D seq_lens");
+    if ((e = cudaMemcpyAsync(base, in_block_host, in_bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(e, "H2D step inputs");
     const int32_t *lens_d = reinterpret_cast<const int32_t *>(base + c.lens);
     if (n_update > 0) {
-        if ((e = cudaMemcpyAsync(base + c.ids, page_ids_host, (size_t)n_update * 4, cudaMemcpyHostToDevice, st)) != cudaSuccess)
-            return cuda_fail(e, "H2D page_ids");
-        const int32_t *nv_d = nullptr;
-        if (n_valid_host) {
-            if ((e = cudaMemcpyAsync(base + c.nval, n_valid_host, (size_t)n_update * 4, cudaMemcpyHostToDevice, st)) != cudaSuccess)
-                return cuda_fail(e, "H2D n_valid");
-            nv_d = reinterpret_cast<const int32_t *>(base + c.nval);
-        }
-        rc = summarize_impl(k_cache, summaries, reinterpret_cast<const int32_t *>(base + c.ids), nv_d, n_update, s, st);
+        rc = summarize_impl(k_cache, summaries, reinterpret_cast<const int32_t *>(base + c.ids),
+                            has_n_valid ? reinterpret_cast<const int32_t *>(base + c.nval) : nullptr, n_update, s, st);
         if (rc) return rc;
     }
     if (sd.kind == SPARROW_SCHED_DENSE) {

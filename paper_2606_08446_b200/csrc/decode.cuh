@@ -4,13 +4,13 @@
 // Work decomposition ("stream-K" over pages, self-scheduled): the (page, kv-head) tiles of the whole batch form
 // ONE flat stream, ordered (sequence, kv-head, list position); its length T = Hkv * sum_i cnt_i is known from
 // sel_count (or from seq_lens for the dense entry).  A persistent grid of one CTA per SM streams it, each warp a
-// contiguous RANGE of tiles at a time.  Warps do not stream at equal speed (measured: equal static ranges finish
-// 15 % apart), so the stream is cut by factoring self-scheduling: round 0 hands every warp one range of 5/8 of its
-// fair share (no atomic: range index = warp index), every later round cuts half of what is left into W equal
-// ranges (down to kDecMinRange tiles), and a warp that runs out takes the next range index from one atomic
-// counter -- fetched a whole range ahead, so its latency is never seen.  The ranges are a pure function of T,
-// which every warp evaluates from a small table in shared memory.  A range that crosses a (sequence, kv-head)
-// boundary closes one softmax state and opens the next; the K/V ring keeps running across range boundaries.
+// contiguous RANGE of tiles.  Default: ONE round of equal static ranges (range index = warp index, no atomic).  A
+// factoring self-scheduler is built in but opt-in (SPARROW_DEC_R0_EIGHTHS < 8: round 0 hands out that many eighths
+// of the fair share, every later round half of what is left, a warp that runs out takes the next range index from
+// one atomic counter): measured slower, because every extra range adds a partial and a merge on the critical path
+// (DESIGN.md 6.3).  The ranges are a pure function of T, which every warp evaluates from a small table in shared
+// memory.  A range that crosses a (sequence, kv-head) boundary closes one softmax state and opens the next; the K/V
+// ring keeps running across range boundaries.
 // The whole GQA group (r <= 8 query heads) is processed together, so each K/V byte is read from HBM once.
 //
 // Split-K merge (a7): a (sequence, kv-head) unit covered by one range is normalised and written straight to `out`;
@@ -368,6 +368,16 @@ __device__ __forceinline__ void decode_warp_stream(const DecodeArgs &A, const in
             const uint32_t kb = ring_u32 + stage * kStageBytes;
             const uint32_t vb = kb + kTileBytes;
             stage = stage + 1 == kDecStages ? 0 : stage + 1;
+            const int valid = info & 31;
+            if (valid < kPage) {
+                // Warp-uniform, at most one tile per unit (plus the sub-tiles past L of a larger page): token rows >= valid
+                // hold whatever the pool held (an unwritten or recycled page).  Their scores are masked to -inf below, so
+                // p = 0, but 0 x NaN/Inf in the P V product would still poison the output row: zero those V rows in the
+                // stage (K needs nothing: a masked score is replaced, never multiplied).
+                for (int idx = valid * 16 + lane; idx < kPage * 16; idx += 32)
+                    asm volatile("st.shared.v4.u32 [%0], {%1,%1,%1,%1};" ::"r"(vb + tile_off(idx >> 4, idx & 15)), "r"(0u) : "memory");
+                __syncwarp();
+            }
 
             // ---- S = Q K^T: two n-tiles (tokens 0-7, 8-15), 8 k-steps ----
             float s0a = 0.f, s0b = 0.f, s1a = 0.f, s1b = 0.f;
@@ -379,7 +389,6 @@ __device__ __forceinline__ void decode_warp_stream(const DecodeArgs &A, const in
                 mma_rows07(s1a, s1b, qa[kk][0], qa[kk][1], b2, b3);
             }
             // ---- online softmax: this lane holds head lane/4, tokens col, col+1, col+8, col+9 of the page ----
-            const int valid = info & 31;
             float x0 = col < valid ? s0a * scale_log2 : -INFINITY;
             float x1 = col + 1 < valid ? s0b * scale_log2 : -INFINITY;
             float x2 = col + 8 < valid ? s1a * scale_log2 : -INFINITY;
@@ -439,13 +448,14 @@ __device__ __forceinline__ void decode_warp_stream(const DecodeArgs &A, const in
                 }
             }
             // release / acquire through ONE atomic of lane 0 (no fence per lane): the warp barrier orders the lanes'
-            // partial stores before lane 0's acq_rel atomic (cumulative at gpu scope), and the shuffle that hands its
-            // result round orders that acquire before the other lanes' reads of the slots (ld.global.cg below)
+            // partial stores before lane 0's acq_rel atomic (cumulative at gpu scope), and the warp barrier after the
+            // shuffle that hands its result round orders that acquire before the other lanes' reads of the slots
             __syncwarp();
             int old = 0;
             if (lane == 0)
                 asm volatile("atom.acq_rel.gpu.global.add.s32 %0, [%1], 1;" : "=r"(old) : "l"(counters + unit) : "memory");
             old = __shfl_sync(kFull, old, 0);
+            __syncwarp();                                            // a shuffle is not a memory-ordering operation; the warp barrier is
             if (old != w1 - w0) continue;                            // not the last segment to arrive
             if (lane == 0) counters[unit] = 0;                       // restore the zero for the next call
             const int nseg = w1 - w0 + 1;

@@ -72,8 +72,9 @@ summarize_kernel(const uint16_t *__restrict__ k_cache, uint16_t *__restrict__ su
 }
 
 // Mean-key landmark (the single vector per page of the paper's cost model): mean[d] = (sum over the
-// page's valid tokens of K[t][d]) / valid, accumulated in fp32 in token order t = 0, 1, ... and rounded to bf16 once
-// (round to nearest even) -- the order is part of the definition, so the result is reproducible bit for bit.
+// page's valid tokens of K[t][d]) / valid, accumulated in fp32 (token order) and rounded to bf16 once (nearest even).
+// The definition is the exact mean rounded once (reading R24); the fp32 sum is within (valid + 1) 2^-24 mean|k| of it,
+// so the stored code is that one or, next to a rounding boundary, its neighbour -- the checker's validity band.
 // One warp per (page, kv-head); lane = 4 channels (8 bytes), so a row is one coalesced 256-byte load.
 __device__ __forceinline__ void mean_of_page(const uint16_t *__restrict__ src, int valid, int lane, uint16_t *__restrict__ dst,
                                              bool coherent)

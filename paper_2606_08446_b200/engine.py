@@ -38,6 +38,8 @@ class SparrowEngine:
         self.sched_spec = dict(spec)
         self.sched = B.make_schedule(spec, page_size=self.wl.page_size)
         max_len = int(self.wl.seq_lens.max().item())
+        self._len_now = max_len          # host-side bound on the longest cached length (appends add to it)
+        self._len_sized = max_len        # the length max_sel is sized for
         self.max_sel = max(1, B.sparrow_max_sel_pages(self.sched, max_len))
         self.sel_pages = torch.full((self.wl.n_seq, self.wl.Hkv, self.max_sel), -1, dtype=torch.int32, device=dev)
         self.sparse_ws = torch.zeros((B.sparrow_decode_workspace_bytes(self.shape, self.max_sel),), dtype=torch.uint8, device=dev)
@@ -80,12 +82,26 @@ class SparrowEngine:
     def append(self, k_new, v_new, stream=None):
         """Cache side of a rollout step: write the token's K/V at position L, L += 1, summarize the page if it filled."""
         wl = self.wl
+        # sparrow_append leaves a sequence untouched when its page table is full, and sparrow_select clamps to max_sel:
+        # both are silent on the device, so the bounds are enforced here on the host (the lengths themselves live on
+        # the device; _len_now is their host-side upper bound)
+        assert self._len_now + 1 <= wl.max_pages * wl.page_size, "append: the page table has no room for another token"
+        assert self._len_now + 1 <= self._len_sized, "append: call reserve(n_steps) first (max_sel is sized for the current lengths)"
+        self._len_now += 1
         return B.sparrow_append(k_new, v_new, wl.k_cache, wl.v_cache, self.summaries, wl.page_table, wl.seq_lens, self.shape, stream)
+
+    def note_appended(self, n_tokens: int):
+        """Tell the engine that n_tokens more tokens per sequence were (or will be) appended outside its view, e.g. by
+        replaying a captured rollout graph again: keeps the host-side length bound, and its checks, in step."""
+        assert self._len_now + n_tokens <= self._len_sized, "note_appended: beyond what reserve() sized the buffers for"
+        self._len_now += n_tokens
 
     def reserve(self, n_steps: int):
         """Size the selection buffers for lengths up to the current maximum + n_steps (B(L) grows with L)."""
-        max_len = int(self.wl.seq_lens.max().item()) + n_steps
+        self._len_now = int(self.wl.seq_lens.max().item())
+        max_len = self._len_now + n_steps
         assert max_len <= self.wl.max_pages * self.wl.page_size, "the page table has no room for that many appended tokens"
+        self._len_sized = max_len
         dev = self.wl.q.device
         self.max_sel = max(1, B.sparrow_max_sel_pages(self.sched, max_len))
         self.sel_pages = torch.full((self.wl.n_seq, self.wl.Hkv, self.max_sel), -1, dtype=torch.int32, device=dev)

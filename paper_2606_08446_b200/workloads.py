@@ -84,6 +84,30 @@ class Workload:
                     seq_lens=self.seq_lens.cpu().numpy().astype(np.int32))
 
 
+def host_subset(wl: "Workload", idx) -> dict:
+    """Host view (exact bit patterns, as Workload.host) of the sequences `idx` only, with the K/V pools COMPACTED to
+    the pages those sequences own and the page table renumbered accordingly -- data movement only, so that a checker
+    can look at a few sequences of a 13 GiB pool without copying the pool.  Extra keys: 'seq_index' (the original
+    sequence numbers, in row order) and 'phys_ids' (original physical page of every compacted page)."""
+    idx = [int(i) for i in idx]
+    P = wl.page_size
+    lens = wl.seq_lens.cpu()[idx].tolist()
+    npg = [-(-L // P) for L in lens]
+    pt_dev = wl.page_table[torch.as_tensor(idx, device=wl.page_table.device)]
+    ids = torch.cat([pt_dev[j, :n] for j, n in enumerate(npg)]).long()
+    new_pt = np.zeros((len(idx), max(npg)), dtype=np.int32)
+    o = 0
+    for j, n in enumerate(npg):
+        new_pt[j, :n] = np.arange(o, o + n, dtype=np.int32)
+        o += n
+
+    def bits(t):
+        return t.detach().contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
+    return dict(q=bits(wl.q[torch.as_tensor(idx, device=wl.q.device)]), k_cache=bits(wl.k_cache[ids]), v_cache=bits(wl.v_cache[ids]),
+                page_table=new_pt, seq_lens=np.asarray(lens, dtype=np.int32), seq_index=np.asarray(idx, dtype=np.int64),
+                phys_ids=ids.cpu().numpy())
+
+
 def draw_lengths(spec, n_seq: int, gen: torch.Generator) -> List[int]:
     kind = spec[0]
     if kind == "list":
@@ -104,7 +128,7 @@ def draw_lengths(spec, n_seq: int, gen: torch.Generator) -> List[int]:
 
 def make_workload(name: str = "custom", *, n_seq: int, Hq: int, Hkv: int, lengths, schedule: dict,
                   plant: bool = False, seed: int = 0, device="cpu", spare_pages: int = 3,
-                  poison_tail: bool = False, plant_scale: float = 3.0, plant_frac: float = 0.05,
+                  poison_tail=False, plant_scale: float = 3.0, plant_frac: float = 0.05,
                   chunk_pages: int = 8192, reserve_tokens: int = 0, page_size: int = PAGE, **_ignored) -> Workload:
     """Draw one batch.  Lengths, page tables and planted pages come from a CPU generator (so they do
     not depend on the device); q/K/V values come from a generator on ``device``."""
@@ -169,8 +193,12 @@ def make_workload(name: str = "custom", *, n_seq: int, Hq: int, Hkv: int, length
             tail = L % P
             if tail:
                 ph = int(page_table[i, L // P])
-                k_cache[ph, :, tail:, :] = 1.0e4
-                v_cache[ph, :, tail:, :] = -1.0e4
+                if poison_tail == "nonfinite":      # what a torch.empty pool or a recycled page may hold
+                    k_cache[ph, :, tail:, :] = float("nan")
+                    v_cache[ph, :, tail:, :] = float("inf")
+                else:
+                    k_cache[ph, :, tail:, :] = 1.0e4
+                    v_cache[ph, :, tail:, :] = -1.0e4
 
     return Workload(
         name=name, n_seq=n_seq, Hq=Hq, Hkv=Hkv, schedule=dict(schedule),

@@ -39,3 +39,18 @@ def test_two_rank_replicas_aggregate_over_max_time():
 def test_single_process_defaults():
     assert D.env_world()[2] >= 1
     assert D.max_over_ranks(3.5) == 3.5 and D.shard_sequences(10, 0, 1) == list(range(10))
+
+
+def test_bench_gpus_n_starts_n_ranks_itself():
+    """`bench.py --gpus 2` without a torchrun environment must start the two ranks itself (one process per GPU on the
+    GPU box; gloo here) and rank 0 must report n_gpus = 2."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT")}
+    p = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--launch-check"], env=env, capture_output=True,
+                       text=True, timeout=300)
+    assert p.returncode == 0, p.stderr[-2000:]
+    line = [json.loads(ln) for ln in p.stdout.splitlines() if ln.startswith("{")]
+    assert len(line) == 1 and line[0] == {"launch_check": True, "n_gpus": 2, "world_size": 2, "requested": 2}

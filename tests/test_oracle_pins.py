@@ -451,6 +451,20 @@ def test_cost_model_against_per_step_sums_and_limits():
         assert math.isclose(c["dense_comp"], 2 * P_ * B_ * N_ * L_out + r_ * B_ * N_ * D_ * c["attn_elems_dense"], rel_tol=1e-15)
         assert math.isclose(c["scoring_mem"], 2.0 * B_ * N_ * D_ * c["landmark_visits"], rel_tol=1e-15)
         assert math.isclose(c["sparse_total"], c["sparse_comp"] + c["scoring_comp"] + I_ * (c["sparse_mem"] + c["scoring_mem"]), rel_tol=1e-15)
+    # Eq. 3's two clean scoring terms as PRINTED at PAPER.md:142 (L_in = 0, one landmark vector per page, B = 1):
+    #   compute r N D L_out^2 / (2 pagesize),  memory (before I) N D L_out^2 / (2 pagesize).
+    # The calculator leaves out the K dense steps at the start (App. F's L_dense), i.e. a factor 1 - (K / L_out)^2.
+    for L_out, K in [(32768.0, 16.0), (20000.0, 2048.0)]:
+        c = oracle.cost_model(0.0, 1.0, N_, 0.0, L_out, D_, r_, I_, K, ps, c=1.0)
+        under_budget = 1.0 - (K / L_out) ** 2
+        assert math.isclose(c["scoring_comp"], r_ * N_ * D_ * L_out ** 2 / (2 * ps) * under_budget, rel_tol=1e-12)
+        assert math.isclose(c["scoring_mem"], N_ * D_ * L_out ** 2 / (2 * ps) * under_budget, rel_tol=1e-12)
+    c = oracle.cost_model(0.0, 1.0, N_, 0.0, 32768.0, D_, r_, I_, 16.0, ps, c=1.0)
+    assert math.isclose(c["scoring_comp"], r_ * N_ * D_ * 32768.0 ** 2 / (2 * ps), rel_tol=1e-6)      # K << L_out: the printed term
+    # the same r : 1 compute-to-memory ratio as the attention terms (Eq. 3's 2 r N D B L_out vs 2 I N D B L_out), any c
+    c2 = oracle.cost_model(P_, B_, N_, 500.0, 9000.0, D_, r_, I_, 1024.0, ps, c=2.0)
+    assert math.isclose(c2["scoring_comp"], r_ * c2["scoring_mem"], rel_tol=1e-15)
+    assert math.isclose(c2["sparse_comp"] - 2 * P_ * B_ * N_ * 9000.0, r_ * (c2["sparse_mem"] - 2 * P_ * 9000.0), rel_tol=1e-12)
     # budget covers the whole context: sparse == dense, nothing is scored
     c = oracle.cost_model(P_, B_, N_, 100.0, 500.0, D_, r_, I_, 4096.0, ps)
     assert c["attn_elems_sparse"] == c["attn_elems_dense"] and c["landmark_visits"] == 0 and c["sparse_total"] == c["dense_total"]
@@ -559,30 +573,61 @@ def test_binned_quantile_is_the_nearest_rank_quantile():
 
 
 # ------------------------------------------------------------------ 8(f)-2: the mean-key landmark ----
-def test_mean_landmark_against_torch_and_exact_mean():
-    """summarize_mean = fp32 running sum in token order / count -> bf16 (nearest even).  Pinned with torch's own fp32
-    cumsum and bf16 rounding (a library routine, not a retyping), against the exact mean (never more than one bf16
-    step away), and on the special cases: one valid token -> that key; identical keys -> that key."""
+def _bf16_neighbours(x: float):
+    """The two bf16 values that bracket x (found by truncating the fp32 pattern; independent of the oracle's rounding)."""
+    f = np.array([x], dtype=np.float32)
+    lo_bits = f.view(np.uint32) & np.uint32(0xFFFF0000)
+    cands = []
+    for d in (-1, 0, 1, 2):
+        b = (lo_bits.astype(np.int64) + d * 0x10000).astype(np.uint32)
+        cands.append((float(b.view(np.float32)[0]), int(b[0] >> 16)))
+    return cands
+
+
+def test_mean_landmark_is_the_exact_mean_rounded_once():
+    """summarize_mean = the arithmetic mean of the page's valid keys rounded ONCE to bf16 (reading R24; PAPER.md:142's
+    one vector per page).  Pinned with exact rational arithmetic (fractions.Fraction, no floating point at all): the
+    returned code is the bf16 value nearest to the exact mean -- nearer than every neighbouring code, ties to the even
+    code -- and on the special cases: one valid token -> that key; identical keys -> that key; mean_landmark_band's
+    exact mean == the rational mean to fp64 precision."""
+    from fractions import Fraction
     wl = W.make_workload(n_seq=2, Hq=4, Hkv=2, lengths=("list", [100, 37]), schedule=W._sched("dense", 0, 0), seed=77, device="cpu")
     h = wl.host()
     ids = np.array([0, 3, 5, 2], np.int32)
     nv = np.array([16, 1, 9, 16], np.int32)
     got = oracle.summarize_mean(h["k_cache"], ids, nv)
+    exact64, err = oracle.mean_landmark_band(h["k_cache"], ids, nv)
+    kf = f64(h["k_cache"])
     for u, (pg, v) in enumerate(zip(ids, nv)):
-        rows = wl.k_cache[int(pg)].float()[:, :v, :]                                     # [Hkv][v][D] fp32 (exact)
-        want = (rows.cumsum(1)[:, -1, :] / float(v)).to(torch.bfloat16)
-        assert np.array_equal(got[u], want.view(torch.int16).numpy().view(np.uint16))
-        exact = f64(h["k_cache"][pg])[:, :v, :].mean(1)
-        step = np.maximum(np.abs(exact), 2.0 ** -126) * 2.0 ** -7                        # one bf16 step at that magnitude
-        assert (np.abs(f64(got[u]) - exact) <= step).all()
+        for g in range(2):
+            for d in range(0, 128, 5):
+                mean = sum(Fraction(float(kf[pg, g, t, d])) for t in range(v)) / int(v)       # exact
+                code = int(got[u, g, d])
+                val = Fraction(float(f64(np.array([code], np.uint16))[0]))
+                dist = abs(val - mean)
+                for nb_val, nb_code in _bf16_neighbours(float(mean)):
+                    if nb_code == code:
+                        continue
+                    nd = abs(Fraction(nb_val) - mean)
+                    assert dist < nd or (dist == nd and code % 2 == 0), (u, g, d, code, nb_code)
+                assert abs(Fraction(float(exact64[u, g, d])) - mean) <= Fraction(2.0 ** -50) * abs(mean) + Fraction(2.0 ** -1000)
+                assert err[u, g, d] >= 0 and err[u, g, d] <= (v + 1) * 2.0 ** -24 * float(np.abs(kf[pg, g, :v, d]).max()) * 1.0000001
     assert np.array_equal(got[1], h["k_cache"][3][:, 0, :])                              # one valid token
     kc = h["k_cache"].copy(); kc[7, :, :, :] = kc[7, :, :1, :]
     assert np.array_equal(oracle.summarize_mean(kc, np.array([7], np.int32))[0], kc[7][:, 0, :])
+    # an fp32 running sum in token order (what a kernel does) lands on the same code or one step away, and only near a boundary
+    for u, (pg, v) in enumerate(zip(ids, nv)):
+        k32 = (wl.k_cache[int(pg)].float()[:, :v, :].cumsum(1)[:, -1, :] / float(v)).to(torch.bfloat16).view(torch.int16).numpy().view(np.uint16)
+        diff = k32.astype(np.int64) - got[u].astype(np.int64)
+        assert (np.abs(diff) <= 1).all()
+        for g, d in zip(*np.nonzero(diff)):
+            mid = 0.5 * (f64(np.array([k32[g, d]], np.uint16))[0] + f64(np.array([got[u, g, d]], np.uint16))[0])
+            assert abs(exact64[u, g, d] - mid) <= err[u, g, d]
 
 
 def test_mean_landmark_step_against_numpy_token_level():
     """The whole step with the mean-key landmark (PAPER.md:142's one vector per page) against a restatement written
-    here: torch fp32 mean per page, score = (sum of the group's queries) . mean, top-k by (score desc, page asc) among the
+    here: fp64 mean per page rounded to the nearer of its two bracketing bf16 values, score = (sum of the group's queries) . mean, top-k by (score desc, page asc) among the
     non-forced pages, softmax over the kept pages' valid tokens; plus planted pages recovered and B >= L == dense."""
     lens = [700, 129, 2050]
     S, Wn, budget = 40, 200, 256
@@ -602,7 +647,8 @@ def test_mean_landmark_step_against_numpy_token_level():
             score = np.zeros(n_pages)
             for p in range(n_pages):
                 v = min(P, L - p * P)
-                m = (wl.k_cache[int(h["page_table"][i, p]), g, :v].float().cumsum(0)[-1] / float(v)).to(torch.bfloat16).double().numpy()
+                mean = Kf[int(h["page_table"][i, p]), g, :v].mean(0)
+                m = np.array([min(_bf16_neighbours(float(x)), key=lambda c: (abs(c[0] - x), c[1] % 2))[0] for x in mean])
                 score[p] = m @ qsum
             cand = [p for p in range(n_pages) if p not in forced]
             keep = list(range(n_pages)) if dense_seq else sorted(forced | set(sorted(cand, key=lambda p: (-score[p], p))[:max(0, budget // P - len(forced))]))
