@@ -3,6 +3,8 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <mutex>
+
 #include "common.cuh"
 #include "decode.cuh"
 #include "select.cuh"
@@ -18,6 +20,59 @@ namespace {
 thread_local int g_launches = 0;
 thread_local char g_errbuf[256] = "";
 constexpr int kNumSmsB200 = 148;
+
+// Per-device launch state: the SM count (queried once per device) and the dynamic shared memory each kernel has been
+// allowed so far (cudaFuncSetAttribute is per device).  Guarded by one mutex: entry points may be called from several
+// host threads, each on its own device.
+struct DevState {
+    bool init = false;
+    int sms = 0;
+    size_t dyn_decode[2] = {0, 0}, dyn_select[2] = {0, 0}, dyn_step = 0, dyn_hist = 0;
+    int fused_ok = -1;           // -1 unknown, 0 the device cannot run the cooperative grid, 1 yes
+};
+constexpr int kMaxDevices = 64;
+DevState g_dev[kMaxDevices];
+std::mutex g_dev_mutex;
+
+// Returns the calling thread's current device state (nullptr + *rc on failure).  The library is written for the
+// B200's 148 SMs: persistent grids are sized from the queried count and capped at 148 (the workspace bounds).
+DevState *dev_state(int *rc)
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess || dev < 0 || dev >= kMaxDevices) {
+        snprintf(g_errbuf, sizeof(g_errbuf), "cudaGetDevice failed or device ordinal >= %d", kMaxDevices);
+        *rc = SPARROW_ERR_CUDA;
+        return nullptr;
+    }
+    DevState *d = &g_dev[dev];
+    std::lock_guard<std::mutex> lock(g_dev_mutex);
+    if (!d->init) {
+        e = cudaDeviceGetAttribute(&d->sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess || d->sms <= 0) {
+            snprintf(g_errbuf, sizeof(g_errbuf), "cannot query the SM count: %s", cudaGetErrorString(e));
+            *rc = SPARROW_ERR_CUDA;
+            return nullptr;
+        }
+        d->init = true;
+    }
+    return d;
+}
+// Raises a kernel's dynamic shared memory limit on this device if `bytes` exceeds what it has been given so far.
+template <typename K>
+int ensure_dyn_smem(K kernel, size_t bytes, size_t *granted, const char *what)
+{
+    std::lock_guard<std::mutex> lock(g_dev_mutex);
+    if (bytes > 32 * 1024 && bytes > *granted) {        // static + dynamic above 48 KiB needs the opt-in; kernels here have < 16 KiB static
+        cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+        if (e != cudaSuccess) {
+            snprintf(g_errbuf, sizeof(g_errbuf), "CUDA error in cudaFuncSetAttribute(%s): %s", what, cudaGetErrorString(e));
+            return SPARROW_ERR_CUDA;
+        }
+        *granted = bytes;
+    }
+    return SPARROW_OK;
+}
 
 int cuda_fail(cudaError_t e, const char *where)
 {
@@ -153,12 +208,11 @@ int launch_decode(const void *q, const void *k_cache, const void *v_cache, const
     float *ws_ml = reinterpret_cast<float *>(reinterpret_cast<uint8_t *>(workspace) + gm.bytes_ctr + gm.bytes_o);
 
     constexpr int kSmemMax = kDecRingBytes + ((kDecMaxSeq + 1) * 4 + 15) / 16 * 16;
-    static bool attr_done[2] = {false, false};
-    if (!attr_done[kDense]) {
-        cudaError_t e = cudaFuncSetAttribute(decode_kernel<kDense>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemMax);
-        if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(decode_kernel)");
-        attr_done[kDense] = true;
-    }
+    int rc_dev = SPARROW_OK;
+    DevState *ds = dev_state(&rc_dev);
+    if (!ds) return rc_dev;
+    rc_dev = ensure_dyn_smem(decode_kernel<kDense>, kSmemMax, &ds->dyn_decode[kDense], "decode_kernel");
+    if (rc_dev) return rc_dev;
     const float scale_log2 = sm_scale * 1.4426950408889634f;
     const int smem = kDecRingBytes + ((s->n_seq + 1) * 4 + 15) / 16 * 16;
     DecodeArgs A;
@@ -192,6 +246,10 @@ int summarize_impl(const void *k_cache, void *summaries, const int32_t *page_ids
     return SPARROW_OK;
 }
 
+// Select workspace: arrival counters (one per (sequence, kv-head) unit; all zero between calls), then the fp32 scores
+// [units][max_pages].
+size_t select_ctr_bytes(const sparrow_shape_t *s) { return align256((size_t)s->n_seq * s->n_kv_heads * sizeof(int32_t)); }
+
 int select_impl(const void *q, const void *summaries, const int32_t *page_table, const int32_t *seq_lens,
                 const SchedDev &sd, int32_t *sel_pages, int32_t max_sel, int32_t *sel_count, float *scores_dbg,
                 void *workspace, size_t workspace_bytes, const sparrow_shape_t *s, cudaStream_t st)
@@ -200,28 +258,26 @@ int select_impl(const void *q, const void *summaries, const int32_t *page_table,
     if (s->max_pages_per_seq > kSelMaxPages) return SPARROW_ERR_UNSUPPORTED;
     if (s->n_phys_pages * s->n_kv_heads >= (1LL << 27)) return SPARROW_ERR_UNSUPPORTED;   // 32-bit offsets in 16-byte units
     if (s->n_seq == 0) return SPARROW_OK;
+    int rc = SPARROW_OK;
+    DevState *ds = dev_state(&rc);
+    if (!ds) return rc;
     int32_t *counters = reinterpret_cast<int32_t *>(workspace);
-    float *scores_ws = reinterpret_cast<float *>(reinterpret_cast<uint8_t *>(workspace) +
-                                                 align256((size_t)s->n_seq * s->n_kv_heads * sizeof(int32_t)));
+    float *scores_ws = reinterpret_cast<float *>(reinterpret_cast<uint8_t *>(workspace) + select_ctr_bytes(s));
     // Pages per CTA: as large as keeps >= 4 CTAs per resident slot (4 per SM) so the tail stays short, because the
-    // per-CTA prologue (plan, Q+/Q-, first table entries) is amortised over the pages a CTA streams.
+    // per-CTA fixed costs (loads of L / table entries / query rows, arrival) are amortised over the pages a CTA streams.
     const int64_t units = (int64_t)s->n_seq * s->n_kv_heads;
     int pages_per_cta = kSelCtaPagesMin;
     for (int p = 4 * kSelCtaPagesMin; p > kSelCtaPagesMin; p >>= 1) {
-        if (units * ((s->max_pages_per_seq + p - 1) / p) >= 4 * kSelMinBlocks * kNumSmsB200) { pages_per_cta = p; break; }
+        if (units * ((s->max_pages_per_seq + p - 1) / p) >= 4 * kSelMinBlocks * ds->sms) { pages_per_cta = p; break; }
     }
 #ifdef SPARROW_SEL_PPC_FIXED
     pages_per_cta = SPARROW_SEL_PPC_FIXED;
 #endif
     const size_t dyn = (size_t)s->max_pages_per_seq * sizeof(uint32_t);
     const bool mean = s->landmark == SPARROW_LANDMARK_MEAN;
-    static size_t dyn_set[2] = {0, 0};
-    if (dyn > 48 * 1024 && dyn > dyn_set[mean]) {
-        cudaError_t e = mean ? cudaFuncSetAttribute(select_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn)
-                             : cudaFuncSetAttribute(select_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
-        if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(select_kernel)");
-        dyn_set[mean] = dyn;
-    }
+    rc = mean ? ensure_dyn_smem(select_kernel<true>, dyn, &ds->dyn_select[1], "select_kernel<mean>")
+              : ensure_dyn_smem(select_kernel<false>, dyn, &ds->dyn_select[0], "select_kernel");
+    if (rc) return rc;
     dim3 grid((s->max_pages_per_seq + pages_per_cta - 1) / pages_per_cta, s->n_kv_heads, s->n_seq);
     if (mean)
         launch_chain(select_kernel<true>, grid, dim3(kSelThreads), dyn, st, (const uint16_t *)q, (const uint16_t *)summaries,
@@ -244,7 +300,7 @@ StepGeom step_geom(const sparrow_shape_t *s, int32_t max_sel)
     StepGeom g;
     const size_t units = (size_t)s->n_seq * s->n_kv_heads;
     const size_t stride = ((size_t)s->max_pages_per_seq + 31) & ~(size_t)31;     // score rows own their 128-byte lines
-    g.sel_bytes = align256(units * sizeof(int32_t)) + align256(units * stride * sizeof(float));
+    g.sel_bytes = align256(units * sizeof(int32_t)) + align256(units * stride * sizeof(float));   // >= the select workspace
     g.flag_bytes = align256((size_t)s->n_seq * s->n_kv_heads * sizeof(int32_t));
     g.dec_bytes = sparrow_decode_workspace_bytes(s, max_sel);
     return g;
@@ -269,25 +325,22 @@ int step_impl(const void *q, const void *k_cache, const void *v_cache, const voi
     constexpr size_t kSmemBudget = 227 * 1024 - 12 * 1024;          // static shared memory and alignment slack
     const bool per_warp = dyn_base + kDecWarps * keys * 4 <= kSmemBudget;
     const size_t dyn = dyn_base + (per_warp ? kDecWarps : 1) * keys * 4;
-    static int fused_ok = -1;                    // -1 unknown, 0 the device cannot run the cooperative grid, 1 yes
-    bool fused = fused_ok != 0 && s->page_size == kPage && s->landmark == SPARROW_LANDMARK_MINMAX && dyn <= kSmemBudget && s->n_seq <= kDecMaxSeq &&
+    int rc_dev = SPARROW_OK;
+    DevState *ds = dev_state(&rc_dev);
+    if (!ds) return rc_dev;
+    bool fused = ds->fused_ok != 0 && s->page_size == kPage && s->landmark == SPARROW_LANDMARK_MINMAX && dyn <= kSmemBudget && s->n_seq <= kDecMaxSeq &&
                  s->n_phys_pages * s->n_kv_heads < (1LL << 27) &&
                  (int64_t)s->n_seq * s->max_pages_per_seq * s->n_kv_heads < (1LL << 31);
-    if (fused && fused_ok < 0) {
-        int dev = 0, coop = 0, sms = 0;
+    if (fused && ds->fused_ok < 0) {
+        int dev = 0, coop = 0;
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        fused_ok = (coop && sms >= kDecGrid) ? 1 : 0;
-        fused = fused_ok == 1;
+        ds->fused_ok = (coop && ds->sms >= kDecGrid) ? 1 : 0;
+        fused = ds->fused_ok == 1;
     }
     if (fused) {
-        static size_t dyn_set = 0;
-        if (dyn > dyn_set) {
-            cudaError_t e = cudaFuncSetAttribute(step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
-            if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(step_kernel)");
-            dyn_set = dyn;
-        }
+        rc_dev = ensure_dyn_smem(step_kernel, dyn, &ds->dyn_step, "step_kernel");
+        if (rc_dev) return rc_dev;
         const DecodeGeom gm = decode_geom(s, max_sel);
         StepArgs S;
         DecodeArgs &A = S.dec;
@@ -317,7 +370,7 @@ int step_impl(const void *q, const void *k_cache, const void *v_cache, const voi
         if (e == cudaSuccess) { ++g_launches; return SPARROW_OK; }
         if (e != cudaErrorCooperativeLaunchTooLarge) return cuda_fail(e, "step_kernel");
         (void)cudaGetLastError();
-        fused_ok = 0;                            // the grid cannot be co-resident here: two launches from now on
+        ds->fused_ok = 0;                        // the grid cannot be co-resident here: two launches from now on
     }
     int rc = select_impl(q, summaries, page_table, seq_lens, sd, sel_pages, max_sel, sel_count, scores_dbg, sel_ws,
                          g.sel_bytes, s, st);
@@ -349,7 +402,7 @@ size_t sparrow_select_workspace_bytes(const sparrow_shape_t *s)
 {
     if (check_shape(s) != SPARROW_OK) return 0;
     const size_t units = (size_t)s->n_seq * s->n_kv_heads;
-    return align256(units * sizeof(int32_t)) + align256(units * s->max_pages_per_seq * sizeof(float));
+    return select_ctr_bytes(s) + align256(units * s->max_pages_per_seq * sizeof(float));
 }
 
 size_t sparrow_decode_workspace_bytes(const sparrow_shape_t *s, int32_t max_sel)
@@ -533,11 +586,12 @@ int sparrow_acceptance(const int32_t *ids_p, const float *logp_p, const int32_t 
     const int bins_per_group = n_bins < 25 ? n_bins : 25;
     const int groups = (n_bins + bins_per_group - 1) / bins_per_group;
     const size_t hsmem = (size_t)bins_per_group * kAccDigits * sizeof(int);
-    static size_t hsmem_set = 0;
-    if (hsmem > 48 * 1024 && hsmem > hsmem_set) {
-        e = cudaFuncSetAttribute(accept_hist_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)hsmem);
-        if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(accept_hist_kernel)");
-        hsmem_set = hsmem;
+    {
+        int rc_dev = SPARROW_OK;
+        DevState *ds = dev_state(&rc_dev);
+        if (!ds) return rc_dev;
+        rc_dev = ensure_dyn_smem(accept_hist_kernel, hsmem, &ds->dyn_hist, "accept_hist_kernel");
+        if (rc_dev) return rc_dev;
     }
     int64_t gx = (n_pos + kAccThreads * 8 - 1) / (kAccThreads * 8);
     const int64_t gmax = (hsmem > 100 * 1024 ? 1 : 2) * kNumSmsB200;

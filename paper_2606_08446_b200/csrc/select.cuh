@@ -5,7 +5,17 @@
 // HBM stream: 512 B of summary per candidate page, gathered through the page table); the LAST CTA of a
 // (sequence, kv-head) to finish -- found with one atomic counter -- runs the top-k over that unit's scores
 // (phase B: radix select on order-preserving keys + ordered compaction).  So the summary stream is spread
-// over all SMs no matter how few (sequence, head) units there are, and selection stays fused in the launch.
+// over all SMs no matter how few (sequence, head) units there are, selection stays fused in the launch, and the
+// hardware's CTA scheduler balances the SMs.  (Round 2 built and measured four persistent forms of this kernel --
+// resident CTAs pulling 256-page items from a counter; per-warp static ranges with a queue of completed units;
+// per-CTA ranges with the octets handed out inside the CTA; one 1024-thread CTA per SM -- and each lost 2-8 us to
+// this one at cfg2 / cfg5: static ranges end 6-8 us apart because CTAs that share an SM are not served equally, and
+// work stealing fine enough to fix that costs a dependent round trip per 4 KiB.  profiles/r2_select.md.)
+//
+// Phase B starts its radix select at the first bit in which the unit's keys differ (scores of one unit share sign,
+// exponent and often more: a fixed top-down pass spends its first passes on bits that split nothing), 8 bits per
+// pass with one histogram bin per thread: typically two passes instead of four, and one packed scan in the
+// compaction instead of two.
 //
 // Score (reading R5): s[p] = sum_{h in group} sum_d max(q_h[d]*mn[d], q_h[d]*mx[d])
 //                          = sum_d ( Q+[d]*mx[d] + Q-[d]*mn[d] ),  Q+ = sum_h max(q_h,0), Q- = sum_h min(q_h,0)
@@ -17,8 +27,8 @@
 // vector, 16-31 the max vector), and kSelBatch such loads are issued back to back before the first is consumed
 // (kSelBatch x 16 B in flight per lane, kSelBatch x 4 KiB per CTA).  Each lane needs only its 8 entries of Q-/Q+
 // in registers.  The per-page partial sums are combined with a transpose-reduce (8 values over 32 lanes in 9
-// shuffles).  (A TMA bulk-copy ring was measured and rejected here: at 512 B per request the copy engine's
-// request rate, not HBM, became the limit -- profiles/r1_select_notes.md.)
+// shuffles).  (A bulk-copy ring was tried in round 1 and dropped: at 512 B per request the copy engine's request
+// rate, not HBM, became the limit.)
 #pragma once
 #include "common.cuh"
 
@@ -34,6 +44,9 @@ constexpr int kSelBatch = 8;                            // summaries in flight p
 constexpr int kSelMinBlocks = SPARROW_SEL_MIN_BLOCKS;   // CTAs / SM the register budget is held to
 constexpr int kSelCtaPagesMin = kSelWarps * kSelPagesPerWarp;                // pages_per_cta is a multiple of this
 constexpr int kSelMaxPages = 16384;  // keys of one unit live in shared memory (64 KiB): 262144 tokens
+constexpr int kSelRadixBits = 8;     // bits per radix-select pass: one histogram bin per thread of the CTA
+constexpr int kSelBins = 1 << kSelRadixBits;
+static_assert(kSelBins == kSelThreads, "the radix-select scan gives every thread one bin");
 
 // fp32 -> uint32 whose unsigned order is the float order (larger score = larger key); never 0 for a real score
 __device__ __forceinline__ uint32_t order_key(float f)
@@ -75,6 +88,131 @@ __device__ __forceinline__ float dot8(const float (&qr)[8], const uint4 v, float
     return acc;
 }
 
+// Phase B: top-k of one (sequence, kv-head) unit by the whole CTA (a5).  The unit's candidate scores are in `ws`
+// (global, written by the CTAs that scored its slices; visible through the arrival atomic).  Exact, no sort:
+//   1. keys -> shared memory (forced pages get the sentinel 0), with the minimum and maximum candidate key;
+//   2. radix select for the k-th best key, 8 bits per pass, starting at the highest bit in which minimum and maximum
+//      differ (everything above it is common to all keys).  Invariant: the k-th best key has (key & mask) == prefix and
+//      is the kk-th best inside that class.  Stops when the class is taken whole (kk == its size) or no bit is left;
+//   3. ordered compaction: forced pages, keys above the class, and the first need_eq keys of the class in page order
+//      are emitted in ascending page order -- the lower-index tie-break (R10) falls out of the scan order.
+__device__ __forceinline__ void unit_topk(const SeqPlan &pl, const float *__restrict__ ws, int32_t *__restrict__ out, int max_sel,
+                                          int32_t *__restrict__ sel_count_slot, uint32_t *s_keys, int *s_hist, int *s_warp,
+                                          uint32_t *s_red, int *s_bcast)
+{
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int n_pages = pl.n_pages;
+    uint32_t kmin = 0xffffffffu, kmax = 0u;
+    for (int p = tid; p < n_pages; p += kSelThreads) {
+        uint32_t key = 0u;
+        if (!pl.forced(p)) {
+            key = order_key(__ldcg(ws + p));
+            kmin = min(kmin, key);
+            kmax = max(kmax, key);
+        }
+        s_keys[p] = key;
+    }
+    s_hist[tid] = 0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        kmin = min(kmin, __shfl_xor_sync(0xffffffffu, kmin, o));
+        kmax = max(kmax, __shfl_xor_sync(0xffffffffu, kmax, o));
+    }
+    if (lane == 0) { s_red[warp] = kmin; s_red[kSelWarps + warp] = kmax; }
+    __syncthreads();
+#pragma unroll
+    for (int w2 = 0; w2 < kSelWarps; ++w2) {
+        kmin = min(kmin, s_red[w2]);
+        kmax = max(kmax, s_red[kSelWarps + w2]);
+    }
+
+    uint32_t prefix = 0, mask = 0;
+    int need_eq = 0;                 // how many keys of the final class are taken (lowest page index first, R10)
+    if (pl.k > 0) {
+        int kk = pl.k;
+        const uint32_t diff = kmin ^ kmax;
+        int top = diff ? 31 - __clz(diff) : -1;          // highest bit still to be resolved (-1: all candidate keys are equal)
+        mask = top < 0 ? 0xffffffffu : (top >= 31 ? 0u : ~((2u << top) - 1u));
+        prefix = kmax & mask;
+        need_eq = kk;
+        int pass = 0;
+        while (top >= 0) {
+            const int shift = top >= kSelRadixBits - 1 ? top - (kSelRadixBits - 1) : 0;
+            const uint32_t dmask = (1u << (top - shift + 1)) - 1u;       // digits of this pass: bits [top, shift]
+            for (int p = tid; p < n_pages; p += kSelThreads) {
+                const uint32_t key = s_keys[p];
+                if (key != 0u && (key & mask) == prefix) atomicAdd(&s_hist[(key >> shift) & dmask], 1);
+            }
+            __syncthreads();
+            // suffix sums over the 256 bins, one bin per thread: S[t] = sum_{j >= t} hist[j]
+            const int h = s_hist[tid];
+            s_hist[tid] = 0;                             // ready for the next pass
+            int suf = h;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int v = __shfl_down_sync(0xffffffffu, suf, o);
+                if (lane + o < 32) suf += v;
+            }
+            if (lane == 0) s_warp[warp] = suf;
+            __syncthreads();
+            for (int w2 = warp + 1; w2 < kSelWarps; ++w2) suf += s_warp[w2];
+            int *bc = s_bcast + 3 * (pass & 1);          // alternate slots: the next pass may write before a slow thread has read
+            if (suf >= kk && suf - h < kk) {             // exactly one bin holds the kk-th best key
+                bc[0] = tid;
+                bc[1] = kk - (suf - h);
+                bc[2] = h;
+            }
+            __syncthreads();
+            prefix |= (uint32_t)bc[0] << shift;
+            mask |= dmask << shift;
+            kk = bc[1];
+            need_eq = kk;
+            if (kk == bc[2]) break;                      // the whole class is taken: no need to split it further
+            top = shift - 1;
+            ++pass;
+        }
+    }
+
+    // Ordered compaction.  Thread t owns the contiguous pages [t*ipt, (t+1)*ipt).  One scan carries both counts: the
+    // pages a thread surely emits (low 16 bits) and its members of the final class (high bits).
+    const int ipt = (n_pages + kSelThreads - 1) / kSelThreads;
+    const int p_lo = tid * ipt, p_hi = min(p_lo + ipt, n_pages);
+    int n_eq = 0, n_sure = 0;
+    for (int p = p_lo; p < p_hi; ++p) {
+        const uint32_t key = s_keys[p];
+        if (key == 0u) n_sure += pl.forced(p);
+        else if (pl.k > 0) {
+            const uint32_t c = key & mask;
+            n_sure += c > prefix;
+            n_eq += c == prefix;
+        }
+    }
+    int tot;
+    const int base = block_excl_scan((n_eq << 16) | n_sure, s_warp, &tot);
+    const int eq_base = base >> 16;                      // class members in lower pages
+    int eq_left = need_eq - eq_base;                     // class members this thread may still take
+    eq_left = eq_left < 0 ? 0 : (eq_left > n_eq ? n_eq : eq_left);
+    int pos = (base & 0xffff) + (eq_base < need_eq ? eq_base : need_eq);
+    for (int p = p_lo; p < p_hi; ++p) {
+        const uint32_t key = s_keys[p];
+        bool take;
+        if (key == 0u) take = pl.forced(p);
+        else if (pl.k > 0) {
+            const uint32_t c = key & mask;
+            take = c > prefix;
+            if (c == prefix && eq_left > 0) { take = true; --eq_left; }
+        } else take = false;
+        if (take) {
+            if (pos < max_sel) out[pos] = p;
+            ++pos;
+        }
+    }
+    if (sel_count_slot && tid == 0) {
+        const int tot_take = (tot & 0xffff) + ((tot >> 16) < need_eq ? (tot >> 16) : need_eq);
+        *sel_count_slot = tot_take < max_sel ? tot_take : max_sel;
+    }
+}
+
 // kMean: the landmark is one vector per page, the mean key (256 B), scored as (sum_h q_h) . mean -- the form the paper's
 // cost model charges (D elements per page); otherwise the min/max pair of north_star (512 B).
 template <bool kMean>
@@ -91,6 +229,7 @@ select_kernel(const uint16_t *__restrict__ q, const uint16_t *__restrict__ summa
     __shared__ int s_hist[256];
     __shared__ int s_warp[kSelWarps];
     __shared__ int s_bcast[4][3];
+    __shared__ uint32_t s_red[2 * kSelWarps];
     __shared__ SeqPlan s_plan;
 
     const int slice = blockIdx.x, g = blockIdx.y, seq = blockIdx.z;
@@ -277,85 +416,7 @@ select_kernel(const uint16_t *__restrict__ q, const uint16_t *__restrict__ summa
     if (!s_bcast[0][0]) return;
 
     // ---------------------------------------------------------------- phase B: top-k of the unit ----
-    const int n_pages = pl.n_pages;
-    for (int p = tid; p < n_pages; p += kSelThreads)
-        s_keys[p] = pl.forced(p) ? 0u : order_key(__ldcg(ws + p));
-    s_hist[tid] = 0;
-    __syncthreads();
-
-    // Radix select, 8 bits per pass, most significant first.  Invariant: the k-th best key has (key & mask) == prefix
-    // and is the kk-th best inside that class.  Stops early when the class is taken whole (kk == its size).
-    uint32_t prefix = 0, mask = 0;
-    int need_eq = 0;                 // how many keys of the final class are taken (lowest page index first, R10)
-    if (pl.k > 0) {
-        int kk = pl.k;
-        for (int pass = 0; pass < 4; ++pass) {
-            const int shift = 24 - 8 * pass;
-            for (int p = tid; p < n_pages; p += kSelThreads) {
-                const uint32_t key = s_keys[p];
-                if (key != 0u && (key & mask) == prefix) atomicAdd(&s_hist[(key >> shift) & 255u], 1);
-            }
-            __syncthreads();
-            // suffix sums over the 256 bins: S[t] = sum_{j >= t} hist[j]
-            const int h = s_hist[tid];
-            s_hist[tid] = 0;                             // ready for the next pass
-            int suf = h;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const int v = __shfl_down_sync(0xffffffffu, suf, o);
-                if (lane + o < 32) suf += v;
-            }
-            if (lane == 0) s_warp[warp] = suf;
-            __syncthreads();
-            for (int w2 = warp + 1; w2 < kSelWarps; ++w2) suf += s_warp[w2];
-            if (suf >= kk && suf - h < kk) {             // exactly one bin holds the kk-th best key
-                s_bcast[pass][0] = tid;
-                s_bcast[pass][1] = kk - (suf - h);
-                s_bcast[pass][2] = h;
-            }
-            __syncthreads();
-            prefix |= (uint32_t)s_bcast[pass][0] << shift;
-            mask |= 255u << shift;
-            kk = s_bcast[pass][1];
-            need_eq = kk;
-            if (kk == s_bcast[pass][2]) break;           // the whole class is taken: no need to split it further
-        }
-    }
-
-    // Ordered compaction.  Thread t owns the contiguous pages [t*ipt, (t+1)*ipt): forced pages, keys above the class,
-    // and the first need_eq keys of the class (page order) are emitted in ascending page order.
-    const int ipt = (n_pages + kSelThreads - 1) / kSelThreads;
-    const int p_lo = tid * ipt, p_hi = min(p_lo + ipt, n_pages);
-    int n_eq = 0, n_sure = 0;
-    for (int p = p_lo; p < p_hi; ++p) {
-        const uint32_t key = s_keys[p];
-        if (key == 0u) n_sure += pl.forced(p);
-        else if (pl.k > 0) {
-            const uint32_t c = key & mask;
-            n_sure += c > prefix;
-            n_eq += c == prefix;
-        }
-    }
-    int tot_eq, tot_take;
-    const int eq_base = block_excl_scan(n_eq, s_warp, &tot_eq);
-    int eq_left = need_eq - eq_base;                     // class members this thread may still take
-    eq_left = eq_left < 0 ? 0 : (eq_left > n_eq ? n_eq : eq_left);
-    int pos = block_excl_scan(n_sure + eq_left, s_warp, &tot_take);
-    for (int p = p_lo; p < p_hi; ++p) {
-        const uint32_t key = s_keys[p];
-        bool take;
-        if (key == 0u) take = pl.forced(p);
-        else if (pl.k > 0) {
-            const uint32_t c = key & mask;
-            take = c > prefix;
-            if (c == prefix && eq_left > 0) { take = true; --eq_left; }
-        } else take = false;
-        if (take) {
-            if (pos < max_sel) out[pos] = p;
-            ++pos;
-        }
-    }
-    if (g == 0 && tid == 0) sel_count[seq] = tot_take < max_sel ? tot_take : max_sel;
+    unit_topk(pl, ws, out, max_sel, g == 0 ? sel_count + seq : nullptr, s_keys, s_hist, s_warp, s_red, &s_bcast[0][0]);
 }
 
 }  // namespace sparrow
