@@ -306,23 +306,16 @@ def run_single(args, cfg, rank, local_rank, world, dev, headline=True) -> dict:
         idx = list(range(wl.n_seq)) if wl.n_seq <= 64 else ext + others[:16 - len(set(ext))]
         chk, h = self_check(eng, wl, idx, dense_idx=ext)
 
-    fused = args.step_form == "fused"
-
     def one_step():
         n = 0
         if upd[0].numel() > 0:
             eng.summarize(upd[0], upd[1], stream=st); n += B.sparrow_last_launch_count()
-        if fused:
-            return n
         eng.select(stream=st); n += B.sparrow_last_launch_count()
         return n
 
     def attend():
-        """second half of the step: the sparse decode launch (or the whole fused select + decode launch)"""
-        if fused:
-            eng.fused_step(stream=st)
-        else:
-            eng.sparse_decode(stream=st)
+        """second half of the step: the sparse decode launch"""
+        eng.sparse_decode(stream=st)
         return B.sparrow_last_launch_count()
 
     # ---- timed region: K steps, device-resident inputs, events on the launching stream ----
@@ -357,8 +350,7 @@ def run_single(args, cfg, rank, local_rank, world, dev, headline=True) -> dict:
             if upd[0].numel() > 0:
                 eng.summarize(upd[0], upd[1], stream=st)
             ev[k][0].record(st)
-            if not fused:
-                eng.select(stream=st)
+            eng.select(stream=st)
             ev[k][1].record(st)
             attend()
             ev[k][2].record(st)
@@ -423,19 +415,18 @@ def run_single(args, cfg, rank, local_rank, world, dev, headline=True) -> dict:
     cnt = eng.sel_count.cpu().numpy()
     ab = algorithmic_bytes(wl, eng, lens, cnt)
     peak, flops, peak_src = measured_peaks()
-    roof_bytes = ab["decode"] + (ab["select"] if fused else 0)       # fused: one launch streams the summaries too
-    roof_kernel = ("step_kernel (one sparrow_step call: scoring + top-k + decode + LSE merge)" if fused else
-                   "decode_kernel<sparse> (one sparrow_sparse_decode call; LSE merge fused in the same launch)")
+    roof_bytes = ab["decode"]
+    roof_kernel = "decode_kernel<sparse> (one sparrow_sparse_decode call; LSE merge fused in the same launch)"
     gbs = lambda b, ms: b / (ms * 1e-3) / 1e9
     dec_gbs, sel_gbs, dense_gbs = gbs(roof_bytes, k_dec["ms"]), gbs(ab["select"], k_sel["ms"]), gbs(ab["dense"], dense_ms)
-    traffic, traffic_note = ncu_traffic(cfg, "step_kernel" if fused else "decode_kernel")
+    traffic, traffic_note = ncu_traffic(cfg, "decode_kernel")
     ms_step = t_max * 1e3 / K
     res = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "bf16", "data": "synthetic",
         "config": {"workload": cfg, "n_seq": wl.n_seq, "Hq": wl.Hq, "Hkv": wl.Hkv, "head_dim": 128, "page_size": 16,
-                   "len_min": int(lens.min()), "len_max": int(lens.max()), "schedule": wl.schedule["kind"], "step_form": args.step_form, "landmark": args.landmark,
+                   "len_min": int(lens.min()), "len_max": int(lens.max()), "schedule": wl.schedule["kind"], "landmark": args.landmark,
                    "sink_tokens": wl.schedule["sink_tokens"], "local_tokens": wl.schedule["local_tokens"],
                    "selected_pages_per_seq_mean": float(cnt.mean()), "parallelism": f"replicas x{world} (no collective)",
                    "l2": "inputs larger than L2: %.0f MB touched per step vs 126 MB L2" % ((ab["decode"] + ab["select"]) / 1e6),
@@ -850,8 +841,6 @@ def main():
                     help="cfg4 (default): the 36-layer step, the largest single-GPU configuration, with the single-layer configs in per_config")
     ap.add_argument("--pools", type=int, default=4, help="cfg4 only: distinct K/V pools the 36 layers rotate over (~14 GiB each)")
     ap.add_argument("--impl", default="sparrow", choices=["sparrow", "reference"])
-    ap.add_argument("--step-form", default="two-launches", choices=["two-launches", "fused"],
-                    help="select + sparse decode as two launches (default, measured faster) or as the one cooperative sparrow_step launch")
     ap.add_argument("--no-per-config", action="store_true", help="cfg4 only: skip the per_config block (cfg2, cfg3, cfg5 single-layer results)")
     ap.add_argument("--rollout", type=int, default=0, metavar="T", help="time a T-step sparse rollout against the dense rollout (SURVEY 8(f)-1)")
     ap.add_argument("--rollout-bucket", type=int, default=512, help="steps per CUDA graph / per row of the rollout table")
@@ -897,7 +886,7 @@ def main():
         line = run_single(args, args.workload, rank, local_rank, world, dev)
     else:
         line = run_cfg4(args, rank, local_rank, world, dev)
-        if not args.no_per_config and args.landmark == "minmax" and args.step_form == "two-launches":
+        if not args.no_per_config and args.landmark == "minmax":
             per = {}
             for cfg in ("cfg2", "cfg3", "cfg5"):
                 r = run_single(args, cfg, rank, local_rank, world, dev, headline=False)

@@ -70,7 +70,7 @@ typedef struct sparrow_shape {
  *           one-vector-per-page landmark that the paper's cost model charges.  mean over the valid
  *           tokens, accumulated in fp32, rounded once to bf16: the stored code is the exactly rounded mean or, where the
  *           exact mean lies within the fp32 accumulation error of a rounding boundary, the neighbouring code (R24).
- * Everything else (budget, forced pages, top-k, attention) is the same.  sparrow_step uses the two launches for MEAN. */
+ * Everything else (budget, forced pages, top-k, attention) is the same. */
 enum { SPARROW_LANDMARK_MINMAX = 0, SPARROW_LANDMARK_MEAN = 1 };
 
 /* Dynamic sparsity schedule B(L) in EXACT integer arithmetic (R3), so that host, device and any checker
@@ -131,7 +131,9 @@ int sparrow_select(const void *q, const void *summaries, const int32_t *page_tab
  * workspace: sparrow_decode_workspace_bytes(shape, max_sel) bytes, ZERO-INITIALISED once by the caller (it
  * holds the split-K arrival counters; the kernel restores the zeros it uses, so it can be reused call
  * after call, but not by two calls in flight at the same time).  n_seq <= 8192.  The merge of the splits
- * is fused into the same launch (one kernel per call). */
+ * is fused into the same launch (one kernel per call).  The K/V tiles are fetched by TMA: each call encodes
+ * two tensor maps over the pools on the host (cuTensorMapEncodeTiled, a few microseconds) and passes them by value,
+ * so the call stays asynchronous and graph-capturable; the result is bit-for-bit reproducible from call to call. */
 int sparrow_sparse_decode(const void *q, const void *k_cache, const void *v_cache, const int32_t *page_table,
                           const int32_t *seq_lens, const int32_t *sel_pages, int32_t max_sel,
                           const int32_t *sel_count, void *out, float *lse, float sm_scale,
@@ -149,27 +151,10 @@ int sparrow_dense_decode(const void *q, const void *k_cache, const void *v_cache
  * bf16) are written at token position L (logical page L/16 through page_table, row L%16), seq_lens[i] becomes
  * L + 1, and if the token fills its page (L%16 == 15) that page's min/max summary is (re)computed in the same
  * launch -- a1 "on page fill".  A sequence whose page table has no room (L/16 >= max_pages_per_seq) is left
- * untouched.  The caller then runs sparrow_select / sparrow_sparse_decode (or sparrow_step) with the new lengths;
+ * untouched.  The caller then runs sparrow_select / sparrow_sparse_decode with the new lengths;
  * a partially filled last page needs no summary because it is always kept (R9). */
 int sparrow_append(const void *k_new, const void *v_new, void *k_cache, void *v_cache, void *summaries,
                    const int32_t *page_table, int32_t *seq_lens, const sparrow_shape_t *shape, void *stream);
-
-/* ---- a2..a7 fused: the whole sparse step in ONE persistent launch ----------------------------------
- * Same results as sparrow_select followed by sparrow_sparse_decode on the same arguments (the selected lists
- * and sel_count are written too), but the summary stream, the per-unit top-k and the K/V stream share one
- * cooperative launch: every warp moves from scoring to decoding as soon as its share is done, and a decode
- * look-up waits only for the one (sequence, kv-head) list it needs.  Falls back to the two launches when the
- * shape does not fit the fused kernel's shared memory (roughly n_seq + max_pages_per_seq/2 > 12000) or the device
- * cannot keep 148 CTAs resident.  sched->kind == DENSE is allowed (identity lists).  Measured on B200 this form is
- * not yet faster than the two calls: it is the opt-in single-launch form.  workspace:
- * sparrow_step_workspace_bytes(shape, max_sel) bytes, ZERO-INITIALISED once by the caller, restored to zero by
- * the call like the other workspaces; not shareable by two calls in flight. */
-int sparrow_step(const void *q, const void *k_cache, const void *v_cache, const void *summaries,
-                 const int32_t *page_table, const int32_t *seq_lens, const sparrow_schedule_t *sched,
-                 int32_t *sel_pages, int32_t max_sel, int32_t *sel_count, float *scores_dbg,
-                 void *out, float *lse, float sm_scale, void *workspace, size_t workspace_bytes,
-                 const sparrow_shape_t *shape, void *stream);
-size_t sparrow_step_workspace_bytes(const sparrow_shape_t *shape, int32_t max_sel);
 
 /* ---- whole step through HOST buffers (the end-to-end measurement path) ----------------------------
  * The step's inputs live in ONE host block (pinned memory makes the copy asynchronous) laid out as

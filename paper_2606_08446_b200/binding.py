@@ -76,8 +76,6 @@ _SIGS = {
     "sparrow_sparse_decode": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _i32, _vp, _vp, _vp, _f, _vp, _sz, _SHP, _vp]),
     "sparrow_dense_decode": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _f, _vp, _sz, _SHP, _vp]),
     "sparrow_append": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _SHP, _vp]),
-    "sparrow_step": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _SCH, _vp, _i32, _vp, _vp, _vp, _vp, _f, _vp, _sz, _SHP, _vp]),
-    "sparrow_step_workspace_bytes": (_sz, [_SHP, _i32]),
     "sparrow_step_host": (C.c_int, [_vp, _i64, C.c_int, _vp, _vp, _vp, _vp, _SCH, _i32, _f, _vp, _vp, _sz, _SHP, _vp]),
     "sparrow_step_host_block_bytes": (_sz, [_SHP, C.POINTER(_sz), C.POINTER(_sz), C.POINTER(_sz)]),
     "sparrow_select_workspace_bytes": (_sz, [_SHP]),
@@ -143,10 +141,6 @@ def sparrow_select_workspace_bytes(shape) -> int:
 
 def sparrow_decode_workspace_bytes(shape, max_sel: int) -> int:
     return _lib.sparrow_decode_workspace_bytes(_by(shape), max_sel)
-
-
-def sparrow_step_workspace_bytes(shape, max_sel: int) -> int:
-    return _lib.sparrow_step_workspace_bytes(_by(shape), max_sel)
 
 
 def sparrow_step_scratch_bytes(shape, max_sel: int) -> int:
@@ -239,17 +233,6 @@ def sparrow_append(k_new, v_new, k_cache, v_cache, summaries, page_table, seq_le
                              _ptr(seq_lens), _by(shape), _stream(stream))
     if check:
         _check(rc, "sparrow_append")
-    return rc
-
-
-def sparrow_step(q, k_cache, v_cache, summaries, page_table, seq_lens, sched, sel_pages, max_sel: int, sel_count, scores_dbg,
-                 out, lse, sm_scale: float, workspace, shape, stream=None, *, check=True):
-    rc = _lib.sparrow_step(_ptr(q), _ptr(k_cache), _ptr(v_cache), _ptr(summaries), _ptr(page_table), _ptr(seq_lens), _by(sched),
-                           _ptr(sel_pages), max_sel, _ptr(sel_count), _ptr(scores_dbg), _ptr(out), _ptr(lse), sm_scale,
-                           _ptr(workspace), 0 if workspace is None else workspace.numel() * workspace.element_size(),
-                           _by(shape), _stream(stream))
-    if check:
-        _check(rc, "sparrow_step")
     return rc
 
 

@@ -8,7 +8,6 @@
 #include "common.cuh"
 #include "decode.cuh"
 #include "select.cuh"
-#include "step.cuh"
 #include "summarize.cuh"
 #include "append.cuh"
 #include "accept.cuh"
@@ -27,8 +26,7 @@ constexpr int kNumSmsB200 = 148;
 struct DevState {
     bool init = false;
     int sms = 0;
-    size_t dyn_decode[2] = {0, 0}, dyn_select[2] = {0, 0}, dyn_step = 0, dyn_hist = 0;
-    int fused_ok = -1;           // -1 unknown, 0 the device cannot run the cooperative grid, 1 yes
+    size_t dyn_decode[2] = {0, 0}, dyn_select[2] = {0, 0}, dyn_hist = 0;
 };
 constexpr int kMaxDevices = 64;
 DevState g_dev[kMaxDevices];
@@ -166,23 +164,57 @@ int to_dev_sched(const sparrow_schedule_t *in, SchedDev *out, int page_tokens = 
     return SPARROW_OK;
 }
 
-// Decode workspace: arrival counters (one per (sequence, kv-head) unit) + the two counters of the range scheduler
-// (all zero between calls), then the fp32 partial slots (indexed unit + range index) and their (m, l) pairs.
+// Decode workspace: arrival counters (one per (sequence, kv-head) unit, all zero between calls), then the fp32 partial
+// slots of the CTAs (indexed unit + CTA index) and their (m, l) pairs.
 struct DecodeGeom {
     size_t bytes_o, bytes_ml, bytes_ctr;
-    int max_rounds;
 };
-DecodeGeom decode_geom(const sparrow_shape_t *s, int32_t max_sel /* 0 = dense */)
+DecodeGeom decode_geom(const sparrow_shape_t *s)
 {
     DecodeGeom gm;
     const size_t units = (size_t)s->n_seq * s->n_kv_heads;
-    const int64_t max_cnt = (max_sel > 0 && max_sel < s->max_pages_per_seq) ? max_sel : s->max_pages_per_seq;
-    gm.max_rounds = decode_max_rounds((int64_t)units * max_cnt * (s->page_size / kPage));
-    const size_t rows = (units + (size_t)kDecW * gm.max_rounds) * (s->n_q_heads / s->n_kv_heads);
+    const size_t rows = (units + (size_t)kDecGrid) * (s->n_q_heads / s->n_kv_heads);
     gm.bytes_o = (rows * kDim * sizeof(float) + 255) & ~(size_t)255;
     gm.bytes_ml = (rows * 2 * sizeof(float) + 255) & ~(size_t)255;
     gm.bytes_ctr = ((units + 2) * sizeof(int32_t) + 255) & ~(size_t)255;
     return gm;
+}
+
+// TMA view of a K or V pool: a 2-D bf16 tensor [rows = pages x kv-heads x page tokens][128 dims], row pitch 256 B, read in
+// boxes of 16 rows x 64 columns (128 B wide: SWIZZLE_128B).  The encoder is a driver entry point (no link against libcuda).
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+int make_pool_map(CUtensorMap *tm, const void *pool, const sparrow_shape_t *s)
+{
+    static EncodeTiledFn encode = nullptr;
+    static std::mutex m;
+    {
+        std::lock_guard<std::mutex> lock(m);
+        if (!encode) {
+            void *fn = nullptr;
+            cudaDriverEntryPointQueryResult qres;
+            cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+            if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !fn) {
+                snprintf(g_errbuf, sizeof(g_errbuf), "cuTensorMapEncodeTiled is not available from this driver");
+                return SPARROW_ERR_CUDA;
+            }
+            encode = reinterpret_cast<EncodeTiledFn>(fn);
+        }
+    }
+    const cuuint64_t rows = (cuuint64_t)s->n_phys_pages * s->n_kv_heads * s->page_size;
+    const cuuint64_t gdim[2] = {(cuuint64_t)kDim, rows};
+    const cuuint64_t gstride[1] = {(cuuint64_t)kDim * 2};
+    const cuuint32_t box[2] = {64, (cuuint32_t)kPage};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult rc = encode(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void *>(pool), gdim, gstride, box, estr,
+                               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (rc != CUDA_SUCCESS) {
+        snprintf(g_errbuf, sizeof(g_errbuf), "cuTensorMapEncodeTiled failed (CUresult %d)", (int)rc);
+        return SPARROW_ERR_CUDA;
+    }
+    return SPARROW_OK;
 }
 
 size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -193,38 +225,40 @@ int launch_decode(const void *q, const void *k_cache, const void *v_cache, const
                   void *out, float *lse, float sm_scale, void *workspace, size_t workspace_bytes,
                   const sparrow_shape_t *s, cudaStream_t st)
 {
-    const DecodeGeom gm = decode_geom(s, kDense ? 0 : max_sel);
+    const DecodeGeom gm = decode_geom(s);
     if (workspace_bytes < gm.bytes_ctr + gm.bytes_o + gm.bytes_ml) return SPARROW_ERR_WORKSPACE_TOO_SMALL;
     if (s->n_seq > kDecMaxSeq) return SPARROW_ERR_UNSUPPORTED;
-    {   // flat tile positions are 32-bit
+    {   // flat tile positions and TMA row coordinates are 32-bit
         const int64_t max_cnt = kDense ? s->max_pages_per_seq : (max_sel < s->max_pages_per_seq ? max_sel : s->max_pages_per_seq);
         const int64_t tpp = s->page_size / kPage;
-        if ((int64_t)s->n_seq * max_cnt * s->n_kv_heads * tpp >= (1LL << 31) || s->n_phys_pages * s->n_kv_heads * tpp >= (1LL << 31))
+        if ((int64_t)s->n_seq * max_cnt * s->n_kv_heads * tpp >= (1LL << 31) || s->n_phys_pages * s->n_kv_heads * tpp >= (1LL << 27))
             return SPARROW_ERR_UNSUPPORTED;
     }
-    if (s->n_seq == 0) return SPARROW_OK;
+    if (s->n_seq == 0 || s->n_phys_pages == 0) return SPARROW_OK;
     int32_t *counters = reinterpret_cast<int32_t *>(workspace);
     float *ws_o = reinterpret_cast<float *>(reinterpret_cast<uint8_t *>(workspace) + gm.bytes_ctr);
     float *ws_ml = reinterpret_cast<float *>(reinterpret_cast<uint8_t *>(workspace) + gm.bytes_ctr + gm.bytes_o);
 
-    constexpr int kSmemMax = kDecRingBytes + ((kDecMaxSeq + 1) * 4 + 15) / 16 * 16;
+    constexpr int kSmemFixed = kDecRingBytes + kDecParkBytes + kDecMetaBytes;
+    constexpr int kSmemMax = kSmemFixed + ((kDecMaxSeq + 1) * 4 + 15) / 16 * 16;
     int rc_dev = SPARROW_OK;
     DevState *ds = dev_state(&rc_dev);
     if (!ds) return rc_dev;
     rc_dev = ensure_dyn_smem(decode_kernel<kDense>, kSmemMax, &ds->dyn_decode[kDense], "decode_kernel");
     if (rc_dev) return rc_dev;
-    const float scale_log2 = sm_scale * 1.4426950408889634f;
-    const int smem = kDecRingBytes + ((s->n_seq + 1) * 4 + 15) / 16 * 16;
+    CUtensorMap tm_k, tm_v;
+    if ((rc_dev = make_pool_map(&tm_k, k_cache, s)) != SPARROW_OK) return rc_dev;
+    if ((rc_dev = make_pool_map(&tm_v, v_cache, s)) != SPARROW_OK) return rc_dev;
+    const int smem = kSmemFixed + ((s->n_seq + 1) * 4 + 15) / 16 * 16;
     DecodeArgs A;
-    A.q = (const uint16_t *)q; A.k_cache = (const uint16_t *)k_cache; A.v_cache = (const uint16_t *)v_cache;
+    A.q = (const uint16_t *)q;
     A.page_table = page_table; A.seq_lens = seq_lens; A.sel_pages = sel_pages; A.sel_count = sel_count;
     A.max_sel = max_sel; A.ws_o = ws_o; A.ws_ml = ws_ml; A.counters = counters;
-    A.sched_ctr = counters + (size_t)s->n_seq * s->n_kv_heads;
-    A.out = (uint16_t *)out; A.lse = lse; A.scale_log2 = scale_log2;
+    A.out = (uint16_t *)out; A.lse = lse; A.scale_log2 = sm_scale * 1.4426950408889634f;
     A.n_seq = s->n_seq; A.n_q_heads = s->n_q_heads; A.n_kv_heads = s->n_kv_heads; A.max_pages = s->max_pages_per_seq;
-    A.ready = nullptr;
     A.tpp_log2 = s->page_size == 16 ? 0 : (s->page_size == 32 ? 1 : (s->page_size == 64 ? 2 : 3));
-    launch_chain(decode_kernel<kDense>, dim3(kDecGrid), dim3(kDecThreads), smem, st, A, gm.max_rounds);
+    const int grid = ds->sms < kDecGrid ? ds->sms : kDecGrid;   // one CTA per SM (the partial slots are sized for 148)
+    launch_chain(decode_kernel<kDense>, dim3(grid), dim3(kDecThreads), smem, st, A, tm_k, tm_v);
     SPARROW_CHECK_LAUNCH("decode_kernel");
     return SPARROW_OK;
 }
@@ -291,94 +325,6 @@ int select_impl(const void *q, const void *summaries, const int32_t *page_table,
     return SPARROW_OK;
 }
 
-// Workspace of the fused step: select workspace (unit counters + scores) | unit flags | decode workspace.
-struct StepGeom {
-    size_t sel_bytes, flag_bytes, dec_bytes;
-};
-StepGeom step_geom(const sparrow_shape_t *s, int32_t max_sel)
-{
-    StepGeom g;
-    const size_t units = (size_t)s->n_seq * s->n_kv_heads;
-    const size_t stride = ((size_t)s->max_pages_per_seq + 31) & ~(size_t)31;     // score rows own their 128-byte lines
-    g.sel_bytes = align256(units * sizeof(int32_t)) + align256(units * stride * sizeof(float));   // >= the select workspace
-    g.flag_bytes = align256((size_t)s->n_seq * s->n_kv_heads * sizeof(int32_t));
-    g.dec_bytes = sparrow_decode_workspace_bytes(s, max_sel);
-    return g;
-}
-
-// a2-a7 in one cooperative launch (step.cuh); falls back to the select and decode launches when the shape does not
-// fit the fused kernel's shared memory or the device cannot hold the grid (still the same CUDA path, two kernels).
-int step_impl(const void *q, const void *k_cache, const void *v_cache, const void *summaries, const int32_t *page_table,
-              const int32_t *seq_lens, const SchedDev &sd, int32_t *sel_pages, int32_t max_sel, int32_t *sel_count,
-              float *scores_dbg, void *out, float *lse, float sm_scale, void *workspace, size_t workspace_bytes,
-              const sparrow_shape_t *s, cudaStream_t st)
-{
-    const StepGeom g = step_geom(s, max_sel);
-    if (workspace_bytes < g.sel_bytes + g.flag_bytes + g.dec_bytes) return SPARROW_ERR_WORKSPACE_TOO_SMALL;
-    if (s->n_seq == 0) return SPARROW_OK;
-    uint8_t *base = reinterpret_cast<uint8_t *>(workspace);
-    uint8_t *sel_ws = base, *flags = base + g.sel_bytes, *dec_ws = flags + g.flag_bytes;
-    const size_t units = (size_t)s->n_seq * s->n_kv_heads;
-    // shared memory: K/V ring | two prefix tables | top-k scratch (one per warp when that fits, else one per CTA)
-    const size_t dyn_base = (size_t)kDecRingBytes + ((2 * (size_t)(s->n_seq + 1) * 4 + 15) & ~(size_t)15);
-    const size_t keys = ((size_t)s->max_pages_per_seq + 31) & ~(size_t)31;
-    constexpr size_t kSmemBudget = 227 * 1024 - 12 * 1024;          // static shared memory and alignment slack
-    const bool per_warp = dyn_base + kDecWarps * keys * 4 <= kSmemBudget;
-    const size_t dyn = dyn_base + (per_warp ? kDecWarps : 1) * keys * 4;
-    int rc_dev = SPARROW_OK;
-    DevState *ds = dev_state(&rc_dev);
-    if (!ds) return rc_dev;
-    bool fused = ds->fused_ok != 0 && s->page_size == kPage && s->landmark == SPARROW_LANDMARK_MINMAX && dyn <= kSmemBudget && s->n_seq <= kDecMaxSeq &&
-                 s->n_phys_pages * s->n_kv_heads < (1LL << 27) &&
-                 (int64_t)s->n_seq * s->max_pages_per_seq * s->n_kv_heads < (1LL << 31);
-    if (fused && ds->fused_ok < 0) {
-        int dev = 0, coop = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
-        ds->fused_ok = (coop && ds->sms >= kDecGrid) ? 1 : 0;
-        fused = ds->fused_ok == 1;
-    }
-    if (fused) {
-        rc_dev = ensure_dyn_smem(step_kernel, dyn, &ds->dyn_step, "step_kernel");
-        if (rc_dev) return rc_dev;
-        const DecodeGeom gm = decode_geom(s, max_sel);
-        StepArgs S;
-        DecodeArgs &A = S.dec;
-        A.q = (const uint16_t *)q; A.k_cache = (const uint16_t *)k_cache; A.v_cache = (const uint16_t *)v_cache;
-        A.page_table = page_table; A.seq_lens = seq_lens; A.sel_pages = sel_pages; A.sel_count = sel_count;
-        A.max_sel = max_sel;
-        A.counters = reinterpret_cast<int32_t *>(dec_ws);
-        A.sched_ctr = A.counters + units;
-        A.ws_o = reinterpret_cast<float *>(dec_ws + gm.bytes_ctr);
-        A.ws_ml = reinterpret_cast<float *>(dec_ws + gm.bytes_ctr + gm.bytes_o);
-        A.out = (uint16_t *)out; A.lse = lse; A.scale_log2 = sm_scale * 1.4426950408889634f;
-        A.n_seq = s->n_seq; A.n_q_heads = s->n_q_heads; A.n_kv_heads = s->n_kv_heads; A.max_pages = s->max_pages_per_seq;
-        A.ready = reinterpret_cast<const int32_t *>(flags);
-        A.tpp_log2 = 0;
-        S.summaries = (const uint16_t *)summaries;
-        S.sel_pages = sel_pages; S.sel_count = sel_count;
-        S.sel_counters = reinterpret_cast<int32_t *>(sel_ws);
-        S.scores_ws = reinterpret_cast<float *>(sel_ws + align256(units * sizeof(int32_t)));
-        S.ws_stride = (int)(((size_t)s->max_pages_per_seq + 31) & ~(size_t)31);
-        S.scores_dbg = scores_dbg;
-        S.ready = reinterpret_cast<int32_t *>(flags);
-        S.max_rounds = gm.max_rounds;
-        S.scratch_stride = per_warp ? (int)keys : 0;
-        SchedDev sd_copy = sd;
-        void *args[] = {&S, &sd_copy};
-        cudaError_t e = cudaLaunchCooperativeKernel((const void *)step_kernel, dim3(kDecGrid), dim3(kDecThreads), args, dyn, st);
-        if (e == cudaSuccess) { ++g_launches; return SPARROW_OK; }
-        if (e != cudaErrorCooperativeLaunchTooLarge) return cuda_fail(e, "step_kernel");
-        (void)cudaGetLastError();
-        ds->fused_ok = 0;                        // the grid cannot be co-resident here: two launches from now on
-    }
-    int rc = select_impl(q, summaries, page_table, seq_lens, sd, sel_pages, max_sel, sel_count, scores_dbg, sel_ws,
-                         g.sel_bytes, s, st);
-    if (rc) return rc;
-    return launch_decode<false>(q, k_cache, v_cache, page_table, seq_lens, sel_pages, max_sel, sel_count, out, lse, sm_scale,
-                                dec_ws, g.dec_bytes, s, st);
-}
-
 }  // namespace
 
 extern "C" {
@@ -408,7 +354,8 @@ size_t sparrow_select_workspace_bytes(const sparrow_shape_t *s)
 size_t sparrow_decode_workspace_bytes(const sparrow_shape_t *s, int32_t max_sel)
 {
     if (check_shape(s) != SPARROW_OK) return 0;
-    const DecodeGeom gm = decode_geom(s, max_sel);
+    (void)max_sel;
+    const DecodeGeom gm = decode_geom(s);
     return gm.bytes_ctr + gm.bytes_o + gm.bytes_ml;
 }
 
@@ -607,38 +554,9 @@ int sparrow_acceptance(const int32_t *ids_p, const float *logp_p, const int32_t 
     return SPARROW_OK;
 }
 
-size_t sparrow_step_workspace_bytes(const sparrow_shape_t *s, int32_t max_sel)
-{
-    if (check_shape(s) != SPARROW_OK || max_sel <= 0) return 0;
-    const StepGeom g = step_geom(s, max_sel);
-    return g.sel_bytes + g.flag_bytes + g.dec_bytes;
-}
-
-int sparrow_step(const void *q, const void *k_cache, const void *v_cache, const void *summaries,
-                 const int32_t *page_table, const int32_t *seq_lens, const sparrow_schedule_t *sched,
-                 int32_t *sel_pages, int32_t max_sel, int32_t *sel_count, float *scores_dbg, void *out, float *lse,
-                 float sm_scale, void *workspace, size_t workspace_bytes, const sparrow_shape_t *shape, void *stream)
-{
-    g_launches = 0;
-    int rc = check_shape(shape);
-    if (rc) return rc;
-    SchedDev sd;
-    rc = to_dev_sched(sched, &sd, shape->page_size);
-    if (rc) return rc;
-    if (!q || !k_cache || !v_cache || !summaries || !page_table || !seq_lens || !sel_pages || !sel_count || !out ||
-        !workspace || max_sel <= 0)
-        return SPARROW_ERR_INVALID_ARG;
-    if (!aligned16(q) || !aligned16(k_cache) || !aligned16(v_cache) || !aligned16(summaries) || !aligned16(out) ||
-        !aligned16(workspace))
-        return SPARROW_ERR_INVALID_ARG;
-    if (shape->max_pages_per_seq > kSelMaxPages) return SPARROW_ERR_UNSUPPORTED;
-    return step_impl(q, k_cache, v_cache, summaries, page_table, seq_lens, sd, sel_pages, max_sel, sel_count, scores_dbg,
-                     out, lse, sm_scale, workspace, workspace_bytes, shape, (cudaStream_t)stream);
-}
-
 // Device scratch of the host-buffer step, carved in this order (each 256-byte aligned):
 //   q | seq_lens | page_ids | n_valid   (the image of the caller's pinned host block: ONE H2D copy brings it over)
-//   | sel_pages | sel_count | out | select + decode workspace | dense decode workspace
+//   | sel_pages | sel_count | out | select workspace | decode workspace
 namespace {
 struct StepCarve {
     size_t q, lens, ids, nval, in_end, sel, cnt, out, sel_ws, dec_ws, total;
@@ -657,9 +575,9 @@ StepCarve step_carve(const sparrow_shape_t *s, int32_t max_sel)
     c.sel = o; o += align256(n * s->n_kv_heads * (size_t)(max_sel > 0 ? max_sel : 1) * 4);
     c.cnt = o; o += align256(n * 4);
     c.out = o; o += align256(n * s->n_q_heads * kDim * 2);
-    c.sel_ws_bytes = sparrow_step_workspace_bytes(s, max_sel > 0 ? max_sel : 1);
+    c.sel_ws_bytes = align256(sparrow_select_workspace_bytes(s));
     c.sel_ws = o; o += c.sel_ws_bytes;
-    c.dec_ws_bytes = sparrow_decode_workspace_bytes(s, 0);
+    c.dec_ws_bytes = sparrow_decode_workspace_bytes(s, 0);       // one decode workspace serves the sparse and the dense call
     c.dec_ws = o; o += c.dec_ws_bytes;
     c.total = o;
     return c;
@@ -717,15 +635,12 @@ int sparrow_step_host(const void *in_block_host, int64_t n_update, int has_n_val
         rc = launch_decode<true>(base + c.q, k_cache, v_cache, page_table, lens_d, nullptr, 0, nullptr, base + c.out, nullptr,
                                  sm_scale, base + c.dec_ws, c.dec_ws_bytes, s, st);
     } else {
-        // two launches: measured faster than the fused step kernel on every configuration
-        uint8_t *ws = base + c.sel_ws;
-        const StepGeom g = step_geom(s, max_sel);
         rc = select_impl(base + c.q, summaries, page_table, lens_d, sd, reinterpret_cast<int32_t *>(base + c.sel), max_sel,
-                         reinterpret_cast<int32_t *>(base + c.cnt), nullptr, ws, g.sel_bytes, s, st);
+                         reinterpret_cast<int32_t *>(base + c.cnt), nullptr, base + c.sel_ws, c.sel_ws_bytes, s, st);
         if (rc) return rc;
         rc = launch_decode<false>(base + c.q, k_cache, v_cache, page_table, lens_d, reinterpret_cast<int32_t *>(base + c.sel),
                                   max_sel, reinterpret_cast<int32_t *>(base + c.cnt), base + c.out, nullptr, sm_scale,
-                                  ws + g.sel_bytes + g.flag_bytes, g.dec_bytes, s, st);
+                                  base + c.dec_ws, c.dec_ws_bytes, s, st);
     }
     if (rc) return rc;
     if ((e = cudaMemcpyAsync(out_host, base + c.out, qbytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e, "D2H out");

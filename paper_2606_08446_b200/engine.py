@@ -43,7 +43,6 @@ class SparrowEngine:
         self.max_sel = max(1, B.sparrow_max_sel_pages(self.sched, max_len))
         self.sel_pages = torch.full((self.wl.n_seq, self.wl.Hkv, self.max_sel), -1, dtype=torch.int32, device=dev)
         self.sparse_ws = torch.zeros((B.sparrow_decode_workspace_bytes(self.shape, self.max_sel),), dtype=torch.uint8, device=dev)
-        self.step_ws = torch.zeros((B.sparrow_step_workspace_bytes(self.shape, self.max_sel),), dtype=torch.uint8, device=dev)
 
     # ---- a1
     def summarize(self, page_ids: Optional[torch.Tensor], n_valid: Optional[torch.Tensor], n_update: Optional[int] = None, stream=None):
@@ -106,7 +105,6 @@ class SparrowEngine:
         self.max_sel = max(1, B.sparrow_max_sel_pages(self.sched, max_len))
         self.sel_pages = torch.full((self.wl.n_seq, self.wl.Hkv, self.max_sel), -1, dtype=torch.int32, device=dev)
         self.sparse_ws = torch.zeros((B.sparrow_decode_workspace_bytes(self.shape, self.max_sel),), dtype=torch.uint8, device=dev)
-        self.step_ws = torch.zeros((B.sparrow_step_workspace_bytes(self.shape, self.max_sel),), dtype=torch.uint8, device=dev)
 
     def rollout(self, q_steps, k_steps, v_steps, out_steps, lse_steps=None, dense=False, stream=None):
         """T decode steps back to back on one stream (capturable as ONE CUDA graph: the lengths live on the device
@@ -121,21 +119,10 @@ class SparrowEngine:
                 self.sparse_decode(q_steps[t], stream, out=out_steps[t], lse=lse)
         return out_steps
 
-    # ---- a2-a7 in one launch
-    def fused_step(self, q=None, stream=None):
-        wl = self.wl
-        return B.sparrow_step(wl.q if q is None else q, wl.k_cache, wl.v_cache, self.summaries, wl.page_table, wl.seq_lens,
-                              self.sched, self.sel_pages, self.max_sel, self.sel_count, self.scores, self.out, self.lse,
-                              wl.sm_scale, self.step_ws, self.shape, stream)
-
-    def step(self, q=None, updates=None, stream=None, fused=False):
-        """One pass of the hot path: summarize the pages that just filled, then select + sparse decode as two launches
-        (the measured-faster form) or, with fused=True, as the one cooperative launch of sparrow_step."""
+    def step(self, q=None, updates=None, stream=None):
+        """One pass of the hot path: summarize the pages that just filled, then select and sparse decode."""
         if updates is not None and updates[0].numel() > 0:
             self.summarize(updates[0], updates[1], stream=stream)
-        if fused:
-            self.fused_step(q, stream)
-        else:
-            self.select(q, stream)
-            self.sparse_decode(q, stream)
+        self.select(q, stream)
+        self.sparse_decode(q, stream)
         return self.out

@@ -22,18 +22,12 @@ def _engine(wl, **kw):
     return eng
 
 
-def _run_sparse(wl, fused=False, **kw):
+def _run_sparse(wl, **kw):
     eng = _engine(wl, **kw)
-    if fused:
-        eng.fused_step()
-    else:
-        eng.select()
-        eng.sparse_decode()
+    eng.select()
+    eng.sparse_decode()
     torch.cuda.synchronize()
     return eng
-
-
-FUSED = False      # the default form of the step is sparrow_select + sparrow_sparse_decode (measured faster)
 
 
 def test_library_loaded_is_in_tree():
@@ -47,20 +41,6 @@ def test_cfg1_sparse_matches_oracle():
     st = check_sparse_step(eng, wl)
     assert eng.sel_count.tolist() == [16, 16]
     assert st["units"] == 4
-
-
-@pytest.mark.parametrize("case", ["cfg1", "ragged"])
-def test_fused_step_form_smoke(case):
-    """sparrow_step (the opt-in one-launch form of a2-a7; not a SURVEY.md 8 row, slower than the two launches on every
-    config) stays parity-green on one tiny and one ragged case."""
-    if case == "cfg1":
-        wl = W.make_config("cfg1", device=DEV)
-    else:
-        lens = [1, 15, 16, 17, 33, 250, 256, 257, 1000, 2049, 4099]
-        wl = W.make_workload(n_seq=len(lens), Hq=8, Hkv=2, lengths=("list", lens), schedule=W._sched("fixed", 16, 64, fixed_tokens=200),
-                             seed=802, device=DEV, poison_tail=True, plant=True)
-    eng = _run_sparse(wl, fused=True, want_scores=True)
-    check_sparse_step(eng, wl)
 
 
 def test_cfg1_budget_covers_context_equals_dense():
@@ -264,7 +244,7 @@ def test_page_size_variants_match_oracle(page, Hq, Hkv):
     sched = W._sched("fixed", 16, 64, fixed_tokens=1024)          # Table 4's budget 1024: 32-32, 64-16, 128-8
     wl = W.make_workload(n_seq=len(lens), Hq=Hq, Hkv=Hkv, lengths=("list", lens), schedule=sched, seed=page + Hq, device=DEV,
                          poison_tail=True, plant=True, page_size=page)
-    eng = _run_sparse(wl, want_scores=True)                        # sparrow_step falls back to the two launches here
+    eng = _run_sparse(wl, want_scores=True)
     st = check_sparse_step(eng, wl)
     assert eng.sel_count.cpu().tolist() == [min(-(-L // page), max(1024 // page, len(set([0]) | set(range(max(L - 64, 0) // page, -(-L // page)))))) for L in lens]
     eng.dense_decode()
@@ -319,7 +299,7 @@ def test_mean_landmark_matches_oracle(Hq, Hkv, page):
     sched = W._sched("fixed", 16, 64, fixed_tokens=320)
     wl = W.make_workload(n_seq=len(lens), Hq=Hq, Hkv=Hkv, lengths=("list", lens), schedule=sched, seed=Hq * 10 + page, device=DEV,
                          poison_tail=True, plant=True, page_size=page)
-    eng = _run_sparse(wl, want_scores=True, landmark="mean")       # sparrow_step takes the two launches for this landmark
+    eng = _run_sparse(wl, want_scores=True, landmark="mean")
     assert eng.summaries.shape == (wl.n_phys, Hkv, 128)
     check_sparse_step(eng, wl)
 

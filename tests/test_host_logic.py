@@ -37,7 +37,9 @@ def test_built_for_sm100a_with_tensor_and_async_copy_instructions(B):
     import subprocess
     sass = subprocess.run(["cuobjdump", "-sass", B.LIB_PATH], capture_output=True, text=True).stdout
     assert "sm_100a" in sass
-    assert "HMMA" in sass and "LDSM" in sass and "LDGSTS" in sass
+    # tensor-core products (mma.sync -> HMMA, operands via ldmatrix -> LDSM) and the TMA K/V ring of the decode kernel
+    # (cp.async.bulk.tensor -> UTMALDG, mbarrier -> SYNCS)
+    assert "HMMA" in sass and "LDSM" in sass and "UTMALDG" in sass and "SYNCS" in sass
 
 
 def _golden():
