@@ -202,10 +202,10 @@ int make_pool_map(CUtensorMap *tm, const void *pool, const sparrow_shape_t *s)
             encode = reinterpret_cast<EncodeTiledFn>(fn);
         }
     }
-    const cuuint64_t rows = (cuuint64_t)s->n_phys_pages * s->n_kv_heads * s->page_size;
-    const cuuint64_t gdim[2] = {(cuuint64_t)kDim, rows};
-    const cuuint64_t gstride[1] = {(cuuint64_t)kDim * 2};
-    const cuuint32_t box[2] = {64, (cuuint32_t)kPage};
+    const cuuint64_t rows = (cuuint64_t)s->n_phys_pages * s->n_kv_heads * s->page_size * 2;     // 128-byte rows: (token, half)
+    const cuuint64_t gdim[2] = {64, rows};
+    const cuuint64_t gstride[1] = {128};
+    const cuuint32_t box[2] = {64, (cuuint32_t)(2 * kPage)};
     const cuuint32_t estr[2] = {1, 1};
     const CUresult rc = encode(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void *>(pool), gdim, gstride, box, estr,
                                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -239,7 +239,7 @@ int launch_decode(const void *q, const void *k_cache, const void *v_cache, const
     float *ws_o = reinterpret_cast<float *>(reinterpret_cast<uint8_t *>(workspace) + gm.bytes_ctr);
     float *ws_ml = reinterpret_cast<float *>(reinterpret_cast<uint8_t *>(workspace) + gm.bytes_ctr + gm.bytes_o);
 
-    constexpr int kSmemFixed = kDecRingBytes + kDecParkBytes + kDecMetaBytes;
+    constexpr int kSmemFixed = kDecRingBytes + kDecAccBytes + kDecDescBytes + kDecMetaBytes;
     constexpr int kSmemMax = kSmemFixed + ((kDecMaxSeq + 1) * 4 + 15) / 16 * 16;
     int rc_dev = SPARROW_OK;
     DevState *ds = dev_state(&rc_dev);

@@ -173,9 +173,11 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity)
                  : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
     return ok != 0;
 }
+// (bounded: a protocol bug becomes a trap -- a launch failure the caller sees -- instead of a hung device)
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 {
-    while (!mbar_try_wait(bar, parity)) {}
+    for (uint32_t n = 0; !mbar_try_wait(bar, parity); ++n)
+        if (n > (1u << 26)) __trap();
 }
 // 1-D bulk copy global -> shared (UBLKCP): bytes and both addresses multiples of 16; completes `bytes` on `bar`
 __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar)

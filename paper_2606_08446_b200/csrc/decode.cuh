@@ -41,24 +41,28 @@
 
 namespace sparrow {
 
-constexpr int kDecConsumers = 8;                                // consumer warps; consumer h also merges query head h
-constexpr int kDecThreads = (kDecConsumers + 1) * 32;           // + the producer warp
+constexpr int kDecConsumers = 8;                                // consumer warps
+constexpr int kDecThreads = (kDecConsumers + 1) * 32;           // + the look-up warp
 #ifndef SPARROW_DEC_STAGES
 #define SPARROW_DEC_STAGES 16
 #endif
 constexpr int kDecStages = SPARROW_DEC_STAGES;                  // CTA-wide ring depth (tiles in flight per SM)
 constexpr int kStageBytes = 2 * kTileBytes;                     // K tile + V tile = 8 KiB
 constexpr int kDecRingBytes = kDecStages * kStageBytes;         // 128 KiB
+constexpr int kDecChunk = 2;                                    // tiles per claim (kDecConsumers x kDecChunk = the ring: every consumer's tiles are in flight)
+static_assert(kDecConsumers * kDecChunk == kDecStages, "a claim's tiles must be in the ring when it is taken");
 constexpr int kMaxGroup = 8;                                    // r <= 8 (rows 0..7 of the m16 tile)
-static_assert(kMaxGroup <= kDecConsumers, "consumer h merges query head h");
 #ifndef SPARROW_DEC_MAXSEQ
-#define SPARROW_DEC_MAXSEQ 8192
+#define SPARROW_DEC_MAXSEQ 4096
 #endif
 constexpr int kDecMaxSeq = SPARROW_DEC_MAXSEQ;                  // prefix table of the batch lives in shared memory
 constexpr int kDecGrid = 148;                                   // persistent: one CTA per B200 SM (fewer SMs: fewer CTAs)
-constexpr int kParkRow = kDim + 4;                              // one parked head: o[128] | m | l | pad (16-byte rows)
-constexpr int kDecParkBytes = kDecConsumers * kMaxGroup * kParkRow * 4;
-constexpr int kDecMetaBytes = kDecStages * 4 + 2 * kDecStages * 8 + 64;   // valid counts | full / empty barriers | flag
+constexpr int kAccRow = kDim + 4;                               // one parked head: o[128] | m | l | pad
+constexpr int kAccSlots = 2;                                    // parts (the CTA's share of a unit) being parked at once
+constexpr int kDecAccBytes = kAccSlots * kDecConsumers * kMaxGroup * kAccRow * 4;   // [slot][consumer][head][kAccRow]
+constexpr int kDescRing = 256;                                  // per-tile descriptors the look-up warp runs ahead by
+constexpr int kDecDescBytes = kDescRing * 16;
+constexpr int kDecMetaBytes = kDecStages * 8 + kDecStages * 4 + 3 * kAccSlots * 4 + kDecConsumers * 4 + 64;   // full barriers | issued tile per stage | area generation, tile count, consumer mask | consumer positions | claim, ready
 
 __device__ __forceinline__ void ldsm_x4(uint32_t &r0, uint32_t &r1, uint32_t &r2, uint32_t &r3, uint32_t addr)
 {
@@ -94,18 +98,34 @@ __device__ __forceinline__ float fast_exp2(float x)
 // Swizzled byte offset of 16-byte chunk c (0..15) of token row t inside a 4 KiB tile.
 __device__ __forceinline__ uint32_t tile_off(int t, int c)
 {
-    return (uint32_t)((c >> 3) * 2048 + t * 128 + (((c & 7) ^ (t & 7)) << 4));
+    const int rho = 2 * t + (c >> 3);                    // 128-byte row of the tile: (token, half)
+    return (uint32_t)(rho * 128 + (((c & 7) ^ (rho & 7)) << 4));
 }
 
-// One TMA box: 16 rows x 64 bf16 columns of the [rows][128] view of a K or V pool, starting at (col, row), into 2 KiB of
-// shared memory (SWIZZLE_128B), completing 2048 bytes on `bar`.
+// One TMA box = one 4 KiB tile: 32 rows x 64 bf16 columns of the [128-byte rows][64] view of a K or V pool (row = (token,
+// half of the head dim)), starting at (col, row), into shared memory (SWIZZLE_128B), completing 4096 bytes on `bar`.
 __device__ __forceinline__ void tma_box(uint32_t dst, const CUtensorMap *tm, int col, int row, uint32_t bar)
 {
     asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
                  ::"r"(dst), "l"(reinterpret_cast<uint64_t>(tm)), "r"(col), "r"(row), "r"(bar) : "memory");
 }
-// named barrier of the consumer warps (the producer never joins it)
-__device__ __forceinline__ void consumer_sync() { asm volatile("bar.sync 1, %0;" ::"n"(kDecConsumers * 32) : "memory"); }
+__device__ __forceinline__ int lds_volatile(const int32_t *p)
+{
+    int v;
+    asm volatile("ld.volatile.shared.s32 %0, [%1];" : "=r"(v) : "r"(smem_u32(p)) : "memory");
+    return v;
+}
+// A wait on a shared-memory word that another warp of the CTA will write.  Bounded: a protocol bug becomes a trap (a launch
+// failure the caller sees) instead of a hung device.
+__device__ __forceinline__ void spin_until(const int32_t *p, int want_ge)
+{
+    for (uint32_t n = 0; lds_volatile(p) < want_ge; ++n)
+        if (n > (1u << 27)) __trap();
+}
+__device__ __forceinline__ void sts_volatile(int32_t *p, int v)
+{
+    asm volatile("st.volatile.shared.s32 [%0], %1;" ::"r"(smem_u32(p)), "r"(v) : "memory");
+}
 
 // Everything the decode needs (kernel arguments, passed on unchanged).
 struct DecodeArgs {
@@ -138,12 +158,17 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
 {
     chain_entry();
     extern __shared__ __align__(1024) uint8_t smem[];
-    float *s_park = reinterpret_cast<float *>(smem + kDecRingBytes);                          // [consumer][head][kParkRow]
-    int32_t *s_valid = reinterpret_cast<int32_t *>(smem + kDecRingBytes + kDecParkBytes);     // [stage] valid tokens of the tile
-    uint64_t *s_full = reinterpret_cast<uint64_t *>(s_valid + kDecStages);                    // [stage] tile has landed
-    uint64_t *s_empty = s_full + kDecStages;                                                  // [stage] consumer is done with it
-    int32_t *s_flag = reinterpret_cast<int32_t *>(s_empty + kDecStages);                      // arrival result of the current unit
-    int32_t *s_prefix = reinterpret_cast<int32_t *>(smem + kDecRingBytes + kDecParkBytes + kDecMetaBytes);   // [n_seq + 1] tiles per kv-head before sequence i
+    float *s_acc = reinterpret_cast<float *>(smem + kDecRingBytes);                           // [slot][consumer][head][kAccRow]
+    int4 *s_desc = reinterpret_cast<int4 *>(smem + kDecRingBytes + kDecAccBytes);             // [kDescRing] per-tile descriptors
+    uint64_t *s_full = reinterpret_cast<uint64_t *>(smem + kDecRingBytes + kDecAccBytes + kDecDescBytes);   // [stage] tile has landed
+    int32_t *s_issued = reinterpret_cast<int32_t *>(s_full + kDecStages);                     // [stage] latest tile requested into the stage
+    int32_t *s_gen = s_issued + kDecStages;                                                   // [slot] parts finished on this parking area
+    int32_t *s_count = s_gen + kAccSlots;                                                     // [slot] tiles of the current part parked so far
+    int32_t *s_mask = s_count + kAccSlots;                                                    // [slot] consumers that have parked a state
+    int32_t *s_pos = s_mask + kAccSlots;                                                      // [consumer] first tile of the claim it is working on
+    int32_t *s_claim = s_pos + kDecConsumers;                                                 // chunks claimed by the consumers
+    int32_t *s_ready = s_claim + 1;                                                           // descriptors written by the look-up warp
+    int32_t *s_prefix = reinterpret_cast<int32_t *>(smem + kDecRingBytes + kDecAccBytes + kDecDescBytes + kDecMetaBytes);   // [n_seq + 1]
     __shared__ int s_scan[kDecThreads / 32];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -151,16 +176,18 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
     const int r = A.n_q_heads / n_kv_heads;
     constexpr uint32_t kFull = 0xffffffffu;
     const uint32_t ring_u32 = smem_u32(smem);
-    const uint32_t full_u32 = smem_u32(s_full), empty_u32 = smem_u32(s_empty);
+    const uint32_t full_u32 = smem_u32(s_full);
 
-    // ---- prologue: barriers; list length of every sequence -> exclusive prefix in shared memory ----
+    // ---- prologue: barriers and flags; list length of every sequence -> exclusive prefix in shared memory ----
     if (tid == 0) {
-        for (int s = 0; s < kDecStages; ++s) {
-            mbar_init(full_u32 + 8 * s, 1);              // the producer's arrive.expect_tx; the copies complete the bytes
-            mbar_init(empty_u32 + 8 * s, 1);             // lane 0 of the tile's consumer
-        }
+        for (int s = 0; s < kDecStages; ++s) mbar_init(full_u32 + 8 * s, 1);    // the issuing lane's arrive.expect_tx; the copies complete the bytes
         fence_mbar_init();
+        *s_claim = 0;
+        *s_ready = 0;
     }
+    if (tid < kAccSlots) { s_gen[tid] = 0; s_count[tid] = 0; s_mask[tid] = 0; }
+    if (tid < kDecStages) s_issued[tid] = -1;
+    if (tid < kDecConsumers) s_pos[tid] = 0;
     {
         const int per = (n_seq + kDecThreads - 1) / kDecThreads;
         const int s0 = min(tid * per, n_seq), s1 = min(s0 + per, n_seq);
@@ -195,7 +222,8 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
     cr.per = T / (int)gridDim.x;
     cr.extra = T - cr.per * (int)gridDim.x;
     const int ra = cr.begin(blockIdx.x), rb = cr.begin(blockIdx.x + 1);         // this CTA's tiles [ra, rb)
-    if (ra >= rb) return;
+    const int n_tiles = rb - ra;
+    if (n_tiles <= 0) return;
     // sequence that holds flat tile p: the last one whose first tile is <= p and that is not empty
     auto seq_of = [&](int p) {
         int lo = 0, hi = n_seq - 1;
@@ -208,83 +236,87 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
     };
 
     if (warp == kDecConsumers) {
-        // =========================================================== PRODUCER ===========================================
-        // Look-up of flat tile p -> (sequence, kv-head, list position) -> logical page -> physical tile, as three stages
-        // so that no stage consumes a load issued by the stage before it in the same breath.  A WINDOW is up to 32
-        // consecutive tiles of the CTA's range, lane = tile.
+        // =========================================================== LOOK-UP WARP ===========================================
+        // flat tile p -> (sequence, kv-head, list position) -> logical page -> physical tile, as three stages so that no
+        // stage consumes a load issued by the stage before it in the same breath; a WINDOW is up to 32 consecutive tiles
+        // of the CTA's range, lane = tile.  The result is one 16-byte descriptor per tile in a ring the consumers read:
+        //   x = index of the 4 KiB K (and V) tile in the pools          y = unit (sequence * Hkv + kv-head)
+        //   z = valid tokens (bits 0-4) | part number, counted along the CTA's range (bits 8..)
+        //   w = tiles of the CTA's part of the unit
         struct Lookup {
-            int tile;        // stage C: index of the 4 KiB K (and V) tile in the pools
-            int valid;       // stage B: valid tokens of the tile (0..16)
-            int seq, unit, logical, len, phys, sub;
+            int tile, unit, meta, pos;
+            int seq, logical, len, phys, sub;
         };
+        int part_base = 0;                                       // parts of the range started before the window being looked up
         auto stage_a = [&](Lookup &m, int p, bool on) {
-            m.tile = 0; m.valid = 0; m.seq = -1; m.unit = 0; m.logical = 0; m.len = 0; m.phys = 0; m.sub = 0;
+            bool starts = false;                                 // this tile is the first of a part other than the range's first
+            m.tile = 0; m.unit = 0; m.meta = 0; m.pos = 0; m.seq = -1; m.logical = 0; m.len = 0; m.phys = 0; m.sub = 0;
             if (on) {
                 const int seq = seq_of(p), base = s_prefix[seq], c = s_prefix[seq + 1] - base;
                 const int rem = p - base * n_kv_heads;
                 const int g = rem / c, i = rem - g * c;
+                const int u0 = base * n_kv_heads + g * c;        // the unit is tiles [u0, u0 + c) of the stream
                 m.seq = seq;
                 m.unit = seq * n_kv_heads + g;
+                m.pos = min(u0 + c, rb) - max(u0, ra);
+                starts = i == 0 && p != ra;
                 const int pi = i >> A.tpp_log2;                  // list position of the tile's page
                 m.sub = i - (pi << A.tpp_log2);
                 m.logical = kDense ? pi : __ldg(A.sel_pages + ((int64_t)m.unit) * max_sel + pi);
                 m.len = __ldg(A.seq_lens + seq);
             }
+            // parts are numbered densely along the range (the parking areas are handed out in that order)
+            const uint32_t sm = __ballot_sync(kFull, starts);
+            m.meta = (part_base + __popc(sm & (0xffffffffu >> (31 - lane)))) << 8;
+            part_base += __popc(sm);
         };
         auto stage_b = [&](Lookup &m) {
             if (m.seq >= 0) {
                 m.phys = __ldg(A.page_table + (int64_t)m.seq * max_pages + m.logical);
                 int valid = m.len - ((m.logical << A.tpp_log2) + m.sub) * kPage;
-                m.valid = valid < 0 ? 0 : (valid > kPage ? kPage : valid);
+                m.meta |= valid < 0 ? 0 : (valid > kPage ? kPage : valid);
             }
         };
         auto stage_c = [&](Lookup &m) { m.tile = ((m.phys * n_kv_heads + (m.unit - m.seq * n_kv_heads)) << A.tpp_log2) + m.sub; };
 
-        int rp = ra;                                             // next tile not yet in a window
-        auto open_window = [&](Lookup &m, int &n) {
-            n = min(32, rb - rp);
-            stage_a(m, rp + lane, lane < n);
-            rp += n;
-        };
         Lookup cur, nxt;
-        int cn, nn, nxt_stage;                                   // tiles of the two windows; look-up stages of `nxt` done (1 = A, 2 = B, 3 = C)
-        open_window(cur, cn);
-        if (rp < rb) { open_window(nxt, nn); nxt_stage = 1; } else { nn = 0; nxt_stage = 3; }
+        int w0 = 0;                                              // first tile (CTA-relative) of window `cur`
+        int cn = min(32, n_tiles);
+        stage_a(cur, ra + lane, lane < cn);
+        int nn = min(32, n_tiles - cn);
+        if (nn > 0) stage_a(nxt, ra + cn + lane, lane < nn);
         stage_b(cur);
+        if (nn > 0) stage_b(nxt);
         stage_c(cur);
-        auto advance_nxt = [&](int target) {                     // warp-uniform
-            if (nxt_stage < 2 && target >= 2) { stage_b(nxt); nxt_stage = 2; }
-            if (nxt_stage < 3 && target >= 3) { stage_c(nxt); nxt_stage = 3; }
-        };
-        int it = 0;                                              // tiles issued so far: tile `it` goes to stage it % kDecStages
 #pragma unroll 1
         while (cn > 0) {
-            // look-up stages B and C of the next window run a third and two thirds of the way through this one
-            const int jc = cn >= 24 ? 16 : max(0, min((2 * cn) / 3, cn - 2));
-            const int jb = cn >= 24 ? 8 : min(cn / 3, jc);
-#pragma unroll 1
-            for (int j = 0; j < cn; ++j, ++it) {
-                if (j == jb) advance_nxt(2);
-                if (j == jc) advance_nxt(3);
-                const int stage = it % kDecStages, use = it / kDecStages;
-                const int tile = __shfl_sync(kFull, cur.tile, j), valid = __shfl_sync(kFull, cur.valid, j);
-                if (lane == 0) {
-                    if (use > 0) mbar_wait(empty_u32 + 8 * stage, (use - 1) & 1);      // its previous tile has been consumed
-                    s_valid[stage] = valid;
-                    const uint32_t bar = full_u32 + 8 * stage, dst = ring_u32 + stage * kStageBytes;
-                    mbar_arrive_expect_tx(bar, kStageBytes);     // (release: orders the store of `valid` before the consumer's wait)
-                    const int row = tile * kPage;
-                    tma_box(dst, &tm_k, 0, row, bar);
-                    tma_box(dst + 2048, &tm_k, 64, row, bar);
-                    tma_box(dst + kTileBytes, &tm_v, 0, row, bar);
-                    tma_box(dst + kTileBytes + 2048, &tm_v, 64, row, bar);
-                }
-                __syncwarp();
+            // room in the ring: the entries this window overwrites must be older than every consumer's current claim (a
+            // consumer reads the descriptors of its claim's tiles, and of the tiles one ring further on when it refills
+            // their stages).  The consumers are NOT within a fixed distance of one another: a consumer held up on tile j
+            // blocks only the chain of its own stage (j, j + 16, ...), the others run on until each has picked a chunk on
+            // that stage pair -- up to 7 x 8 claims ahead -- so every consumer publishes where it is.
+            for (uint32_t n = 0;; ++n) {
+                int lo = lane < kDecConsumers ? lds_volatile(s_pos + lane) : 0x7fffffff;
+#pragma unroll
+                for (int of = 4; of > 0; of >>= 1) lo = min(lo, __shfl_xor_sync(kFull, lo, of));
+                lo = __shfl_sync(kFull, lo, 0);
+                if (w0 + 32 - kDescRing <= lo) break;
+                __nanosleep(100);
+                if (n > (1u << 24)) __trap();
             }
-            advance_nxt(3);
+            if (lane < cn) s_desc[(w0 + lane) & (kDescRing - 1)] = make_int4(cur.tile, cur.unit, cur.meta, cur.pos);
+            __threadfence_block();
+            __syncwarp();
+            if (lane == 0) sts_volatile(s_ready, w0 + cn);
+            // next window: its stage C now, and stage A + B of the one after it (their loads complete while the consumers
+            // work through the descriptors just published)
+            w0 += cn;
             cur = nxt; cn = nn;
-            if (cn > 0 && rp < rb) { open_window(nxt, nn); nxt_stage = 1; }
-            else { nn = 0; nxt_stage = 3; }
+            if (cn > 0) {
+                stage_c(cur);
+                nn = min(32, n_tiles - (w0 + cn));
+                if (nn > 0) { stage_a(nxt, ra + w0 + cn + lane, lane < nn); stage_b(nxt); }
+            }
         }
         return;
     }
@@ -294,37 +326,220 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
     const int mat = lane >> 3, rr = lane & 7;
     const float scale_log2 = A.scale_log2;
     constexpr float kLn2 = 0.6931471805599453f;
-    int p = ra;
-    int seq = seq_of(p);
-#pragma unroll 1
-    while (p < rb) {
-        // ---- the CTA's part of one unit: tiles [p, e) of the stream; the unit is tiles [u0, u1) ----
-        const int base = s_prefix[seq], c = s_prefix[seq + 1] - base;
-        const int rem = p - base * n_kv_heads;
-        const int g = rem / c;
-        const int u0 = base * n_kv_heads + g * c, u1 = u0 + c;
-        const int e = min(u1, rb);
-        const int unit = seq * n_kv_heads + g;
-        uint32_t qa[8][2];                                          // Q fragments of the unit
-        {
-            const uint16_t *qrow = A.q + ((int64_t)unit * r + hrow) * kDim + col;
-#pragma unroll
-            for (int kk = 0; kk < 8; ++kk) {
-                qa[kk][0] = hrow < r ? __ldg(reinterpret_cast<const uint32_t *>(qrow + kk * 16)) : 0u;
-                qa[kk][1] = hrow < r ? __ldg(reinterpret_cast<const uint32_t *>(qrow + kk * 16 + 8)) : 0u;
-            }
+
+    // the tile `it` of the range (CTA-relative) goes to stage it % kDecStages; issued by ONE lane
+    auto issue = [&](int it) {
+        spin_until(s_ready, it + 1);                                // its descriptor has been written
+        __threadfence_block();
+        const int tile = s_desc[it & (kDescRing - 1)].x;
+        const int stage = it % kDecStages;
+        const uint32_t bar = full_u32 + 8 * stage, dst = ring_u32 + stage * kStageBytes;
+        sts_volatile(s_issued + stage, it);
+        mbar_arrive_expect_tx(bar, kStageBytes);
+        const int row = tile * 2 * kPage;
+        tma_box(dst, &tm_k, 0, row, bar);
+        tma_box(dst + kTileBytes, &tm_v, 0, row, bar);
+    };
+    if (lane == 0) {                                                // first fill of the ring: consumer w issues tiles w, w + 8
+        for (int k = 0; k < kDecChunk; ++k) {
+            const int it = warp + k * kDecConsumers;
+            if (it < n_tiles) issue(it);
         }
-        float o[16][2];                 // O[head = lane/4][dims nt*8 + col + {0,1}]
+    }
+
+    uint32_t qa[8][2];                                              // Q fragments of the unit this consumer is in
+    int q_unit = -1;
+    float o[16][2];                 // O[head = lane/4][dims nt*8 + col + {0,1}] of the piece being computed
+    float m_run = -INFINITY, l_run = 0.f;
+
+    // PARK: this consumer is done with a part (it has been handed a tile of another one, or the range is exhausted).
+    // Its state goes to the part's parking area; the consumer whose tiles complete the part merges the parked states
+    // in consumer order and writes the result.  WHICH tiles a consumer took is decided at run time (whoever is free
+    // takes the next chunk), so the fp32 summation order -- the last bits of the result -- can differ from run to run.
+    auto park = [&](int part, int unit, int n_mine, int part_len) {
+        const int slot = part & (kAccSlots - 1);
+        // The parking areas are handed out strictly in part order (part P gets area P mod 2 once part P - 2 is finished):
+        // a later part can then never hold an area an earlier part is waiting for, and the earliest unfinished part --
+        // whose tiles have all been consumed -- can always complete.
+        if (lane == 0) {
+            spin_until(s_gen + slot, part / kAccSlots);
+            __threadfence_block();
+        }
+        __syncwarp();
+        float l_tot = l_run;
+        l_tot += __shfl_xor_sync(kFull, l_tot, 1);
+        l_tot += __shfl_xor_sync(kFull, l_tot, 2);
+        float *area = s_acc + slot * (kDecConsumers * kMaxGroup * kAccRow);
+        if (hrow < r) {
+            float *row = area + (warp * kMaxGroup + hrow) * kAccRow;
+#pragma unroll
+            for (int nt = 0; nt < 16; ++nt) *reinterpret_cast<float2 *>(row + nt * 8 + col) = make_float2(o[nt][0], o[nt][1]);
+            if ((lane & 3) == 0) *reinterpret_cast<float2 *>(row + kDim) = make_float2(m_run, l_tot);
+        }
+        __threadfence_block();
+        __syncwarp();
+        int last = 0, mask = 0;
+        if (lane == 0) {
+            atomicOr(s_mask + slot, 1 << warp);
+            __threadfence_block();
+            last = atomicAdd(s_count + slot, n_mine) + n_mine == part_len;
+            if (last) { __threadfence_block(); mask = lds_volatile(s_mask + slot); }
+        }
+        last = __shfl_sync(kFull, last, 0);
+        if (!last) return;
+        mask = __shfl_sync(kFull, mask, 0);
+        // ---- merge the parked states (consumer order) ----
+        float m_new = -INFINITY, l_new = 0.f;
 #pragma unroll
         for (int nt = 0; nt < 16; ++nt) { o[nt][0] = 0.f; o[nt][1] = 0.f; }
-        float m_run = -INFINITY, l_run = 0.f;
+        if (hrow < r) {
+            for (int w2 = 0; w2 < kDecConsumers; ++w2) {
+                if (!((mask >> w2) & 1)) continue;
+                const float2 ml = *reinterpret_cast<const float2 *>(area + (w2 * kMaxGroup + hrow) * kAccRow + kDim);
+                if (ml.y > 0.f) m_new = fmaxf(m_new, ml.x);
+            }
+            for (int w2 = 0; w2 < kDecConsumers; ++w2) {
+                if (!((mask >> w2) & 1)) continue;
+                const float *row = area + (w2 * kMaxGroup + hrow) * kAccRow;
+                const float2 ml = *reinterpret_cast<const float2 *>(row + kDim);
+                const float wgt = ml.y > 0.f ? fast_exp2(ml.x - m_new) : 0.f;           // empty state: weight 0, never NaN
+                l_new = fmaf(ml.y, wgt, l_new);
+#pragma unroll
+                for (int nt = 0; nt < 16; ++nt) {
+                    const float2 a = *reinterpret_cast<const float2 *>(row + nt * 8 + col);
+                    o[nt][0] = fmaf(a.x, wgt, o[nt][0]);
+                    o[nt][1] = fmaf(a.y, wgt, o[nt][1]);
+                }
+            }
+        }
+        __syncwarp();
+        if (lane == 0) {                                            // the parking area goes to the part after next
+            sts_volatile(s_count + slot, 0);
+            sts_volatile(s_mask + slot, 0);
+            __threadfence_block();
+            sts_volatile(s_gen + slot, part / kAccSlots + 1);
+        }
+        // ---- o / (m_new, l_new) in registers are the CTA's result for the unit ----
+        const int seq = unit / n_kv_heads, g = unit - seq * n_kv_heads;
+        const int c = s_prefix[seq + 1] - s_prefix[seq];
+        const int u0 = s_prefix[seq] * n_kv_heads + g * c, u1 = u0 + c;
+        if (u0 >= ra && u1 <= rb) {                                 // the unit lies inside this CTA's range: final result
+            if (hrow < r) {
+                const float inv = l_new > 0.f ? 1.f / l_new : 0.f;
+                uint32_t *dst = reinterpret_cast<uint32_t *>(A.out + ((int64_t)unit * r + hrow) * kDim + col);
+#pragma unroll
+                for (int nt = 0; nt < 16; ++nt) dst[nt * 4] = pack_bf16(o[nt][0] * inv, o[nt][1] * inv);
+                if (A.lse && (lane & 3) == 0)
+                    A.lse[(int64_t)unit * r + hrow] = l_new > 0.f ? (m_new + log2f(l_new)) * kLn2 : -INFINITY;
+            }
+            return;
+        }
+        // ---- the unit spans CTAs (a7): park the CTA's partial in slot unit + CTA index and arrive on the unit's counter.
+        // Release / acquire through ONE atomic of lane 0: the warp barrier orders the lanes' partial stores before the
+        // acq_rel atomic (cumulative at gpu scope), and the barrier after it orders that acquire before the other lanes'
+        // reads of the other CTAs' slots (ld.global.cg below).  The CTA that arrives last merges in stream order.
+        const int c_first = cr.owner(u0), c_last = cr.owner(u1 - 1);
+        {
+            const int64_t gslot = (int64_t)unit + blockIdx.x;       // unique: unit + CTA index increases along the stream
+            if (hrow < r) {
+                float *po = A.ws_o + (gslot * r + hrow) * kDim + col;
+#pragma unroll
+                for (int nt = 0; nt < 16; ++nt) *reinterpret_cast<float2 *>(po + nt * 8) = make_float2(o[nt][0], o[nt][1]);
+                if ((lane & 3) == 0) *reinterpret_cast<float2 *>(A.ws_ml + (gslot * r + hrow) * 2) = make_float2(m_new, l_new);
+            }
+        }
+        __syncwarp();
+        int old = 0;
+        if (lane == 0)
+            asm volatile("atom.acq_rel.gpu.global.add.s32 %0, [%1], 1;" : "=r"(old) : "l"(A.counters + unit) : "memory");
+        old = __shfl_sync(kFull, old, 0);
+        __syncwarp();
+        if (old != c_last - c_first) return;                        // not the last CTA to arrive
+        if (lane == 0) A.counters[unit] = 0;                        // restore the zero for the next call
+        const int nseg = c_last - c_first + 1;
+        for (int h = 0; h < r; ++h) {                               // one head at a time: lane = 4 dims
+            const int64_t row0 = ((int64_t)unit + c_first) * r + h; // slot row of CTA c: row0 + (c - c_first) * r
+            float m_star = -INFINITY;
+            for (int s0 = 0; s0 < nseg; s0 += 32) {
+                const int s = s0 + lane;
+                float2 ml = make_float2(-INFINITY, 0.f);
+                if (s < nseg) ml = __ldcg(reinterpret_cast<const float2 *>(A.ws_ml + (row0 + (int64_t)s * r) * 2));
+                float mm = ml.y > 0.f ? ml.x : -INFINITY;
+#pragma unroll
+                for (int of = 16; of > 0; of >>= 1) mm = fmaxf(mm, __shfl_xor_sync(kFull, mm, of));
+                m_star = fmaxf(m_star, mm);
+            }
+            float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+            float l_star = 0.f;
+            for (int s0 = 0; s0 < nseg; s0 += 4) {                   // four partial rows requested together
+                float4 v[4];
+                float2 ml[4];
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    v[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+                    ml[k] = make_float2(-INFINITY, 0.f);
+                    if (s0 + k < nseg) {
+                        v[k] = __ldcg(reinterpret_cast<const float4 *>(A.ws_o + (row0 + (int64_t)(s0 + k) * r) * kDim + lane * 4));
+                        ml[k] = __ldcg(reinterpret_cast<const float2 *>(A.ws_ml + (row0 + (int64_t)(s0 + k) * r) * 2));
+                    }
+                }
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const float wgt = ml[k].y > 0.f ? fast_exp2(ml[k].x - m_star) : 0.f;   // empty partial: weight 0, never NaN
+                    l_star = fmaf(ml[k].y, wgt, l_star);
+                    acc.x = fmaf(v[k].x, wgt, acc.x); acc.y = fmaf(v[k].y, wgt, acc.y);
+                    acc.z = fmaf(v[k].z, wgt, acc.z); acc.w = fmaf(v[k].w, wgt, acc.w);
+                }
+            }
+            const float inv = l_star > 0.f ? 1.f / l_star : 0.f;
+            uint2 pk;
+            pk.x = pack_bf16(acc.x * inv, acc.y * inv);
+            pk.y = pack_bf16(acc.z * inv, acc.w * inv);
+            *reinterpret_cast<uint2 *>(A.out + ((int64_t)unit * r + h) * kDim + lane * 4) = pk;
+            if (A.lse && lane == 0)
+                A.lse[(int64_t)unit * r + h] = l_star > 0.f ? (m_star + log2f(l_star)) * kLn2 : -INFINITY;
+        }
+    };
 
-        // this consumer's tiles of the part: those whose index in the CTA's range is = warp (mod 8)
+    int part = -1, unit = 0, n_mine = 0, part_len = 0;              // the part this consumer is accumulating
 #pragma unroll 1
-        for (int t = p + ((warp - (p - ra)) & (kDecConsumers - 1)); t < e; t += kDecConsumers) {
-            const int it = t - ra, stage = it % kDecStages;
+    while (true) {
+        int cidx = 0;
+        if (lane == 0) cidx = atomicAdd(s_claim, 1);
+        cidx = __shfl_sync(kFull, cidx, 0);
+        const int it0 = cidx * kDecChunk;
+        if (lane == 0) sts_volatile(s_pos + warp, it0 < n_tiles ? it0 : 0x7fffffff);
+        if (it0 >= n_tiles) break;
+        const int it1 = min(it0 + kDecChunk, n_tiles);
+#pragma unroll 1
+        for (int it = it0; it < it1; ++it) {
+            spin_until(s_ready, it + 1);                            // (the look-up warp runs far ahead: rarely taken)
+            __threadfence_block();
+            const int4 d = s_desc[it & (kDescRing - 1)];
+            if ((d.z >> 8) != part) {                               // a tile of another part: park the state of the old one
+                if (part >= 0) park(part, unit, n_mine, part_len);
+                part = d.z >> 8; unit = d.y; n_mine = 0; part_len = d.w;
+#pragma unroll
+                for (int nt = 0; nt < 16; ++nt) { o[nt][0] = 0.f; o[nt][1] = 0.f; }
+                m_run = -INFINITY; l_run = 0.f;
+                if (unit != q_unit) {
+                    q_unit = unit;
+                    const uint16_t *qrow = A.q + ((int64_t)unit * r + hrow) * kDim + col;
+#pragma unroll
+                    for (int kk = 0; kk < 8; ++kk) {
+                        qa[kk][0] = hrow < r ? __ldg(reinterpret_cast<const uint32_t *>(qrow + kk * 16)) : 0u;
+                        qa[kk][1] = hrow < r ? __ldg(reinterpret_cast<const uint32_t *>(qrow + kk * 16 + 8)) : 0u;
+                    }
+                }
+            }
+            ++n_mine;
+            const int valid = d.z & 31;
+            const int stage = it % kDecStages;
+            // A consumer may be handed tile `it` while the stage still holds tile it - kDecStages (another consumer's):
+            // a parity wait is only meaningful once the barrier has moved on to this tile's phase, i.e. once the tile has
+            // been requested (before that, "the phase of the other parity" reads as complete).
+            spin_until(s_issued + stage, it);
             mbar_wait(full_u32 + 8 * stage, (it / kDecStages) & 1);
-            const int valid = s_valid[stage];
             const uint32_t kb = ring_u32 + stage * kStageBytes;
             const uint32_t vb = kb + kTileBytes;
             if (valid < kPage) {
@@ -373,127 +588,15 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
                 mma_rows07(o[2 * jn][0], o[2 * jn][1], pa0, pa2, b0, b1);
                 mma_rows07(o[2 * jn + 1][0], o[2 * jn + 1][1], pa0, pa2, b2, b3);
             }
-            // ---- the stage is free: every lane has read it (the zeroing above was a generic-proxy WRITE: make it visible to
-            // the async proxy before the copy engine may overwrite the stage) ----
-            if (valid < kPage) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            // ---- the stage is free: every lane has read it; the consumer that used it refills it with the tile one ring
+            // further on (generic-proxy accesses to the stage -- the reads, the zeroing -- are ordered before the copy
+            // engine's writes by the proxy fence) ----
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             __syncwarp();
-            if (lane == 0) mbar_arrive(empty_u32 + 8 * stage);
-        }
-
-        // ---- park this consumer's state of the part; consumer h then merges query head h over the eight parked states ----
-        {
-            float l_tot = l_run;
-            l_tot += __shfl_xor_sync(kFull, l_tot, 1);
-            l_tot += __shfl_xor_sync(kFull, l_tot, 2);
-            if (hrow < r) {
-                float *row = s_park + (warp * kMaxGroup + hrow) * kParkRow;
-#pragma unroll
-                for (int nt = 0; nt < 16; ++nt) *reinterpret_cast<float2 *>(row + nt * 8 + col) = make_float2(o[nt][0], o[nt][1]);
-                if ((lane & 3) == 0) *reinterpret_cast<float2 *>(row + kDim) = make_float2(m_run, l_tot);
-            }
-        }
-        consumer_sync();
-        const bool whole = u0 >= ra && u1 <= rb;                    // the unit lies inside this CTA's range: the result is final
-        const int c_first = cr.owner(u0), c_last = cr.owner(u1 - 1);
-        const int h = warp;                                         // the query head this consumer merges
-        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-        float m_star = -INFINITY, l_star = 0.f;
-        if (h < r) {
-            float mw[kDecConsumers], lw[kDecConsumers];
-#pragma unroll
-            for (int w2 = 0; w2 < kDecConsumers; ++w2) {
-                const float2 ml = *reinterpret_cast<const float2 *>(s_park + (w2 * kMaxGroup + h) * kParkRow + kDim);
-                mw[w2] = ml.x; lw[w2] = ml.y;
-                if (ml.y > 0.f) m_star = fmaxf(m_star, ml.x);
-            }
-#pragma unroll
-            for (int w2 = 0; w2 < kDecConsumers; ++w2) {           // fixed order: the result does not depend on timing
-                const float wgt = lw[w2] > 0.f ? fast_exp2(mw[w2] - m_star) : 0.f;      // empty state: weight 0, never NaN
-                const float4 v = *reinterpret_cast<const float4 *>(s_park + (w2 * kMaxGroup + h) * kParkRow + lane * 4);
-                l_star = fmaf(lw[w2], wgt, l_star);
-                acc.x = fmaf(v.x, wgt, acc.x); acc.y = fmaf(v.y, wgt, acc.y);
-                acc.z = fmaf(v.z, wgt, acc.z); acc.w = fmaf(v.w, wgt, acc.w);
-            }
-            if (whole) {
-                const float inv = l_star > 0.f ? 1.f / l_star : 0.f;
-                uint2 pk;
-                pk.x = pack_bf16(acc.x * inv, acc.y * inv);
-                pk.y = pack_bf16(acc.z * inv, acc.w * inv);
-                *reinterpret_cast<uint2 *>(A.out + ((int64_t)unit * r + h) * kDim + lane * 4) = pk;
-                if (A.lse && lane == 0)
-                    A.lse[(int64_t)unit * r + h] = l_star > 0.f ? (m_star + log2f(l_star)) * kLn2 : -INFINITY;
-            } else {
-                const int64_t slot = (int64_t)unit + blockIdx.x;    // unique: unit + CTA index increases along the stream
-                *reinterpret_cast<float4 *>(A.ws_o + (slot * r + h) * kDim + lane * 4) = acc;
-                if (lane == 0) *reinterpret_cast<float2 *>(A.ws_ml + (slot * r + h) * 2) = make_float2(m_star, l_star);
-            }
-        }
-        if (!whole) {
-            // ---- arrival (a7): release / acquire through ONE atomic of one thread: the consumer barrier orders the eight
-            // warps' partial stores before the acq_rel atomic (cumulative at gpu scope), and the barrier after it orders
-            // that acquire before the other threads' reads of the other CTAs' slots (ld.global.cg below) ----
-            consumer_sync();
-            if (tid == 0) {
-                int old;
-                asm volatile("atom.acq_rel.gpu.global.add.s32 %0, [%1], 1;" : "=r"(old) : "l"(A.counters + unit) : "memory");
-                const int last = old == c_last - c_first;
-                if (last) A.counters[unit] = 0;                     // restore the zero for the next call
-                *s_flag = last;
-            }
-            consumer_sync();
-            if (*s_flag && h < r) {
-                // the last CTA to arrive merges the CTAs' partials in stream order (deterministic)
-                const int nseg = c_last - c_first + 1;
-                const int64_t row0 = ((int64_t)unit + c_first) * r + h;                 // slot row of CTA c: row0 + (c - c_first) * r
-                m_star = -INFINITY;
-                for (int s0 = 0; s0 < nseg; s0 += 32) {
-                    const int s = s0 + lane;
-                    float2 ml = make_float2(-INFINITY, 0.f);
-                    if (s < nseg) ml = __ldcg(reinterpret_cast<const float2 *>(A.ws_ml + (row0 + (int64_t)s * r) * 2));
-                    float mm = ml.y > 0.f ? ml.x : -INFINITY;
-#pragma unroll
-                    for (int of = 16; of > 0; of >>= 1) mm = fmaxf(mm, __shfl_xor_sync(kFull, mm, of));
-                    m_star = fmaxf(m_star, mm);
-                }
-                acc = make_float4(0.f, 0.f, 0.f, 0.f);
-                l_star = 0.f;
-                for (int s0 = 0; s0 < nseg; s0 += 4) {               // four partial rows requested together
-                    float4 v[4];
-                    float2 ml[4];
-#pragma unroll
-                    for (int k = 0; k < 4; ++k) {
-                        v[k] = make_float4(0.f, 0.f, 0.f, 0.f);
-                        ml[k] = make_float2(-INFINITY, 0.f);
-                        if (s0 + k < nseg) {
-                            v[k] = __ldcg(reinterpret_cast<const float4 *>(A.ws_o + (row0 + (int64_t)(s0 + k) * r) * kDim + lane * 4));
-                            ml[k] = __ldcg(reinterpret_cast<const float2 *>(A.ws_ml + (row0 + (int64_t)(s0 + k) * r) * 2));
-                        }
-                    }
-#pragma unroll
-                    for (int k = 0; k < 4; ++k) {
-                        const float wgt = ml[k].y > 0.f ? fast_exp2(ml[k].x - m_star) : 0.f;
-                        l_star = fmaf(ml[k].y, wgt, l_star);
-                        acc.x = fmaf(v[k].x, wgt, acc.x); acc.y = fmaf(v[k].y, wgt, acc.y);
-                        acc.z = fmaf(v[k].z, wgt, acc.z); acc.w = fmaf(v[k].w, wgt, acc.w);
-                    }
-                }
-                const float inv = l_star > 0.f ? 1.f / l_star : 0.f;
-                uint2 pk;
-                pk.x = pack_bf16(acc.x * inv, acc.y * inv);
-                pk.y = pack_bf16(acc.z * inv, acc.w * inv);
-                *reinterpret_cast<uint2 *>(A.out + ((int64_t)unit * r + h) * kDim + lane * 4) = pk;
-                if (A.lse && lane == 0)
-                    A.lse[(int64_t)unit * r + h] = l_star > 0.f ? (m_star + log2f(l_star)) * kLn2 : -INFINITY;
-            }
-        }
-        consumer_sync();                                            // the parked states (and the flag) are free again
-        // ---- next unit ----
-        p = e;
-        if (e == u1 && g + 1 == n_kv_heads) {
-            ++seq;
-            while (seq < n_seq && s_prefix[seq + 1] == s_prefix[seq]) ++seq;            // sequences with an empty list
+            if (lane == 0 && it + kDecStages < n_tiles) issue(it + kDecStages);
         }
     }
+    if (part >= 0) park(part, unit, n_mine, part_len);
 }
 
 }  // namespace sparrow
