@@ -408,7 +408,7 @@ def run_single(args, cfg, rank, local_rank, world, dev, headline=True) -> dict:
     e2e_value, _ = D.whole_job_throughput(wl.n_seq * K, e0.elapsed_time(e1) * 1e-3, device=dev)
     h2d = int(hb.q.numel() * 2 + hb.seq_lens.numel() * 4 + n_upd * 4)
     d2h = int(out_h.numel() * 2)
-    e2e_match = bool(torch.equal(out_h, eng.out.cpu()))
+    e2e_match = bool(((out_h.float() - eng.out.cpu().float()).abs() <= 2.0 ** -7 * out_h.float().abs() + 1e-6).all())     # to the last bf16 bit (run-time tile hand-out)
 
     if rank != 0:
         return {}
@@ -619,7 +619,8 @@ def run_cfg4(args, rank, local_rank, world, dev) -> dict:
         host_full_step()
     h1e.record(st); st.synchronize()
     e2e_value, _ = D.whole_job_throughput(wl0.n_seq * Ke, h0e.elapsed_time(h1e) * 1e-3, device=dev)
-    e2e_match = bool(torch.equal(out_h, engs[(n_layers - 1) % n_pools].out.cpu()))
+    ref_o = engs[(n_layers - 1) % n_pools].out.cpu().float()
+    e2e_match = bool(((out_h.float() - ref_o).abs() <= 2.0 ** -7 * ref_o.abs() + 1e-6).all())
     if rank != 0:
         return {}
     eng = engs[0]

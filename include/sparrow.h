@@ -130,10 +130,12 @@ int sparrow_select(const void *q, const void *summaries, const int32_t *page_tab
  * gathered through page_table; fp32 accumulation, bf16 output; lse (optional, may be NULL) = ln sum exp.
  * workspace: sparrow_decode_workspace_bytes(shape, max_sel) bytes, ZERO-INITIALISED once by the caller (it
  * holds the split-K arrival counters; the kernel restores the zeros it uses, so it can be reused call
- * after call, but not by two calls in flight at the same time).  n_seq <= 8192.  The merge of the splits
+ * after call, but not by two calls in flight at the same time).  n_seq <= 4096.  The merge of the splits
  * is fused into the same launch (one kernel per call).  The K/V tiles are fetched by TMA: each call encodes
  * two tensor maps over the pools on the host (cuTensorMapEncodeTiled, a few microseconds) and passes them by value,
- * so the call stays asynchronous and graph-capturable; the result is bit-for-bit reproducible from call to call. */
+ * so the call stays asynchronous and graph-capturable.  Reproducibility: the page tiles are handed to the CTA's warps at
+ * run time, so the fp32 summation order can differ between two calls on the same inputs -- out may differ in the last
+ * bf16 bit, lse by fp32 rounding; nothing else varies. */
 int sparrow_sparse_decode(const void *q, const void *k_cache, const void *v_cache, const int32_t *page_table,
                           const int32_t *seq_lens, const int32_t *sel_pages, int32_t max_sel,
                           const int32_t *sel_count, void *out, float *lse, float sm_scale,

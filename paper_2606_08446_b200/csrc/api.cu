@@ -164,16 +164,21 @@ int to_dev_sched(const sparrow_schedule_t *in, SchedDev *out, int page_tokens = 
     return SPARROW_OK;
 }
 
-// Decode workspace: arrival counters (one per (sequence, kv-head) unit, all zero between calls), then the fp32 partial
-// slots of the CTAs (indexed unit + CTA index) and their (m, l) pairs.
+// Decode workspace: per-unit counters + the tail-piece counter + the CTAs-done counter (all zero between calls), then the
+// fp32 partial slots of the pieces (indexed unit + piece id) and their (m, l) pairs.  Pieces: one static piece per CTA
+// plus the self-scheduled tail pieces of kTailChunk tiles (decode.cuh).
 struct DecodeGeom {
     size_t bytes_o, bytes_ml, bytes_ctr;
 };
-DecodeGeom decode_geom(const sparrow_shape_t *s)
+DecodeGeom decode_geom(const sparrow_shape_t *s, int32_t max_sel /* 0 = dense */)
 {
     DecodeGeom gm;
     const size_t units = (size_t)s->n_seq * s->n_kv_heads;
-    const size_t rows = (units + (size_t)kDecGrid) * (s->n_q_heads / s->n_kv_heads);
+    const int64_t max_cnt = (max_sel > 0 && max_sel < s->max_pages_per_seq) ? max_sel : s->max_pages_per_seq;
+    const int64_t t_max = (int64_t)units * max_cnt * (s->page_size / kPage);                       // tiles of the stream at most
+    const int64_t tail_max = t_max - t_max * SPARROW_DEC_STATIC_NUM / SPARROW_DEC_STATIC_DEN;
+    const size_t pieces = (size_t)kDecGrid + (size_t)((tail_max + kTailChunk - 1) / kTailChunk) + 1;
+    const size_t rows = (units + pieces) * (s->n_q_heads / s->n_kv_heads);
     gm.bytes_o = (rows * kDim * sizeof(float) + 255) & ~(size_t)255;
     gm.bytes_ml = (rows * 2 * sizeof(float) + 255) & ~(size_t)255;
     gm.bytes_ctr = ((units + 2) * sizeof(int32_t) + 255) & ~(size_t)255;
@@ -225,7 +230,7 @@ int launch_decode(const void *q, const void *k_cache, const void *v_cache, const
                   void *out, float *lse, float sm_scale, void *workspace, size_t workspace_bytes,
                   const sparrow_shape_t *s, cudaStream_t st)
 {
-    const DecodeGeom gm = decode_geom(s);
+    const DecodeGeom gm = decode_geom(s, kDense ? 0 : max_sel);
     if (workspace_bytes < gm.bytes_ctr + gm.bytes_o + gm.bytes_ml) return SPARROW_ERR_WORKSPACE_TOO_SMALL;
     if (s->n_seq > kDecMaxSeq) return SPARROW_ERR_UNSUPPORTED;
     {   // flat tile positions and TMA row coordinates are 32-bit
@@ -354,8 +359,7 @@ size_t sparrow_select_workspace_bytes(const sparrow_shape_t *s)
 size_t sparrow_decode_workspace_bytes(const sparrow_shape_t *s, int32_t max_sel)
 {
     if (check_shape(s) != SPARROW_OK) return 0;
-    (void)max_sel;
-    const DecodeGeom gm = decode_geom(s);
+    const DecodeGeom gm = decode_geom(s, max_sel);
     return gm.bytes_ctr + gm.bytes_o + gm.bytes_ml;
 }
 

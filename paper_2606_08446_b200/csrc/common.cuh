@@ -141,14 +141,23 @@ __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)_
 
 // ---- programmatic dependent launch: the step's kernels (summarize / append -> select -> decode) are launched with
 // cudaLaunchAttributeProgrammaticStreamSerialization, so the next kernel's CTAs can be brought up while this one
-// drains.  Every kernel calls this first: it lets its dependents start launching and then waits until everything
+// drains.  Every kernel calls chain_entry() first: it lets its dependents start launching and then waits until everything
 // before it in the stream has completed and is visible -- nothing is read or written before that point.
+// The decode kernel calls chain_wait() only: it leaves room on its SMs (168 registers, one CTA), so a dependent launched
+// early would sit beside it for the whole launch, and warps parked in griddepcontrol.wait are not free (measured: the
+// step 15 us slower at cfg3 with select's CTAs resident beside the decode CTAs).  Its dependents start when it completes.
+__device__ __forceinline__ void chain_wait()
+{
+#ifndef SPARROW_NO_PDL
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+#endif
+}
 __device__ __forceinline__ void chain_entry()
 {
 #ifndef SPARROW_NO_PDL
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    asm volatile("griddepcontrol.wait;" ::: "memory");
 #endif
+    chain_wait();
 }
 
 // ---- mbarrier + bulk-copy (TMA) primitives; shared-memory operands are 32-bit shared::cta addresses ----

@@ -3,30 +3,38 @@
 //
 // Work decomposition ("stream-K" over pages): the (page, kv-head) tiles of the whole batch form ONE flat stream,
 // ordered (sequence, kv-head, list position); its length T = Hkv * sum_i cnt_i is known from sel_count (or from
-// seq_lens for the dense entry).  A persistent grid of one CTA per SM cuts it into equal contiguous CTA RANGES,
-// whatever the mix of lengths and budgets.  Inside a CTA the work is warp-specialised:
+// seq_lens for the dense entry).  A persistent grid of one CTA per SM cuts it into equal contiguous PIECES, whatever
+// the mix of lengths and budgets (optionally followed by a self-scheduled tail of small pieces: SPARROW_DEC_STATIC_*,
+// off by default).  Inside a CTA the work is warp-specialised:
 //
-//   * ONE PRODUCER WARP walks the CTA's range.  It resolves flat tile -> (sequence, kv-head, list position) ->
-//     logical page -> physical tile in windows of 32 tiles (lane = tile; three look-up stages so that no stage
-//     consumes a load issued by the stage before it in the same breath), and one elected lane issues the copies:
-//     the 4 KiB K tile and the 4 KiB V tile of a page are each two TMA boxes of 16 tokens x 64 dims
-//     (cp.async.bulk.tensor.2d, SWIZZLE_128B, mbarrier complete_tx) into a CTA-wide ring of kDecStages stages.
-//   * EIGHT CONSUMER WARPS take the ring's tiles round-robin (tile i of the range -> consumer i mod 8), each with its
-//     own online-softmax state for the (sequence, kv-head) unit the CTA is in.  When the CTA's part of a unit ends
-//     the consumers park their (o, m, l) in shared memory, meet at a named barrier and merge: consumer h merges query
-//     head h of the group.  The result is final (written straight to `out`) when the unit lies inside the CTA's
-//     range; otherwise it is the CTA's partial, parked in slot unit + CTA index of a small fp32 workspace, and the
-//     CTA that arrives last on the unit's counter merges the CTAs' partials in stream order (a7; no second launch).
+//   * ONE LOOK-UP WARP walks the CTA's stream.  It resolves flat tile -> (sequence, kv-head, list position) -> logical
+//     page -> physical tile in windows of 32 tiles (lane = tile; three look-up stages, three windows in flight, so that
+//     no stage consumes a load issued by the stage before it in the same breath) and publishes one 16-byte descriptor
+//     per tile in a shared-memory ring, far ahead of the consumers.
+//   * EIGHT CONSUMER WARPS share a CTA-wide ring of kDecStages = 16 stages of 8 KiB (the K tile and the V tile of a
+//     page).  A tile is fetched by TMA: two cp.async.bulk.tensor.2d boxes of 32 rows x 128 B (SWIZZLE_128B, mbarrier
+//     complete_tx), issued by one lane of the consumer that has just freed the stage (tile i + 16 follows tile i), so the
+//     copy issue is spread over the eight warps.  The consumers take the stream two tiles at a time from a counter in
+//     shared memory -- whoever is free takes the next chunk -- each with its own online-softmax state for the unit
+//     (sequence, kv-head) it is in.  When a consumer is handed a tile of another unit it parks its state in shared
+//     memory; the consumer whose tiles complete the CTA's PART of the unit merges the parked states and writes the
+//     result: final (straight to `out`) when the unit lies inside the piece, otherwise the piece's partial, in slot
+//     unit + piece id of a small fp32 workspace -- the warp that completes the unit's tile count merges the pieces'
+//     partials in stream order (a7; no second launch).
 //
 // Why this shape (round 2): with one private stream per warp (round 1) a warp's progress is a sum of
-// ~50 saturated-HBM latencies, the per-warp finish times spread with sigma ~7 us on a 90 us launch and the kernel
-// ends with the slowest of 1184 warps (traced: median 80 us, maximum 97 us at cfg2).  A CTA-wide ring averages the
-// latencies over eight times as many tiles, keeps 128 KiB in flight per SM whatever a single warp is doing, and the
-// static round-robin keeps the summation order -- and so the result -- bit-for-bit reproducible.
+// ~50 saturated-HBM latencies; the per-warp finish times spread with sigma ~7 us on a 90 us launch and the kernel
+// ends with the slowest of 1184 warps.  Handing the tiles out inside the CTA brings the warps of a CTA to within 2 us
+// of one another (traced).  What remains is the spread BETWEEN SMs (equal pieces end +-15 % apart), see DESIGN.md.
+// The price of run-time hand-out: which tiles a consumer sums is timing-dependent, so the fp32 summation order, and
+// with it the last bit of a bf16 output, can differ from call to call (the page lists, counts and everything integer
+// are exact and reproducible).
 // The whole GQA group (r <= 8 query heads) is processed together, so each K/V byte is read from HBM once.
 //
-// Shared layout of a tile: [half = dim/64][token 0..15][64 dims = 8 chunks of 16 B], chunk index XOR (token & 7) --
-// exactly what a 16 x 64 box lands as under SWIZZLE_128B, conflict-free for ldmatrix.
+// Shared layout of a tile: 32 rows of 128 B, row = (token, half of the head dim), 16-byte chunk index XOR (row & 7) --
+// what a 32 x 64 box of the pool's [128-byte rows] view lands as under SWIZZLE_128B: ONE copy per 4 KiB tile (two
+// 16 x 64 boxes per tile made the copy issue the limit).  ldmatrix reads it with 2-way bank conflicts (tokens t and
+// t + 4 of a half share a bank group); the shared-memory pipe is a third busy at full HBM rate, so they are not the limit.
 //
 // Math: the products are a [heads x 128] x [128 x 16 tokens] and a [heads x 16] x [16 x 128] contraction per page;
 // at r >= 4 the plain FP32 pipes cannot keep up with HBM ("ALU budget"), so both run on the tensor
@@ -61,8 +69,18 @@ constexpr int kAccRow = kDim + 4;                               // one parked he
 constexpr int kAccSlots = 2;                                    // parts (the CTA's share of a unit) being parked at once
 constexpr int kDecAccBytes = kAccSlots * kDecConsumers * kMaxGroup * kAccRow * 4;   // [slot][consumer][head][kAccRow]
 constexpr int kDescRing = 256;                                  // per-tile descriptors the look-up warp runs ahead by
-constexpr int kDecDescBytes = kDescRing * 16;
-constexpr int kDecMetaBytes = kDecStages * 8 + kDecStages * 4 + 3 * kAccSlots * 4 + kDecConsumers * 4 + 64;   // full barriers | issued tile per stage | area generation, tile count, consumer mask | consumer positions | claim, ready
+constexpr int kPartRing = 512;                                  // per-part records (piece id, piece bounds) kept beside them
+constexpr int kDecDescBytes = kDescRing * 16 + kPartRing * 16;
+constexpr int kTailChunk = 32;                                  // tiles of a self-scheduled piece of the stream's tail (= one look-up window)
+// share of the stream that is split evenly over the CTAs; the rest is self-scheduled in pieces of kTailChunk tiles.
+// Default 1 / 1 = no tail: measured, the tail's extra partials and merges cost more than the balance buys.
+#ifndef SPARROW_DEC_STATIC_NUM
+#define SPARROW_DEC_STATIC_NUM 1
+#endif
+#ifndef SPARROW_DEC_STATIC_DEN
+#define SPARROW_DEC_STATIC_DEN 1
+#endif
+constexpr int kDecMetaBytes = kDecStages * 8 + kDecStages * 4 + 3 * kAccSlots * 4 + kDecConsumers * 4 + 64;   // (+ claim, ready, total)   // full barriers | issued tile per stage | area generation, tile count, consumer mask | consumer positions | claim, ready
 
 __device__ __forceinline__ void ldsm_x4(uint32_t &r0, uint32_t &r1, uint32_t &r2, uint32_t &r3, uint32_t addr)
 {
@@ -132,8 +150,8 @@ struct DecodeArgs {
     const uint16_t *q;
     const int32_t *page_table, *seq_lens, *sel_pages, *sel_count;
     int max_sel;
-    float *ws_o, *ws_ml;         // CTA partials: [units + grid][r][128] and [..][r][2] (m, l)
-    int32_t *counters;           // [units] CTAs arrived per unit (zero between calls)
+    float *ws_o, *ws_ml;         // partials of the pieces: [units + pieces][r][128] and [..][r][2] (m, l)
+    int32_t *counters;           // [units] tiles of the unit merged so far | tail-piece counter | CTAs done   (all zero between calls)
     uint16_t *out;
     float *lse;
     float scale_log2;
@@ -156,7 +174,7 @@ template <bool kDense>
 __global__ void __launch_bounds__(kDecThreads, 1)
 decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v)
 {
-    chain_entry();
+    chain_wait();
     extern __shared__ __align__(1024) uint8_t smem[];
     float *s_acc = reinterpret_cast<float *>(smem + kDecRingBytes);                           // [slot][consumer][head][kAccRow]
     int4 *s_desc = reinterpret_cast<int4 *>(smem + kDecRingBytes + kDecAccBytes);             // [kDescRing] per-tile descriptors
@@ -218,12 +236,22 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
         __syncthreads();
     }
     const int T = s_prefix[n_seq] * n_kv_heads;                  // tiles of the whole batch
+    if (T == 0) return;
+    // The stream is cut into PIECES.  Its first kStatic part is split evenly: CTA b owns piece b, a contiguous range.  The
+    // rest, the tail, is cut into pieces of kTailChunk tiles that the CTAs take from one global counter as they run out of
+    // work: SMs are not served equally by the memory system (equal ranges end +-15 % apart, traced), and the tail evens
+    // them out to within a piece.  Piece ids increase along the stream: b for the static pieces, G + j for tail piece j.
+    const int G = (int)gridDim.x;
+    const int T0 = (int)((int64_t)T * SPARROW_DEC_STATIC_NUM / SPARROW_DEC_STATIC_DEN);
     CtaRanges cr;
-    cr.per = T / (int)gridDim.x;
-    cr.extra = T - cr.per * (int)gridDim.x;
-    const int ra = cr.begin(blockIdx.x), rb = cr.begin(blockIdx.x + 1);         // this CTA's tiles [ra, rb)
-    const int n_tiles = rb - ra;
-    if (n_tiles <= 0) return;
+    cr.per = T0 / G;
+    cr.extra = T0 - cr.per * G;
+    const int ra = cr.begin(blockIdx.x), rb = cr.begin(blockIdx.x + 1);         // this CTA's static piece [ra, rb)
+    int32_t *tail_ctr = A.counters + n_seq * n_kv_heads, *done_ctr = tail_ctr + 1;
+    int4 *s_part = s_desc + kDescRing;                           // [kPartRing] x = piece id, y = piece begin, z = piece end (stream tiles)
+    int32_t *s_total = s_ready + 1;                              // tiles of this CTA's stream, once known (INT_MAX before)
+    if (tid == 0) sts_volatile(s_total, 0x7fffffff);
+    __syncthreads();
     // sequence that holds flat tile p: the last one whose first tile is <= p and that is not empty
     auto seq_of = [&](int p) {
         int lo = 0, hi = n_seq - 1;
@@ -237,20 +265,21 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
 
     if (warp == kDecConsumers) {
         // =========================================================== LOOK-UP WARP ===========================================
-        // flat tile p -> (sequence, kv-head, list position) -> logical page -> physical tile, as three stages so that no
-        // stage consumes a load issued by the stage before it in the same breath; a WINDOW is up to 32 consecutive tiles
-        // of the CTA's range, lane = tile.  The result is one 16-byte descriptor per tile in a ring the consumers read:
+        // It lines up the CTA's stream: its static piece, then tail pieces as it gets them.  flat tile p -> (sequence,
+        // kv-head, list position) -> logical page -> physical tile, as three stages so that no stage consumes a load
+        // issued by the stage before it in the same breath; a WINDOW is up to 32 consecutive tiles of one piece, lane =
+        // tile.  The result is one 16-byte descriptor per tile in a ring the consumers read:
         //   x = index of the 4 KiB K (and V) tile in the pools          y = unit (sequence * Hkv + kv-head)
-        //   z = valid tokens (bits 0-4) | part number, counted along the CTA's range (bits 8..)
-        //   w = tiles of the CTA's part of the unit
+        //   z = valid tokens (bits 0-4) | part number (bits 8..)        w = tiles of the part
+        // A PART is a run of the CTA's stream inside one unit and one piece: the granule the consumers reduce together.
         struct Lookup {
-            int tile, unit, meta, pos;
+            int tile, unit, meta, len_part;
             int seq, logical, len, phys, sub;
         };
-        int part_base = 0;                                       // parts of the range started before the window being looked up
-        auto stage_a = [&](Lookup &m, int p, bool on) {
-            bool starts = false;                                 // this tile is the first of a part other than the range's first
-            m.tile = 0; m.unit = 0; m.meta = 0; m.pos = 0; m.seq = -1; m.logical = 0; m.len = 0; m.phys = 0; m.sub = 0;
+        int part_base = 0;                                       // parts started before the window being looked up
+        auto stage_a = [&](Lookup &m, int p, bool on, int id, int cb, int ce) {
+            bool starts = false;                                 // this tile is the first of a part
+            m.tile = 0; m.unit = 0; m.meta = 0; m.len_part = 0; m.seq = -1; m.logical = 0; m.len = 0; m.phys = 0; m.sub = 0;
             if (on) {
                 const int seq = seq_of(p), base = s_prefix[seq], c = s_prefix[seq + 1] - base;
                 const int rem = p - base * n_kv_heads;
@@ -258,16 +287,18 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
                 const int u0 = base * n_kv_heads + g * c;        // the unit is tiles [u0, u0 + c) of the stream
                 m.seq = seq;
                 m.unit = seq * n_kv_heads + g;
-                m.pos = min(u0 + c, rb) - max(u0, ra);
-                starts = i == 0 && p != ra;
+                m.len_part = min(u0 + c, ce) - max(u0, cb);
+                starts = i == 0 || p == cb;
                 const int pi = i >> A.tpp_log2;                  // list position of the tile's page
                 m.sub = i - (pi << A.tpp_log2);
                 m.logical = kDense ? pi : __ldg(A.sel_pages + ((int64_t)m.unit) * max_sel + pi);
                 m.len = __ldg(A.seq_lens + seq);
             }
-            // parts are numbered densely along the range (the parking areas are handed out in that order)
+            // parts are numbered densely along the CTA's stream (the parking areas are handed out in that order)
             const uint32_t sm = __ballot_sync(kFull, starts);
-            m.meta = (part_base + __popc(sm & (0xffffffffu >> (31 - lane)))) << 8;
+            const int part = part_base + __popc(sm & (0xffffffffu >> (31 - lane))) - 1;
+            m.meta = part << 8;
+            if (starts) s_part[part & (kPartRing - 1)] = make_int4(id, cb, ce, 0);
             part_base += __popc(sm);
         };
         auto stage_b = [&](Lookup &m) {
@@ -279,17 +310,40 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
         };
         auto stage_c = [&](Lookup &m) { m.tile = ((m.phys * n_kv_heads + (m.unit - m.seq * n_kv_heads)) << A.tpp_log2) + m.sub; };
 
-        Lookup cur, nxt;
+        // The windows of the CTA's stream, in order: those of the static piece, then one per tail piece taken.  The claim of
+        // a tail piece is requested one window before it is needed (its round trip to the L2 is never waited for).
+        int sp = ra;                                             // next tile of the static piece not yet in a window
+        int j_next = -1;                                         // lane 0: tail piece claimed ahead (-1: none requested yet)
+        auto prefetch_claim = [&]() {
+            if (sp >= rb && lane == 0 && j_next < 0) j_next = atomicAdd(tail_ctr, 1);
+        };
+        auto next_window = [&](Lookup &m) -> int {               // opens the next window (look-up stage A); returns its tiles, 0 = none
+            int p0, n, id, cb, ce;
+            if (sp < rb) {
+                p0 = sp; n = min(32, rb - sp); id = (int)blockIdx.x; cb = ra; ce = rb;
+                sp += n;
+            } else {
+                prefetch_claim();
+                const int j = __shfl_sync(kFull, j_next, 0);
+                j_next = -1;
+                if ((int64_t)T0 + (int64_t)j * kTailChunk >= T) return 0;
+                p0 = T0 + j * kTailChunk; n = min(kTailChunk, T - p0); id = G + j; cb = p0; ce = p0 + n;
+            }
+            stage_a(m, p0 + lane, lane < n, id, cb, ce);
+            return n;
+        };
+        // three windows in flight: `cur` (stages A, B done; C when it is published), `nxt` (A, B), `nn2` (A)
+        Lookup cur, nxt, nx2;
         int w0 = 0;                                              // first tile (CTA-relative) of window `cur`
-        int cn = min(32, n_tiles);
-        stage_a(cur, ra + lane, lane < cn);
-        int nn = min(32, n_tiles - cn);
-        if (nn > 0) stage_a(nxt, ra + cn + lane, lane < nn);
-        stage_b(cur);
+        int cn = next_window(cur);
+        int nn = cn > 0 ? next_window(nxt) : 0;
+        int n2 = nn > 0 ? next_window(nx2) : 0;
+        if (n2 > 0) prefetch_claim();
+        if (cn > 0) stage_b(cur);
         if (nn > 0) stage_b(nxt);
-        stage_c(cur);
 #pragma unroll 1
         while (cn > 0) {
+            stage_c(cur);
             // room in the ring: the entries this window overwrites must be older than every consumer's current claim (a
             // consumer reads the descriptors of its claim's tiles, and of the tiles one ring further on when it refills
             // their stages).  The consumers are NOT within a fixed distance of one another: a consumer held up on tile j
@@ -304,20 +358,23 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
                 __nanosleep(100);
                 if (n > (1u << 24)) __trap();
             }
-            if (lane < cn) s_desc[(w0 + lane) & (kDescRing - 1)] = make_int4(cur.tile, cur.unit, cur.meta, cur.pos);
+            if (lane < cn) s_desc[(w0 + lane) & (kDescRing - 1)] = make_int4(cur.tile, cur.unit, cur.meta, cur.len_part);
             __threadfence_block();
             __syncwarp();
             if (lane == 0) sts_volatile(s_ready, w0 + cn);
-            // next window: its stage C now, and stage A + B of the one after it (their loads complete while the consumers
-            // work through the descriptors just published)
+            // shift the pipeline: stage B of the window after next, stage A of a new one, the claim of the one after that
             w0 += cn;
             cur = nxt; cn = nn;
-            if (cn > 0) {
-                stage_c(cur);
-                nn = min(32, n_tiles - (w0 + cn));
-                if (nn > 0) { stage_a(nxt, ra + w0 + cn + lane, lane < nn); stage_b(nxt); }
+            nxt = nx2; nn = n2;
+            if (nn > 0) {
+                stage_b(nxt);
+                n2 = next_window(nx2);
+                if (n2 > 0) prefetch_claim();
+            } else {
+                n2 = 0;
             }
         }
+        if (lane == 0) sts_volatile(s_total, w0);                // the CTA's stream ends here
         return;
     }
 
@@ -327,9 +384,16 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
     const float scale_log2 = A.scale_log2;
     constexpr float kLn2 = 0.6931471805599453f;
 
-    // the tile `it` of the range (CTA-relative) goes to stage it % kDecStages; issued by ONE lane
+    // does tile `it` of the CTA's stream exist?  (waits until the look-up warp has either described it or closed the stream)
+    auto exists = [&](int it) {
+        for (uint32_t n = 0;; ++n) {
+            if (lds_volatile(s_ready) > it) return true;
+            if (lds_volatile(s_total) <= it) return false;
+            if (n > (1u << 27)) __trap();
+        }
+    };
+    // the tile `it` of the stream goes to stage it % kDecStages; issued by ONE lane
     auto issue = [&](int it) {
-        spin_until(s_ready, it + 1);                                // its descriptor has been written
         __threadfence_block();
         const int tile = s_desc[it & (kDescRing - 1)].x;
         const int stage = it % kDecStages;
@@ -343,20 +407,20 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
     if (lane == 0) {                                                // first fill of the ring: consumer w issues tiles w, w + 8
         for (int k = 0; k < kDecChunk; ++k) {
             const int it = warp + k * kDecConsumers;
-            if (it < n_tiles) issue(it);
+            if (exists(it)) issue(it);
         }
     }
 
     uint32_t qa[8][2];                                              // Q fragments of the unit this consumer is in
     int q_unit = -1;
-    float o[16][2];                 // O[head = lane/4][dims nt*8 + col + {0,1}] of the piece being computed
+    float o[16][2];                 // O[head = lane/4][dims nt*8 + col + {0,1}] of the part being accumulated
     float m_run = -INFINITY, l_run = 0.f;
 
-    // PARK: this consumer is done with a part (it has been handed a tile of another one, or the range is exhausted).
+    // PARK: this consumer is done with a part (it has been handed a tile of another one, or the stream is exhausted).
     // Its state goes to the part's parking area; the consumer whose tiles complete the part merges the parked states
     // in consumer order and writes the result.  WHICH tiles a consumer took is decided at run time (whoever is free
     // takes the next chunk), so the fp32 summation order -- the last bits of the result -- can differ from run to run.
-    auto park = [&](int part, int unit, int n_mine, int part_len) {
+    auto park = [&](int part, int unit, int n_mine, int part_len, int4 piece) {
         const int slot = part & (kAccSlots - 1);
         // The parking areas are handed out strictly in part order (part P gets area P mod 2 once part P - 2 is finished):
         // a later part can then never hold an area an earlier part is waiting for, and the earliest unfinished part --
@@ -370,60 +434,63 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
         l_tot += __shfl_xor_sync(kFull, l_tot, 1);
         l_tot += __shfl_xor_sync(kFull, l_tot, 2);
         float *area = s_acc + slot * (kDecConsumers * kMaxGroup * kAccRow);
-        if (hrow < r) {
-            float *row = area + (warp * kMaxGroup + hrow) * kAccRow;
+        float m_new = m_run, l_new = l_tot;
+        if (n_mine < part_len) {                                    // (a consumer that took the whole part keeps it in registers)
+            if (hrow < r) {
+                float *row = area + (warp * kMaxGroup + hrow) * kAccRow;
 #pragma unroll
-            for (int nt = 0; nt < 16; ++nt) *reinterpret_cast<float2 *>(row + nt * 8 + col) = make_float2(o[nt][0], o[nt][1]);
-            if ((lane & 3) == 0) *reinterpret_cast<float2 *>(row + kDim) = make_float2(m_run, l_tot);
-        }
-        __threadfence_block();
-        __syncwarp();
-        int last = 0, mask = 0;
-        if (lane == 0) {
-            atomicOr(s_mask + slot, 1 << warp);
-            __threadfence_block();
-            last = atomicAdd(s_count + slot, n_mine) + n_mine == part_len;
-            if (last) { __threadfence_block(); mask = lds_volatile(s_mask + slot); }
-        }
-        last = __shfl_sync(kFull, last, 0);
-        if (!last) return;
-        mask = __shfl_sync(kFull, mask, 0);
-        // ---- merge the parked states (consumer order) ----
-        float m_new = -INFINITY, l_new = 0.f;
-#pragma unroll
-        for (int nt = 0; nt < 16; ++nt) { o[nt][0] = 0.f; o[nt][1] = 0.f; }
-        if (hrow < r) {
-            for (int w2 = 0; w2 < kDecConsumers; ++w2) {
-                if (!((mask >> w2) & 1)) continue;
-                const float2 ml = *reinterpret_cast<const float2 *>(area + (w2 * kMaxGroup + hrow) * kAccRow + kDim);
-                if (ml.y > 0.f) m_new = fmaxf(m_new, ml.x);
+                for (int nt = 0; nt < 16; ++nt) *reinterpret_cast<float2 *>(row + nt * 8 + col) = make_float2(o[nt][0], o[nt][1]);
+                if ((lane & 3) == 0) *reinterpret_cast<float2 *>(row + kDim) = make_float2(m_run, l_tot);
             }
-            for (int w2 = 0; w2 < kDecConsumers; ++w2) {
-                if (!((mask >> w2) & 1)) continue;
-                const float *row = area + (w2 * kMaxGroup + hrow) * kAccRow;
-                const float2 ml = *reinterpret_cast<const float2 *>(row + kDim);
-                const float wgt = ml.y > 0.f ? fast_exp2(ml.x - m_new) : 0.f;           // empty state: weight 0, never NaN
-                l_new = fmaf(ml.y, wgt, l_new);
+            __threadfence_block();
+            __syncwarp();
+            int last = 0, mask = 0;
+            if (lane == 0) {
+                atomicOr(s_mask + slot, 1 << warp);
+                __threadfence_block();
+                last = atomicAdd(s_count + slot, n_mine) + n_mine == part_len;
+                if (last) { __threadfence_block(); mask = lds_volatile(s_mask + slot); }
+            }
+            last = __shfl_sync(kFull, last, 0);
+            if (!last) return;
+            mask = __shfl_sync(kFull, mask, 0);
+            // ---- merge the parked states (consumer order) ----
+            m_new = -INFINITY; l_new = 0.f;
 #pragma unroll
-                for (int nt = 0; nt < 16; ++nt) {
-                    const float2 a = *reinterpret_cast<const float2 *>(row + nt * 8 + col);
-                    o[nt][0] = fmaf(a.x, wgt, o[nt][0]);
-                    o[nt][1] = fmaf(a.y, wgt, o[nt][1]);
+            for (int nt = 0; nt < 16; ++nt) { o[nt][0] = 0.f; o[nt][1] = 0.f; }
+            if (hrow < r) {
+                for (int w2 = 0; w2 < kDecConsumers; ++w2) {
+                    if (!((mask >> w2) & 1)) continue;
+                    const float2 ml = *reinterpret_cast<const float2 *>(area + (w2 * kMaxGroup + hrow) * kAccRow + kDim);
+                    if (ml.y > 0.f) m_new = fmaxf(m_new, ml.x);
+                }
+                for (int w2 = 0; w2 < kDecConsumers; ++w2) {
+                    if (!((mask >> w2) & 1)) continue;
+                    const float *row = area + (w2 * kMaxGroup + hrow) * kAccRow;
+                    const float2 ml = *reinterpret_cast<const float2 *>(row + kDim);
+                    const float wgt = ml.y > 0.f ? fast_exp2(ml.x - m_new) : 0.f;       // empty state: weight 0, never NaN
+                    l_new = fmaf(ml.y, wgt, l_new);
+#pragma unroll
+                    for (int nt = 0; nt < 16; ++nt) {
+                        const float2 a = *reinterpret_cast<const float2 *>(row + nt * 8 + col);
+                        o[nt][0] = fmaf(a.x, wgt, o[nt][0]);
+                        o[nt][1] = fmaf(a.y, wgt, o[nt][1]);
+                    }
                 }
             }
+            __syncwarp();
         }
-        __syncwarp();
         if (lane == 0) {                                            // the parking area goes to the part after next
             sts_volatile(s_count + slot, 0);
             sts_volatile(s_mask + slot, 0);
             __threadfence_block();
             sts_volatile(s_gen + slot, part / kAccSlots + 1);
         }
-        // ---- o / (m_new, l_new) in registers are the CTA's result for the unit ----
+        // ---- o / (m_new, l_new) in registers are the part's result: the piece's share of the unit ----
         const int seq = unit / n_kv_heads, g = unit - seq * n_kv_heads;
         const int c = s_prefix[seq + 1] - s_prefix[seq];
         const int u0 = s_prefix[seq] * n_kv_heads + g * c, u1 = u0 + c;
-        if (u0 >= ra && u1 <= rb) {                                 // the unit lies inside this CTA's range: final result
+        if (u0 >= piece.y && u1 <= piece.z) {                       // the unit lies inside this piece: final result
             if (hrow < r) {
                 const float inv = l_new > 0.f ? 1.f / l_new : 0.f;
                 uint32_t *dst = reinterpret_cast<uint32_t *>(A.out + ((int64_t)unit * r + hrow) * kDim + col);
@@ -434,13 +501,13 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
             }
             return;
         }
-        // ---- the unit spans CTAs (a7): park the CTA's partial in slot unit + CTA index and arrive on the unit's counter.
-        // Release / acquire through ONE atomic of lane 0: the warp barrier orders the lanes' partial stores before the
-        // acq_rel atomic (cumulative at gpu scope), and the barrier after it orders that acquire before the other lanes'
-        // reads of the other CTAs' slots (ld.global.cg below).  The CTA that arrives last merges in stream order.
-        const int c_first = cr.owner(u0), c_last = cr.owner(u1 - 1);
+        // ---- the unit spans pieces (a7): park the partial in slot unit + piece id and add this part's tiles to the unit's
+        // counter.  Release / acquire through ONE atomic of lane 0: the warp barrier orders the lanes' partial stores
+        // before the acq_rel atomic (cumulative at gpu scope), and the barrier after it orders that acquire before the
+        // other lanes' reads of the other pieces' slots (ld.global.cg below).  Whoever completes the unit merges the
+        // partials in stream order.
         {
-            const int64_t gslot = (int64_t)unit + blockIdx.x;       // unique: unit + CTA index increases along the stream
+            const int64_t gslot = (int64_t)unit + piece.x;          // unique: unit + piece id increases along the stream
             if (hrow < r) {
                 float *po = A.ws_o + (gslot * r + hrow) * kDim + col;
 #pragma unroll
@@ -451,19 +518,23 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
         __syncwarp();
         int old = 0;
         if (lane == 0)
-            asm volatile("atom.acq_rel.gpu.global.add.s32 %0, [%1], 1;" : "=r"(old) : "l"(A.counters + unit) : "memory");
+            asm volatile("atom.acq_rel.gpu.global.add.s32 %0, [%1], %2;" : "=r"(old) : "l"(A.counters + unit), "r"(part_len) : "memory");
         old = __shfl_sync(kFull, old, 0);
         __syncwarp();
-        if (old != c_last - c_first) return;                        // not the last CTA to arrive
+        if (old + part_len != c) return;                            // the unit is not complete yet
         if (lane == 0) A.counters[unit] = 0;                        // restore the zero for the next call
-        const int nseg = c_last - c_first + 1;
+        // the pieces that hold tiles of the unit, in stream order: static pieces id_a..id_b, then tail pieces id_c..id_d
+        int id_a = 0, id_b = -1, id_c = 0, id_d = -1;
+        if (u0 < T0) { id_a = cr.owner(u0); id_b = cr.owner(min(u1, T0) - 1); }
+        if (u1 > T0) { id_c = G + (max(u0, T0) - T0) / kTailChunk; id_d = G + (u1 - 1 - T0) / kTailChunk; }
+        const int n_a = id_b - id_a + 1, nseg = n_a + (id_d - id_c + 1);
+        auto piece_of = [&](int s) { return s < n_a ? id_a + s : id_c + (s - n_a); };
         for (int h = 0; h < r; ++h) {                               // one head at a time: lane = 4 dims
-            const int64_t row0 = ((int64_t)unit + c_first) * r + h; // slot row of CTA c: row0 + (c - c_first) * r
             float m_star = -INFINITY;
             for (int s0 = 0; s0 < nseg; s0 += 32) {
-                const int s = s0 + lane;
+                const int s2 = s0 + lane;
                 float2 ml = make_float2(-INFINITY, 0.f);
-                if (s < nseg) ml = __ldcg(reinterpret_cast<const float2 *>(A.ws_ml + (row0 + (int64_t)s * r) * 2));
+                if (s2 < nseg) ml = __ldcg(reinterpret_cast<const float2 *>(A.ws_ml + (((int64_t)unit + piece_of(s2)) * r + h) * 2));
                 float mm = ml.y > 0.f ? ml.x : -INFINITY;
 #pragma unroll
                 for (int of = 16; of > 0; of >>= 1) mm = fmaxf(mm, __shfl_xor_sync(kFull, mm, of));
@@ -479,8 +550,9 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
                     v[k] = make_float4(0.f, 0.f, 0.f, 0.f);
                     ml[k] = make_float2(-INFINITY, 0.f);
                     if (s0 + k < nseg) {
-                        v[k] = __ldcg(reinterpret_cast<const float4 *>(A.ws_o + (row0 + (int64_t)(s0 + k) * r) * kDim + lane * 4));
-                        ml[k] = __ldcg(reinterpret_cast<const float2 *>(A.ws_ml + (row0 + (int64_t)(s0 + k) * r) * 2));
+                        const int64_t row = ((int64_t)unit + piece_of(s0 + k)) * r + h;
+                        v[k] = __ldcg(reinterpret_cast<const float4 *>(A.ws_o + row * kDim + lane * 4));
+                        ml[k] = __ldcg(reinterpret_cast<const float2 *>(A.ws_ml + row * 2));
                     }
                 }
 #pragma unroll
@@ -502,23 +574,29 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
     };
 
     int part = -1, unit = 0, n_mine = 0, part_len = 0;              // the part this consumer is accumulating
+    int4 piece = make_int4(0, 0, 0, 0);                             // ... and the piece it belongs to (id, begin, end)
 #pragma unroll 1
     while (true) {
         int cidx = 0;
         if (lane == 0) cidx = atomicAdd(s_claim, 1);
         cidx = __shfl_sync(kFull, cidx, 0);
         const int it0 = cidx * kDecChunk;
-        if (lane == 0) sts_volatile(s_pos + warp, it0 < n_tiles ? it0 : 0x7fffffff);
-        if (it0 >= n_tiles) break;
-        const int it1 = min(it0 + kDecChunk, n_tiles);
+        if (lane == 0) sts_volatile(s_pos + warp, it0);
+        int n_it = 0;                                               // tiles of this claim that exist
+        if (lane == 0) { n_it = exists(it0) ? (exists(it0 + 1) ? 2 : 1) : 0; }
+        n_it = __shfl_sync(kFull, n_it, 0);
+        if (n_it == 0) {
+            if (lane == 0) sts_volatile(s_pos + warp, 0x7fffffff);
+            break;
+        }
 #pragma unroll 1
-        for (int it = it0; it < it1; ++it) {
-            spin_until(s_ready, it + 1);                            // (the look-up warp runs far ahead: rarely taken)
+        for (int it = it0; it < it0 + n_it; ++it) {
             __threadfence_block();
             const int4 d = s_desc[it & (kDescRing - 1)];
             if ((d.z >> 8) != part) {                               // a tile of another part: park the state of the old one
-                if (part >= 0) park(part, unit, n_mine, part_len);
+                if (part >= 0) park(part, unit, n_mine, part_len, piece);
                 part = d.z >> 8; unit = d.y; n_mine = 0; part_len = d.w;
+                piece = s_part[part & (kPartRing - 1)];
 #pragma unroll
                 for (int nt = 0; nt < 16; ++nt) { o[nt][0] = 0.f; o[nt][1] = 0.f; }
                 m_run = -INFINITY; l_run = 0.f;
@@ -593,10 +671,19 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
             // engine's writes by the proxy fence) ----
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             __syncwarp();
-            if (lane == 0 && it + kDecStages < n_tiles) issue(it + kDecStages);
+            if (lane == 0 && exists(it + kDecStages)) issue(it + kDecStages);
         }
     }
-    if (part >= 0) park(part, unit, n_mine, part_len);
+    if (part >= 0) park(part, unit, n_mine, part_len, piece);
+    // ---- the last CTA out restores the tail counter's zero for the next call (every CTA's look-up warp has made its last
+    // claim before its consumers see the end of the stream) ----
+    if (warp == 0 && lane == 0) {
+        const int done = atomicAdd(done_ctr, 1);
+        if (done == G - 1) {
+            *tail_ctr = 0;
+            *done_ctr = 0;
+        }
+    }
 }
 
 }  // namespace sparrow

@@ -180,6 +180,18 @@ def check_sparse_step(eng, wl, h=None, idx=None, check_summ=True, out_idx=None) 
     return stats
 
 
+def assert_same_result(out_a: torch.Tensor, out_b: torch.Tensor, what: str, lse_a=None, lse_b=None):
+    """Two runs of the decode on the same inputs.  The kernel hands its tiles to whichever warp is free, so the fp32
+    summation order is timing-dependent: the two bf16 outputs may differ in the last bit (never more: the sums differ
+    by fp32 rounding only), the lse by fp32 rounding.  Everything integer (page lists, counts) must be identical."""
+    a, b = out_a.float(), out_b.float()
+    tol = 2.0 ** -7 * torch.maximum(a.abs(), b.abs()) + 1e-6            # one bf16 step (2^-8 relative) with slack for a carry
+    bad = (a - b).abs() > tol
+    assert not bad.any(), f"{what}: {int(bad.sum())} outputs differ by more than a bf16 step between two runs"
+    if lse_a is not None:
+        assert (lse_a - lse_b).abs().max().item() <= 2e-5, f"{what}: lse differs between two runs"
+
+
 def check_dense(eng, wl, h=None, idx=None) -> dict:
     h = h or wl.host()
     idx = (np.asarray(h["seq_index"]) if "seq_index" in h else np.arange(wl.n_seq)) if idx is None else np.asarray(idx)

@@ -9,7 +9,7 @@ import torch
 import oracle
 from paper_2606_08446_b200 import workloads as W
 
-from parity_util import check_dense, check_sparse_step, check_summaries, check_outputs, sub_host
+from parity_util import assert_same_result, check_dense, check_sparse_step, check_summaries, check_outputs, sub_host
 
 pytestmark = pytest.mark.gpu
 DEV = "cuda"
@@ -146,7 +146,8 @@ def test_select_is_repeatable_and_graph_capturable():
             g.replay()
     st.synchronize()
     torch.cuda.synchronize()
-    assert torch.equal(eng.sel_pages, ref_sel) and torch.equal(eng.out, ref_out)
+    assert torch.equal(eng.sel_pages, ref_sel)                 # the selection is exact and reproducible
+    assert_same_result(eng.out, ref_out, "graph replay")      # the attention to within the last bf16 bit (run-time tile hand-out)
     check_sparse_step(eng, wl)
 
 
@@ -166,7 +167,7 @@ def test_step_host_entry_matches_device_path():
     B.sparrow_step_host(hb.block, ids.numel(), True, wl.k_cache, wl.v_cache, eng.summaries, wl.page_table,
                         eng.sched, eng.max_sel, wl.sm_scale, out_h, scratch, eng.shape)
     assert B.sparrow_last_launch_count() == 3                 # summarize, select, decode (merge fused in the decode launch)
-    assert torch.equal(out_h, eng.out.cpu())
+    assert_same_result(out_h, eng.out.cpu(), "host-buffer entry vs device path")
     check_summaries(eng.summaries, wl.host(), ids.numpy(), nv.numpy())
 
 

@@ -8,7 +8,7 @@ import torch
 import oracle
 from paper_2606_08446_b200 import workloads as W
 
-from parity_util import check_outputs, check_selection, check_summaries
+from parity_util import assert_same_result, check_outputs, check_selection, check_summaries
 
 pytestmark = pytest.mark.gpu
 DEV = "cuda"
@@ -80,7 +80,7 @@ def test_rollout_eager_every_step_matches_oracle_and_graph_replay_is_bitwise_equ
     st.synchronize()
     torch.cuda.synchronize()
     assert wl2.seq_lens.cpu().tolist() == [L + T for L in LENS]
-    assert torch.equal(out2, out) and torch.equal(lse2, lse)
+    assert_same_result(out2, out, "rollout as one CUDA graph vs step by step", lse2, lse)
     assert torch.equal(wl2.k_cache, wl.k_cache) and torch.equal(eng2.summaries, eng.summaries)
 
 
