@@ -501,11 +501,65 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
             }
             return;
         }
-        // ---- the unit spans pieces (a7): park the partial in slot unit + piece id and add this part's tiles to the unit's
-        // counter.  Release / acquire through ONE atomic of lane 0: the warp barrier orders the lanes' partial stores
-        // before the acq_rel atomic (cumulative at gpu scope), and the barrier after it orders that acquire before the
-        // other lanes' reads of the other pieces' slots (ld.global.cg below).  Whoever completes the unit merges the
-        // partials in stream order.
+        // ---- the unit spans pieces (a7).  The pieces that hold tiles of the unit, in stream order: static pieces id_a..id_b,
+        // then tail pieces id_c..id_d; piece p's partial lives in slot unit + p of the workspace.
+        int id_a = 0, id_b = -1, id_c = 0, id_d = -1;
+        if (u0 < T0) { id_a = cr.owner(u0); id_b = cr.owner(min(u1, T0) - 1); }
+        if (u1 > T0) { id_c = G + (max(u0, T0) - T0) / kTailChunk; id_d = G + (u1 - 1 - T0) / kTailChunk; }
+        const int n_a = id_b - id_a + 1, nseg = n_a + (id_d - id_c + 1);
+        auto piece_of = [&](int s) { return s < n_a ? id_a + s : id_c + (s - n_a); };
+        // FAST PATH: if every other piece of the unit has already been counted, this part completes the unit: fold the others'
+        // partials into the registers and write the result -- one acquire load and one round trip for the rows, instead of
+        // store -> release atomic -> load -> store (four dependent trips, all at the very end of a CTA's stream, where they
+        // are the launch's tail: the piece that ends a CTA's range is usually the LAST of its unit to finish, its neighbour
+        // having started with it).
+        {
+            int cur = 0;
+            if (lane == 0) asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(cur) : "l"(A.counters + unit) : "memory");
+            cur = __shfl_sync(kFull, cur, 0);
+            __syncwarp();                                           // orders lane 0's acquire before the other lanes' loads
+            if (cur + part_len == c) {
+                float m_f = m_new, l_f = l_new;
+                for (int s2 = 0; s2 < nseg; ++s2) {
+                    const int pid = piece_of(s2);
+                    if (pid == piece.x) continue;
+                    float2 ml2 = make_float2(-INFINITY, 0.f);
+                    const int64_t row = ((int64_t)unit + pid) * r + (hrow < r ? hrow : 0);
+                    if (hrow < r) ml2 = __ldcg(reinterpret_cast<const float2 *>(A.ws_ml + row * 2));
+                    const bool has = ml2.y > 0.f;                   // (an empty partial contributes nothing, never NaN)
+                    const float m2 = has ? fmaxf(m_f, ml2.x) : m_f;
+                    const float w_old = has ? fast_exp2(m_f - m2) : 1.f, w_new = has ? fast_exp2(ml2.x - m2) : 0.f;   // own part empty: exp2(-inf) = 0
+#pragma unroll
+                    for (int half = 0; half < 2; ++half) {          // the row in two halves: 8 loads in flight per lane (register budget)
+                        float2 v[8];
+#pragma unroll
+                        for (int nt = 0; nt < 8; ++nt)
+                            v[nt] = has ? __ldcg(reinterpret_cast<const float2 *>(A.ws_o + row * kDim + col + (half * 8 + nt) * 8)) : make_float2(0.f, 0.f);
+#pragma unroll
+                        for (int nt = 0; nt < 8; ++nt) {
+                            o[half * 8 + nt][0] = fmaf(v[nt].x, w_new, o[half * 8 + nt][0] * w_old);
+                            o[half * 8 + nt][1] = fmaf(v[nt].y, w_new, o[half * 8 + nt][1] * w_old);
+                        }
+                    }
+                    l_f = fmaf(ml2.y, w_new, l_f * w_old);
+                    m_f = m2;
+                }
+                if (hrow < r) {
+                    const float inv = l_f > 0.f ? 1.f / l_f : 0.f;
+                    uint32_t *dst = reinterpret_cast<uint32_t *>(A.out + ((int64_t)unit * r + hrow) * kDim + col);
+#pragma unroll
+                    for (int nt = 0; nt < 16; ++nt) dst[nt * 4] = pack_bf16(o[nt][0] * inv, o[nt][1] * inv);
+                    if (A.lse && (lane & 3) == 0)
+                        A.lse[(int64_t)unit * r + hrow] = l_f > 0.f ? (m_f + log2f(l_f)) * kLn2 : -INFINITY;
+                }
+                if (lane == 0) A.counters[unit] = 0;                // restore the zero for the next call (nobody else is left to touch it)
+                return;
+            }
+        }
+        // SLOW PATH: park the partial in slot unit + piece id and add this part's tiles to the unit's counter.  Release /
+        // acquire through ONE atomic of lane 0: the warp barrier orders the lanes' partial stores before the acq_rel atomic
+        // (cumulative at gpu scope), and the barrier after it orders that acquire before the other lanes' reads of the other
+        // pieces' slots (ld.global.cg below).  Whoever completes the unit merges the partials in stream order.
         {
             const int64_t gslot = (int64_t)unit + piece.x;          // unique: unit + piece id increases along the stream
             if (hrow < r) {
@@ -523,53 +577,58 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
         __syncwarp();
         if (old + part_len != c) return;                            // the unit is not complete yet
         if (lane == 0) A.counters[unit] = 0;                        // restore the zero for the next call
-        // the pieces that hold tiles of the unit, in stream order: static pieces id_a..id_b, then tail pieces id_c..id_d
-        int id_a = 0, id_b = -1, id_c = 0, id_d = -1;
-        if (u0 < T0) { id_a = cr.owner(u0); id_b = cr.owner(min(u1, T0) - 1); }
-        if (u1 > T0) { id_c = G + (max(u0, T0) - T0) / kTailChunk; id_d = G + (u1 - 1 - T0) / kTailChunk; }
-        const int n_a = id_b - id_a + 1, nseg = n_a + (id_d - id_c + 1);
-        auto piece_of = [&](int s) { return s < n_a ? id_a + s : id_c + (s - n_a); };
-        for (int h = 0; h < r; ++h) {                               // one head at a time: lane = 4 dims
-            float m_star = -INFINITY;
-            for (int s0 = 0; s0 < nseg; s0 += 32) {
-                const int s2 = s0 + lane;
-                float2 ml = make_float2(-INFINITY, 0.f);
-                if (s2 < nseg) ml = __ldcg(reinterpret_cast<const float2 *>(A.ws_ml + (((int64_t)unit + piece_of(s2)) * r + h) * 2));
-                float mm = ml.y > 0.f ? ml.x : -INFINITY;
+        // One pass in stream order, four heads at once (lane = 4 dims of each): the rows and (m, l) pairs of two pieces
+        // and four heads are requested together and folded into running (m, l, o) per head, so a unit that spans two
+        // pieces -- the usual case -- costs ONE round trip to the L2.  (Head by head with the maxima first it was 2 r
+        // dependent round trips, ~9 us at r = 5, all of it at the very end of the launch: traced, profiles/r2_decode.md.)
+        constexpr int kSegs = 2, kHeads = 4;                        // heads in groups of four: 8 rows + 8 pairs in flight per lane
+        for (int h0 = 0; h0 < r; h0 += kHeads) {
+            float4 acc[kHeads];
+            float m_acc[kHeads], l_acc[kHeads];
 #pragma unroll
-                for (int of = 16; of > 0; of >>= 1) mm = fmaxf(mm, __shfl_xor_sync(kFull, mm, of));
-                m_star = fmaxf(m_star, mm);
-            }
-            float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-            float l_star = 0.f;
-            for (int s0 = 0; s0 < nseg; s0 += 4) {                   // four partial rows requested together
-                float4 v[4];
-                float2 ml[4];
+            for (int h = 0; h < kHeads; ++h) { acc[h] = make_float4(0.f, 0.f, 0.f, 0.f); m_acc[h] = -INFINITY; l_acc[h] = 0.f; }
+            for (int s0 = 0; s0 < nseg; s0 += kSegs) {
+                float4 v[kHeads][kSegs];
+                float2 ml[kHeads][kSegs];
 #pragma unroll
-                for (int k = 0; k < 4; ++k) {
-                    v[k] = make_float4(0.f, 0.f, 0.f, 0.f);
-                    ml[k] = make_float2(-INFINITY, 0.f);
-                    if (s0 + k < nseg) {
-                        const int64_t row = ((int64_t)unit + piece_of(s0 + k)) * r + h;
-                        v[k] = __ldcg(reinterpret_cast<const float4 *>(A.ws_o + row * kDim + lane * 4));
-                        ml[k] = __ldcg(reinterpret_cast<const float2 *>(A.ws_ml + row * 2));
+                for (int k = 0; k < kSegs; ++k) {
+                    const bool on = s0 + k < nseg;
+                    const int64_t row0 = ((int64_t)unit + piece_of(on ? s0 + k : s0)) * r + h0;
+#pragma unroll
+                    for (int h = 0; h < kHeads; ++h) {
+                        v[h][k] = make_float4(0.f, 0.f, 0.f, 0.f);
+                        ml[h][k] = make_float2(-INFINITY, 0.f);
+                        if (on && h0 + h < r) {
+                            v[h][k] = __ldcg(reinterpret_cast<const float4 *>(A.ws_o + (row0 + h) * kDim + lane * 4));
+                            ml[h][k] = __ldcg(reinterpret_cast<const float2 *>(A.ws_ml + (row0 + h) * 2));
+                        }
                     }
                 }
 #pragma unroll
-                for (int k = 0; k < 4; ++k) {
-                    const float wgt = ml[k].y > 0.f ? fast_exp2(ml[k].x - m_star) : 0.f;   // empty partial: weight 0, never NaN
-                    l_star = fmaf(ml[k].y, wgt, l_star);
-                    acc.x = fmaf(v[k].x, wgt, acc.x); acc.y = fmaf(v[k].y, wgt, acc.y);
-                    acc.z = fmaf(v[k].z, wgt, acc.z); acc.w = fmaf(v[k].w, wgt, acc.w);
+                for (int k = 0; k < kSegs; ++k) {
+#pragma unroll
+                    for (int h = 0; h < kHeads; ++h) {
+                        if (!(ml[h][k].y > 0.f)) continue;              // empty partial (or no such piece / head): contributes nothing, never NaN
+                        const float m_new2 = fmaxf(m_acc[h], ml[h][k].x);
+                        const float w_old = fast_exp2(m_acc[h] - m_new2), w_new = fast_exp2(ml[h][k].x - m_new2);   // first piece: w_old = exp2(-inf) = 0
+                        l_acc[h] = fmaf(ml[h][k].y, w_new, l_acc[h] * w_old);
+                        acc[h].x = fmaf(v[h][k].x, w_new, acc[h].x * w_old); acc[h].y = fmaf(v[h][k].y, w_new, acc[h].y * w_old);
+                        acc[h].z = fmaf(v[h][k].z, w_new, acc[h].z * w_old); acc[h].w = fmaf(v[h][k].w, w_new, acc[h].w * w_old);
+                        m_acc[h] = m_new2;
+                    }
                 }
             }
-            const float inv = l_star > 0.f ? 1.f / l_star : 0.f;
-            uint2 pk;
-            pk.x = pack_bf16(acc.x * inv, acc.y * inv);
-            pk.y = pack_bf16(acc.z * inv, acc.w * inv);
-            *reinterpret_cast<uint2 *>(A.out + ((int64_t)unit * r + h) * kDim + lane * 4) = pk;
-            if (A.lse && lane == 0)
-                A.lse[(int64_t)unit * r + h] = l_star > 0.f ? (m_star + log2f(l_star)) * kLn2 : -INFINITY;
+#pragma unroll
+            for (int h = 0; h < kHeads; ++h) {
+                if (h0 + h >= r) break;
+                const float inv = l_acc[h] > 0.f ? 1.f / l_acc[h] : 0.f;
+                uint2 pk;
+                pk.x = pack_bf16(acc[h].x * inv, acc[h].y * inv);
+                pk.y = pack_bf16(acc[h].z * inv, acc[h].w * inv);
+                *reinterpret_cast<uint2 *>(A.out + ((int64_t)unit * r + h0 + h) * kDim + lane * 4) = pk;
+                if (A.lse && lane == 0)
+                    A.lse[(int64_t)unit * r + h0 + h] = l_acc[h] > 0.f ? (m_acc[h] + log2f(l_acc[h])) * kLn2 : -INFINITY;
+            }
         }
     };
 
