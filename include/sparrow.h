@@ -134,8 +134,9 @@ int sparrow_select(const void *q, const void *summaries, const int32_t *page_tab
  * is fused into the same launch (one kernel per call).  The K/V tiles are fetched by TMA: each call encodes
  * two tensor maps over the pools on the host (cuTensorMapEncodeTiled, a few microseconds) and passes them by value,
  * so the call stays asynchronous and graph-capturable.  Reproducibility: the page tiles are handed to the CTA's warps at
- * run time, so the fp32 summation order can differ between two calls on the same inputs -- out may differ in the last
- * bf16 bit, lse by fp32 rounding; nothing else varies. */
+ * run time, so the running maximum under which a probability is rounded to bf16, and the fp32 summation order, can
+ * differ between two calls on the same inputs -- the two outs agree to the arithmetic's own error (about 1e-3 absolute
+ * for unit-variance V, the distance of either from an exact evaluation), lse to fp32 rounding; nothing else varies. */
 int sparrow_sparse_decode(const void *q, const void *k_cache, const void *v_cache, const int32_t *page_table,
                           const int32_t *seq_lens, const int32_t *sel_pages, int32_t max_sel,
                           const int32_t *sel_count, void *out, float *lse, float sm_scale,

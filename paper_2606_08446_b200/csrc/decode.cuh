@@ -26,9 +26,10 @@
 // ~50 saturated-HBM latencies; the per-warp finish times spread with sigma ~7 us on a 90 us launch and the kernel
 // ends with the slowest of 1184 warps.  Handing the tiles out inside the CTA brings the warps of a CTA to within 2 us
 // of one another (traced).  What remains is the spread BETWEEN SMs (equal pieces end +-15 % apart), see DESIGN.md.
-// The price of run-time hand-out: which tiles a consumer sums is timing-dependent, so the fp32 summation order, and
-// with it the last bit of a bf16 output, can differ from call to call (the page lists, counts and everything integer
-// are exact and reproducible).
+// The price of run-time hand-out: which tiles a consumer sums is timing-dependent, so the running maximum under which a
+// probability is rounded to bf16 (2^-9 relative per term) and the fp32 summation order differ from call to call: two
+// calls agree to the arithmetic's own error (~1e-3 absolute on these inputs, the size of either call's distance from the
+// fp64 oracle), not bit for bit.  The page lists, counts, lse to fp32 rounding, and everything integer are reproducible.
 // The whole GQA group (r <= 8 query heads) is processed together, so each K/V byte is read from HBM once.
 //
 // Shared layout of a tile: 32 rows of 128 B, row = (token, half of the head dim), 16-byte chunk index XOR (row & 7) --
@@ -419,7 +420,7 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
     // PARK: this consumer is done with a part (it has been handed a tile of another one, or the stream is exhausted).
     // Its state goes to the part's parking area; the consumer whose tiles complete the part merges the parked states
     // in consumer order and writes the result.  WHICH tiles a consumer took is decided at run time (whoever is free
-    // takes the next chunk), so the fp32 summation order -- the last bits of the result -- can differ from run to run.
+    // takes the next chunk), so the result can differ from run to run within the arithmetic's error (see the file header).
     auto park = [&](int part, int unit, int n_mine, int part_len, int4 piece) {
         const int slot = part & (kAccSlots - 1);
         // The parking areas are handed out strictly in part order (part P gets area P mod 2 once part P - 2 is finished):

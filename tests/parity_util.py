@@ -181,13 +181,15 @@ def check_sparse_step(eng, wl, h=None, idx=None, check_summ=True, out_idx=None) 
 
 
 def assert_same_result(out_a: torch.Tensor, out_b: torch.Tensor, what: str, lse_a=None, lse_b=None):
-    """Two runs of the decode on the same inputs.  The kernel hands its tiles to whichever warp is free, so the fp32
-    summation order is timing-dependent: the two bf16 outputs may differ in the last bit (never more: the sums differ
-    by fp32 rounding only), the lse by fp32 rounding.  Everything integer (page lists, counts) must be identical."""
+    """Two runs of the decode on the same inputs.  The kernel hands its tiles to whichever warp is free, so which tiles a
+    warp sums is timing-dependent: the running maximum under which a probability is rounded to bf16 (2^-9 relative per term)
+    and the fp32 summation order differ between two runs.  Both runs are valid evaluations, each within the arithmetic's own
+    error of the exact result (the oracle gate: max-abs 3e-3), so they agree to about that error -- not bit for bit.
+    Everything integer (page lists, counts) must be identical; the lse is summed in fp32 and agrees to fp32 rounding."""
     a, b = out_a.float(), out_b.float()
-    tol = 2.0 ** -7 * torch.maximum(a.abs(), b.abs()) + 1e-6            # one bf16 step (2^-8 relative) with slack for a carry
+    tol = 2.0 ** -7 * torch.maximum(a.abs(), b.abs()) + 1.5e-3
     bad = (a - b).abs() > tol
-    assert not bad.any(), f"{what}: {int(bad.sum())} outputs differ by more than a bf16 step between two runs"
+    assert not bad.any(), f"{what}: {int(bad.sum())} outputs differ by more than the arithmetic's error between two runs"
     if lse_a is not None:
         assert (lse_a - lse_b).abs().max().item() <= 2e-5, f"{what}: lse differs between two runs"
 

@@ -1,6 +1,6 @@
 """GPU parity of the rollout loop (``-m gpu``): sparrow_append (+ summarize on page fill) ->
 sparrow_select -> sparrow_sparse_decode for T steps with the lengths on the device, eagerly (every step checked
-against the oracle's rollout) and as ONE CUDA graph (bitwise equal to the eager run)."""
+against the oracle's rollout) and as ONE CUDA graph (page lists and counts identical to the eager run, outputs equal to within the arithmetic's error: the decode hands tiles out at run time)."""
 import numpy as np
 import pytest
 import torch
@@ -32,7 +32,7 @@ def _bits(t):
     return t.contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
 
 
-def test_rollout_eager_every_step_matches_oracle_and_graph_replay_is_bitwise_equal():
+def test_rollout_eager_every_step_matches_oracle_and_graph_replay_agrees():
     wl, eng, qs, ks, vs = _setup()
     h0 = wl.host()
     osched = oracle.Schedule.from_spec(SCHED)
