@@ -59,7 +59,7 @@ constexpr int kDecStages = SPARROW_DEC_STAGES;                  // CTA-wide ring
 constexpr int kStageBytes = 2 * kTileBytes;                     // K tile + V tile = 8 KiB
 constexpr int kDecRingBytes = kDecStages * kStageBytes;         // 128 KiB
 constexpr int kDecChunk = 2;                                    // tiles per claim (kDecConsumers x kDecChunk = the ring: every consumer's tiles are in flight)
-static_assert(kDecConsumers * kDecChunk == kDecStages, "a claim's tiles must be in the ring when it is taken");
+static_assert(kDecConsumers * kDecChunk <= kDecStages, "the tiles of every consumer's claim are in the ring together");
 constexpr int kMaxGroup = 8;                                    // r <= 8 (rows 0..7 of the m16 tile)
 #ifndef SPARROW_DEC_MAXSEQ
 #define SPARROW_DEC_MAXSEQ 4096
@@ -68,7 +68,11 @@ constexpr int kDecMaxSeq = SPARROW_DEC_MAXSEQ;                  // prefix table 
 constexpr int kDecGrid = 148;                                   // persistent: one CTA per B200 SM (fewer SMs: fewer CTAs)
 constexpr int kAccRow = kDim + 4;                               // one parked head: o[128] | m | l | pad
 constexpr int kAccSlots = 2;                                    // parts (the CTA's share of a unit) being parked at once
-constexpr int kDecAccBytes = kAccSlots * kDecConsumers * kMaxGroup * kAccRow * 4;   // [slot][consumer][head][kAccRow]
+#ifndef SPARROW_DEC_ACC_GROUP
+#define SPARROW_DEC_ACC_GROUP kMaxGroup
+#endif
+constexpr int kAccGroup = SPARROW_DEC_ACC_GROUP;                   // heads a parking area has room for
+constexpr int kDecAccBytes = kAccSlots * kDecConsumers * kAccGroup * kAccRow * 4;   // [slot][consumer][head][kAccRow]
 constexpr int kDescRing = 256;                                  // per-tile descriptors the look-up warp runs ahead by
 constexpr int kPartRing = 512;                                  // per-part records (piece id, piece bounds) kept beside them
 constexpr int kDecDescBytes = kDescRing * 16 + kPartRing * 16;
@@ -175,6 +179,12 @@ template <bool kDense>
 __global__ void __launch_bounds__(kDecThreads, 1)
 decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v)
 {
+    // the tensor maps are kernel parameters, not data of the kernel before this one: fetch them into the descriptor cache now,
+    // so that the first TMA copy (on the launch's critical path: DESIGN.md 6.3, "ramp") does not start with that miss
+    if (threadIdx.x == 0) {
+        asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&tm_k)) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&tm_v)) : "memory");
+    }
     chain_wait();
     extern __shared__ __align__(1024) uint8_t smem[];
     float *s_acc = reinterpret_cast<float *>(smem + kDecRingBytes);                           // [slot][consumer][head][kAccRow]
@@ -313,16 +323,29 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
 
         // The windows of the CTA's stream, in order: those of the static piece, then one per tail piece taken.  The claim of
         // a tail piece is requested one window before it is needed (its round trip to the L2 is never waited for).
-        int sp = ra;                                             // next tile of the static piece not yet in a window
+        // The static piece is walked LAST PART FIRST when its last unit runs on into the next CTA's piece: [p_tail, rb), then
+        // [ra, p_tail).  The neighbour starts with the other half of that unit, so both halves -- and the cross-piece merge
+        // (a7), several dependent round trips -- are done early in the launch instead of forming every CTA's tail; what a
+        // CTA ends with is a unit that lies inside its piece and is written straight to `out`.
+        int p_tail = ra;
+        if (rb > ra) {
+            const int seq = seq_of(rb - 1), base = s_prefix[seq], c = s_prefix[seq + 1] - base;
+            const int g = (rb - 1 - base * n_kv_heads) / c;
+            const int u0 = base * n_kv_heads + g * c;            // the unit that holds the piece's last tile is tiles [u0, u0 + c)
+            if (u0 > ra && u0 + c > rb) p_tail = u0;
+        }
+        int sp = p_tail, seg_end = rb;                           // next tile of the static piece not yet in a window; end of the segment being walked
+        bool wrapped = p_tail == ra;                             // the second segment [ra, p_tail) has been entered (or does not exist)
         int j_next = -1;                                         // lane 0: tail piece claimed ahead (-1: none requested yet)
         auto prefetch_claim = [&]() {
-            if (sp >= rb && lane == 0 && j_next < 0) j_next = atomicAdd(tail_ctr, 1);
+            if (sp >= seg_end && wrapped && lane == 0 && j_next < 0) j_next = atomicAdd(tail_ctr, 1);
         };
         auto next_window = [&](Lookup &m) -> int {               // opens the next window (look-up stage A); returns its tiles, 0 = none
             int p0, n, id, cb, ce;
-            if (sp < rb) {
-                p0 = sp; n = min(32, rb - sp); id = (int)blockIdx.x; cb = ra; ce = rb;
+            if (sp < seg_end) {
+                p0 = sp; n = min(32, seg_end - sp); id = (int)blockIdx.x; cb = ra; ce = rb;
                 sp += n;
+                if (sp == seg_end && !wrapped) { wrapped = true; sp = ra; seg_end = p_tail; }
             } else {
                 prefetch_claim();
                 const int j = __shfl_sync(kFull, j_next, 0);
@@ -385,17 +408,24 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
     const float scale_log2 = A.scale_log2;
     constexpr float kLn2 = 0.6931471805599453f;
 
-    // does tile `it` of the CTA's stream exist?  (waits until the look-up warp has either described it or closed the stream)
-    auto exists = [&](int it) {
+    // Does tile `it` of the CTA's stream exist?  Warp-uniform (every lane calls it and keeps the same cached bounds): the
+    // look-up warp runs hundreds of tiles ahead, so the shared-memory words it publishes are re-read only when the cached
+    // bound is reached -- and the fence that makes the descriptors behind a new bound visible is paid there, not per tile.
+    int ready_seen = 0;                                             // descriptors [0, ready_seen) are published and visible to this warp
+    int total_seen = 0x7fffffff;                                    // the length of the CTA's stream, once this warp has seen it
+    auto exists = [&](int it) -> bool {
+        if (it < ready_seen) return true;
+        if (it >= total_seen) return false;
         for (uint32_t n = 0;; ++n) {
-            if (lds_volatile(s_ready) > it) return true;
-            if (lds_volatile(s_total) <= it) return false;
+            const int rd = lds_volatile(s_ready);
+            if (rd > it) { __threadfence_block(); ready_seen = rd; return true; }
+            const int tt = lds_volatile(s_total);
+            if (tt <= it) { total_seen = tt; return false; }
             if (n > (1u << 27)) __trap();
         }
     };
-    // the tile `it` of the stream goes to stage it % kDecStages; issued by ONE lane
+    // the tile `it` of the stream goes to stage it % kDecStages; issued by ONE lane (after exists(it) returned true)
     auto issue = [&](int it) {
-        __threadfence_block();
         const int tile = s_desc[it & (kDescRing - 1)].x;
         const int stage = it % kDecStages;
         const uint32_t bar = full_u32 + 8 * stage, dst = ring_u32 + stage * kStageBytes;
@@ -405,11 +435,9 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
         tma_box(dst, &tm_k, 0, row, bar);
         tma_box(dst + kTileBytes, &tm_v, 0, row, bar);
     };
-    if (lane == 0) {                                                // first fill of the ring: consumer w issues tiles w, w + 8
-        for (int k = 0; k < kDecChunk; ++k) {
-            const int it = warp + k * kDecConsumers;
-            if (exists(it)) issue(it);
-        }
+    for (int it = warp; it < kDecStages; it += kDecConsumers) {     // first fill of the ring: consumer w issues tiles w, w + 8, ...
+        const bool ex = exists(it);
+        if (ex && lane == 0) issue(it);
     }
 
     uint32_t qa[8][2];                                              // Q fragments of the unit this consumer is in
@@ -434,11 +462,11 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
         float l_tot = l_run;
         l_tot += __shfl_xor_sync(kFull, l_tot, 1);
         l_tot += __shfl_xor_sync(kFull, l_tot, 2);
-        float *area = s_acc + slot * (kDecConsumers * kMaxGroup * kAccRow);
+        float *area = s_acc + slot * (kDecConsumers * kAccGroup * kAccRow);
         float m_new = m_run, l_new = l_tot;
         if (n_mine < part_len) {                                    // (a consumer that took the whole part keeps it in registers)
             if (hrow < r) {
-                float *row = area + (warp * kMaxGroup + hrow) * kAccRow;
+                float *row = area + (warp * kAccGroup + hrow) * kAccRow;
 #pragma unroll
                 for (int nt = 0; nt < 16; ++nt) *reinterpret_cast<float2 *>(row + nt * 8 + col) = make_float2(o[nt][0], o[nt][1]);
                 if ((lane & 3) == 0) *reinterpret_cast<float2 *>(row + kDim) = make_float2(m_run, l_tot);
@@ -462,12 +490,12 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
             if (hrow < r) {
                 for (int w2 = 0; w2 < kDecConsumers; ++w2) {
                     if (!((mask >> w2) & 1)) continue;
-                    const float2 ml = *reinterpret_cast<const float2 *>(area + (w2 * kMaxGroup + hrow) * kAccRow + kDim);
+                    const float2 ml = *reinterpret_cast<const float2 *>(area + (w2 * kAccGroup + hrow) * kAccRow + kDim);
                     if (ml.y > 0.f) m_new = fmaxf(m_new, ml.x);
                 }
                 for (int w2 = 0; w2 < kDecConsumers; ++w2) {
                     if (!((mask >> w2) & 1)) continue;
-                    const float *row = area + (w2 * kMaxGroup + hrow) * kAccRow;
+                    const float *row = area + (w2 * kAccGroup + hrow) * kAccRow;
                     const float2 ml = *reinterpret_cast<const float2 *>(row + kDim);
                     const float wgt = ml.y > 0.f ? fast_exp2(ml.x - m_new) : 0.f;       // empty state: weight 0, never NaN
                     l_new = fmaf(ml.y, wgt, l_new);
@@ -642,16 +670,13 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
         cidx = __shfl_sync(kFull, cidx, 0);
         const int it0 = cidx * kDecChunk;
         if (lane == 0) sts_volatile(s_pos + warp, it0);
-        int n_it = 0;                                               // tiles of this claim that exist
-        if (lane == 0) { n_it = exists(it0) ? (exists(it0 + 1) ? 2 : 1) : 0; }
-        n_it = __shfl_sync(kFull, n_it, 0);
+        const int n_it = exists(it0) ? (exists(it0 + 1) ? 2 : 1) : 0;   // tiles of this claim that exist
         if (n_it == 0) {
             if (lane == 0) sts_volatile(s_pos + warp, 0x7fffffff);
             break;
         }
 #pragma unroll 1
         for (int it = it0; it < it0 + n_it; ++it) {
-            __threadfence_block();
             const int4 d = s_desc[it & (kDescRing - 1)];
             if ((d.z >> 8) != part) {                               // a tile of another part: park the state of the old one
                 if (part >= 0) park(part, unit, n_mine, part_len, piece);
@@ -731,7 +756,8 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
             // engine's writes by the proxy fence) ----
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             __syncwarp();
-            if (lane == 0 && exists(it + kDecStages)) issue(it + kDecStages);
+            const bool more = exists(it + kDecStages);
+            if (more && lane == 0) issue(it + kDecStages);
         }
     }
     if (part >= 0) park(part, unit, n_mine, part_len, piece);
