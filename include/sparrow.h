@@ -228,6 +228,12 @@ const char *sparrow_strerror(int status);   /* static string; for SPARROW_ERR_CU
 int sparrow_version(void);
 /* Kernels launched by the most recent entry-point call on this thread (for gpu_launches accounting). */
 int sparrow_last_launch_count(void);
+/* Tracing build only (compiled with -DSPARROW_TRACE: `python -m paper_2606_08446_b200.build --trace`): the select and
+ * decode kernels drop %globaltimer stamps per CTA / warp into `buffer`, a DEVICE array of 65536 x 8 64-bit words the
+ * caller zeroes (layout: csrc/common.cuh); NULL switches the stamps off.  Synchronous (a symbol copy).  The normal build
+ * carries no stamps and returns SPARROW_ERR_UNSUPPORTED.  Used by paper_2606_08446_b200/trace.py for the timelines under
+ * profiles/. */
+int sparrow_trace_set(void *buffer);
 
 #ifdef __cplusplus
 }

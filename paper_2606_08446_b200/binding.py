@@ -13,7 +13,8 @@ from typing import Optional
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libsparrow_b200.so")
+# SPARROW_B200_LIB names another build of this same library (the tracing build, libsparrow_b200_trace.so: build.py --trace)
+LIB_PATH = os.environ.get("SPARROW_B200_LIB") or os.path.join(_HERE, "libsparrow_b200.so")
 if not os.path.exists(LIB_PATH):
     raise ImportError(
         f"{LIB_PATH} is missing: build it with `python -m paper_2606_08446_b200.build` "
@@ -92,6 +93,7 @@ _SIGS = {
     "sparrow_strerror": (C.c_char_p, [C.c_int]),
     "sparrow_version": (C.c_int, []),
     "sparrow_last_launch_count": (C.c_int, []),
+    "sparrow_trace_set": (C.c_int, [_vp]),
 }
 for _name, (_res, _args) in _SIGS.items():
     _fn = getattr(_lib, _name)          # AttributeError here = the library does not export a declared symbol
@@ -125,6 +127,13 @@ def _by(x):
 
 def sparrow_version() -> int:
     return _lib.sparrow_version()
+
+
+def sparrow_trace_set(buffer: Optional[torch.Tensor]):
+    """Tracing build only: point the kernels' stamps at `buffer` (int64 [65536][8] on the device, zeroed) or switch them off."""
+    if buffer is not None:
+        assert buffer.is_cuda and buffer.dtype == torch.int64 and buffer.numel() >= 65536 * 8 and buffer.is_contiguous()
+    _check(_lib.sparrow_trace_set(_ptr(buffer)), "sparrow_trace_set")
 
 
 def sparrow_last_launch_count() -> int:

@@ -34,13 +34,20 @@ def stale() -> bool:
     return any(os.path.getmtime(s) > t for s in sources())
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if force or stale():
-        cmd = [NVCC, *FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-o", LIB, os.path.join(CSRC, "api.cu")]
+LIB_TRACE = os.path.join(_HERE, "libsparrow_b200_trace.so")
+
+
+def build(force: bool = False, verbose: bool = False, trace: bool = False) -> str:
+    """trace=True: the tracing build (-DSPARROW_TRACE, csrc/common.cuh) beside the normal one; loaded through
+    SPARROW_B200_LIB (binding.py), used by trace.py."""
+    lib = LIB_TRACE if trace else LIB
+    if force or trace or stale():
+        cmd = [NVCC, *FLAGS, *(["-DSPARROW_TRACE"] if trace else []), *(["-Xptxas", "-v"] if verbose else []), "-o", lib,
+               os.path.join(CSRC, "api.cu")]
         subprocess.check_call(cmd)
-    return LIB
+    return lib
 
 
 if __name__ == "__main__":
     import sys
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, trace="--trace" in sys.argv))

@@ -335,6 +335,17 @@ int select_impl(const void *q, const void *summaries, const int32_t *page_table,
 extern "C" {
 
 int sparrow_version(void) { return 100; }
+
+int sparrow_trace_set(void *buffer)
+{
+#ifdef SPARROW_TRACE
+    cudaError_t e = cudaMemcpyToSymbol(sparrow::g_trace, &buffer, sizeof(buffer));
+    return e == cudaSuccess ? SPARROW_OK : cuda_fail(e, "cudaMemcpyToSymbol(g_trace)");
+#else
+    (void)buffer;
+    return SPARROW_ERR_UNSUPPORTED;      // this build carries no stamps: build with -DSPARROW_TRACE (build.py --trace)
+#endif
+}
 int sparrow_last_launch_count(void) { return g_launches; }
 
 const char *sparrow_strerror(int status)

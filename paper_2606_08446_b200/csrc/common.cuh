@@ -125,6 +125,32 @@ __host__ __device__ inline SeqPlan make_plan(const SchedDev &s, int64_t L)
     return pl;
 }
 
+// ---- tracing build (-DSPARROW_TRACE; `python -m paper_2606_08446_b200.build --trace`, read by paper_2606_08446_b200/trace.py):
+// the kernels drop %globaltimer stamps into a caller-provided buffer [65536 slots][8] of 64-bit words (sparrow_trace_set).
+// In the normal build SPARROW_TR() is empty and the kernels carry no trace of it.
+//   select_kernel:  slot = linear CTA index; 0 start, 1 prologue done, 2 summary stream done (warp 0), 3 CTA barrier passed,
+//                   4 arrival atomic done, 5 top-k done (last CTA of a unit), 7 keys in shared memory, 6 radix select done
+//   decode_kernel:  slot = 60000 + CTA; 0 start, 1 dependency wait over, 2 prefix table built, 3 look-up warp finished,
+//                   4 first tile landed;   slot = 56000 + 9 x CTA + warp; 0 warp entry, 1 warp exit
+#ifdef SPARROW_TRACE
+__device__ unsigned long long *g_trace = nullptr;
+__device__ __forceinline__ unsigned long long trace_now()
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+    return t;
+}
+#define SPARROW_TR(slot, k)                                                       \
+    do {                                                                          \
+        const unsigned long long t__ = sparrow::trace_now();                      \
+        unsigned long long *g__ = sparrow::g_trace;                               \
+        if (g__) g__[(size_t)(slot) * 8 + (k)] = t__;                             \
+    } while (0)
+#else
+#define SPARROW_TR(slot, k) do { } while (0)
+#endif
+constexpr int kTraceSlots = 65536, kTraceDecodeCta = 60000, kTraceDecodeWarp = 56000;
+
 // ---------------------------------------------------------------- small device helpers ----
 __device__ __forceinline__ float bf16_lo(uint32_t x) { return __uint_as_float(x << 16); }
 __device__ __forceinline__ float bf16_hi(uint32_t x) { return __uint_as_float(x & 0xffff0000u); }

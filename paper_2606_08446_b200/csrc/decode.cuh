@@ -185,7 +185,10 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
         asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&tm_k)) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&tm_v)) : "memory");
     }
+    if (threadIdx.x == 0) SPARROW_TR(kTraceDecodeCta + blockIdx.x, 0);
+    if ((threadIdx.x & 31) == 0) SPARROW_TR(kTraceDecodeWarp + blockIdx.x * (kDecThreads / 32) + (threadIdx.x >> 5), 0);
     chain_wait();
+    if (threadIdx.x == 0) SPARROW_TR(kTraceDecodeCta + blockIdx.x, 1);
     extern __shared__ __align__(1024) uint8_t smem[];
     float *s_acc = reinterpret_cast<float *>(smem + kDecRingBytes);                           // [slot][consumer][head][kAccRow]
     int4 *s_desc = reinterpret_cast<int4 *>(smem + kDecRingBytes + kDecAccBytes);             // [kDescRing] per-tile descriptors
@@ -247,6 +250,7 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
         __syncthreads();
     }
     const int T = s_prefix[n_seq] * n_kv_heads;                  // tiles of the whole batch
+    if (threadIdx.x == 0) SPARROW_TR(kTraceDecodeCta + blockIdx.x, 2);
     if (T == 0) return;
     // The stream is cut into PIECES.  Its first kStatic part is split evenly: CTA b owns piece b, a contiguous range.  The
     // rest, the tail, is cut into pieces of kTailChunk tiles that the CTAs take from one global counter as they run out of
@@ -399,6 +403,7 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
             }
         }
         if (lane == 0) sts_volatile(s_total, w0);                // the CTA's stream ends here
+        if (lane == 0) { SPARROW_TR(kTraceDecodeCta + blockIdx.x, 3); SPARROW_TR(kTraceDecodeWarp + blockIdx.x * (kDecThreads / 32) + warp, 1); }
         return;
     }
 
@@ -703,6 +708,7 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
             // been requested (before that, "the phase of the other parity" reads as complete).
             spin_until(s_issued + stage, it);
             mbar_wait(full_u32 + 8 * stage, (it / kDecStages) & 1);
+            if (it == 0 && lane == 0) SPARROW_TR(kTraceDecodeCta + blockIdx.x, 4);
             const uint32_t kb = ring_u32 + stage * kStageBytes;
             const uint32_t vb = kb + kTileBytes;
             if (valid < kPage) {
@@ -770,6 +776,7 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
             *done_ctr = 0;
         }
     }
+    if (lane == 0) SPARROW_TR(kTraceDecodeWarp + blockIdx.x * (kDecThreads / 32) + warp, 1);
 }
 
 }  // namespace sparrow

@@ -98,8 +98,9 @@ __device__ __forceinline__ float dot8(const float (&qr)[8], const uint4 v, float
 //      are emitted in ascending page order -- the lower-index tie-break (R10) falls out of the scan order.
 __device__ __forceinline__ void unit_topk(const SeqPlan &pl, const float *__restrict__ ws, int32_t *__restrict__ out, int max_sel,
                                           int32_t *__restrict__ sel_count_slot, uint32_t *s_keys, int *s_hist, int *s_warp,
-                                          uint32_t *s_red, int *s_bcast)
+                                          uint32_t *s_red, int *s_bcast, int tr_slot)
 {
+    (void)tr_slot;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int n_pages = pl.n_pages;
     uint32_t kmin = 0xffffffffu, kmax = 0u;
@@ -126,6 +127,7 @@ __device__ __forceinline__ void unit_topk(const SeqPlan &pl, const float *__rest
         kmax = max(kmax, s_red[kSelWarps + w2]);
     }
 
+    if (threadIdx.x == 0) SPARROW_TR(tr_slot, 7);
     uint32_t prefix = 0, mask = 0;
     int need_eq = 0;                 // how many keys of the final class are taken (lowest page index first, R10)
     if (pl.k > 0) {
@@ -173,6 +175,7 @@ __device__ __forceinline__ void unit_topk(const SeqPlan &pl, const float *__rest
         }
     }
 
+    if (threadIdx.x == 0) SPARROW_TR(tr_slot, 6);
     // Ordered compaction.  Thread t owns the contiguous pages [t*ipt, (t+1)*ipt).  One scan carries both counts: the
     // pages a thread surely emits (low 16 bits) and its members of the final class (high bits).
     const int ipt = (n_pages + kSelThreads - 1) / kSelThreads;
@@ -224,6 +227,9 @@ select_kernel(const uint16_t *__restrict__ q, const uint16_t *__restrict__ summa
               int n_q_heads, int n_kv_heads, int max_pages, int pages_per_cta)
 {
     chain_entry();
+    const int tr_slot = (blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;   // tracing build only
+    (void)tr_slot;
+    if (threadIdx.x == 0) SPARROW_TR(tr_slot, 0);
     extern __shared__ uint32_t s_keys[];                 // [n_pages] (phase B only)
     __shared__ float s_q[2][kDim];                       // [0] = Q- (pairs with min), [1] = Q+ (pairs with max)
     __shared__ int s_hist[256];
@@ -263,6 +269,7 @@ select_kernel(const uint16_t *__restrict__ q, const uint16_t *__restrict__ summa
         s_q[1][tid] = qp;
     }
     __syncthreads();
+    if (threadIdx.x == 0) SPARROW_TR(tr_slot, 1);
     const SeqPlan pl = s_plan;
     int32_t *out = sel_pages + ((int64_t)seq * n_kv_heads + g) * max_sel;
 
@@ -399,12 +406,14 @@ select_kernel(const uint16_t *__restrict__ q, const uint16_t *__restrict__ summa
         }
     }
 
+    if (threadIdx.x == 0) SPARROW_TR(tr_slot, 2);
     // ------------------------------------------------ last CTA of this (sequence, kv-head)? --------
     // Release / acquire through ONE atomic of thread 0 instead of a fence by every thread: the CTA barrier orders the
     // warps' score stores before thread 0's acq_rel atomic (cumulative at gpu scope), and in the last CTA the barrier
     // after it orders that acquire before the other threads' reads of the scores (ld.global.cg below).
     __syncthreads();
     if (tid == 0) {
+        SPARROW_TR(tr_slot, 3);
         int32_t *ctr = counters + seq * n_kv_heads + g;
         int old;
         asm volatile("atom.acq_rel.gpu.global.add.s32 %0, [%1], 1;" : "=r"(old) : "l"(ctr) : "memory");
@@ -413,10 +422,15 @@ select_kernel(const uint16_t *__restrict__ q, const uint16_t *__restrict__ summa
         s_bcast[0][0] = last;
     }
     __syncthreads();
+    if (tid == 0) SPARROW_TR(tr_slot, 4);
     if (!s_bcast[0][0]) return;
 
     // ---------------------------------------------------------------- phase B: top-k of the unit ----
-    unit_topk(pl, ws, out, max_sel, g == 0 ? sel_count + seq : nullptr, s_keys, s_hist, s_warp, s_red, &s_bcast[0][0]);
+    unit_topk(pl, ws, out, max_sel, g == 0 ? sel_count + seq : nullptr, s_keys, s_hist, s_warp, s_red, &s_bcast[0][0], tr_slot);
+#ifdef SPARROW_TRACE
+    __syncthreads();
+    if (tid == 0) SPARROW_TR(tr_slot, 5);
+#endif
 }
 
 }  // namespace sparrow

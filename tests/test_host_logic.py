@@ -33,6 +33,16 @@ def test_library_exports_every_declared_symbol(B):
     assert declared == set(B.EXPORTS), "binding and header disagree"
 
 
+def test_normal_build_carries_no_trace_stamps(B):
+    """sparrow_trace_set is declared for every build; only the tracing build (build.py --trace) implements it."""
+    lib = ctypes.CDLL(B.LIB_PATH)
+    lib.sparrow_trace_set.argtypes = [ctypes.c_void_p]
+    assert lib.sparrow_trace_set(None) == -2          # SPARROW_ERR_UNSUPPORTED, and no CUDA call was made
+    import subprocess
+    sass = subprocess.run(["cuobjdump", "-sass", B.LIB_PATH], capture_output=True, text=True).stdout
+    assert "globaltimer" not in sass.lower(), "the normal build reads %globaltimer: trace stamps leaked into it"
+
+
 def test_built_for_sm100a_with_tensor_and_async_copy_instructions(B):
     import subprocess
     sass = subprocess.run(["cuobjdump", "-sass", B.LIB_PATH], capture_output=True, text=True).stdout
