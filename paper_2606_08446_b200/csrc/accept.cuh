@@ -4,8 +4,8 @@
 //   PAPER.md:95            approximated from the top-20 tokens and logprobs each policy returns per position (R23:
 //                          the sum runs over the tokens present in BOTH lists; a token missing from a list adds 0)
 //   PAPER.md:101, :119     tokens are grouped by position in 2K bins; the statistic is the 5-percentile per bin
-// Two kernels.  alpha: a warp stages the lists of four positions in shared memory with coalesced loads, then per
-// position lane = Q entry scans P's row with 16-byte broadcast reads.  Quantile: exact nearest-rank selection (rank ceil(quantile * count)) per
+// Two kernels.  alpha: a CTA stages the lists of 128 positions in shared memory with coalesced loads, then ONE THREAD per
+// position compares its 20 x 20 ids out of registers.  Quantile: exact nearest-rank selection (rank ceil(quantile * count)) per
 // bin by a 3-pass radix select (11 + 11 + 10 bits) over the fp32 bit patterns (alpha >= 0: bit order = value order);
 // each pass is one streaming histogram launch (block-private shared-memory histograms of all bins) and one tiny
 // scan launch that picks the digit, keeps the remaining rank and clears the histogram for the next pass / call.
@@ -17,59 +17,67 @@ namespace sparrow {
 constexpr int kAccDigits = 2048;                  // histogram bins per pass (11 bits)
 constexpr int kAccThreads = 256;
 
-// One warp per kAccPosPerWarp consecutive positions.  Their slices of the four [n_pos][top_n] arrays are contiguous, so
-// the warp stages them with full-width coalesced loads (all issued before the first use: ~1.5 KiB in flight per
-// warp) into shared memory rows padded to 32 entries.  Then, per position, lane = Q entry: it scans P's row four ids
-// per 16-byte broadcast read.  (One position per warp with 80-byte loads was latency bound, a 20-step shuffle loop
-// shuffle bound; __match_any_sync pairing and a thread-per-position outward search were slower still.)
-// min(p, q) = exp(min(log p, log q)): one exp per matched pair.
-constexpr int kAccPosPerWarp = 4;
+// One thread per position.  The slices of the four [n_pos][top_n] arrays that belong to the CTA's kAlphaThreads consecutive
+// positions are contiguous, so the CTA stages them with full-width coalesced loads (all issued before the first use) into
+// shared-memory rows of odd stride (conflict-free when thread t reads row t).  A thread then holds P's ids in registers and
+// walks Q's: top_n x top_n compares on the integer pipe, ~25 warp instructions per position.  (Round 1's form -- a warp
+// per four positions, lane = Q entry, P's row scanned with broadcast reads -- spent 214 warp instructions per position and
+// was issue-bound at 0.21 of the copy peak on its bytes; lane-per-entry leaves 12 of 32 lanes idle and pays a shuffle
+// reduction per position.)  min(p, q) = exp(min(log p, log q)): one exp per matched pair.  The ids of a list are distinct
+// (it is a top-N list).
+constexpr int kAlphaThreads = 128;
+constexpr int kAlphaMaxTop = 32;
 
-__global__ void __launch_bounds__(kAccThreads)
+template <int kTop>                                  // kTop = 20: the paper's lists; 32: any top_n <= 32
+__global__ void __launch_bounds__(kAlphaThreads)
 accept_alpha_kernel(const int32_t *__restrict__ ids_p, const float *__restrict__ logp_p, const int32_t *__restrict__ ids_q,
-                    const float *__restrict__ logp_q, int64_t n_pos, int top_n, float *__restrict__ alpha)
+                    const float *__restrict__ logp_q, int64_t n_pos, int top_n, int vec16, float *__restrict__ alpha)
 {
-    constexpr int kW = kAccThreads / 32, kP = kAccPosPerWarp;
-    __shared__ __align__(16) int s_idp[kW][kP][32];
-    __shared__ int s_idq[kW][kP][32];
-    __shared__ float s_lp[kW][kP][32], s_lq[kW][kP][32];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int64_t pos0 = ((int64_t)blockIdx.x * kW + warp) * kP;
-    if (pos0 >= n_pos) return;
-    const int n_here = (int)min((int64_t)kP, n_pos - pos0);
+    extern __shared__ int s_acc_all[];               // [4][kAlphaThreads][stride]: ids_p | ids_q | logp_p | logp_q
+    const int stride = top_n | 1;
+    int *s_idp = s_acc_all, *s_idq = s_idp + kAlphaThreads * stride;
+    float *s_lp = reinterpret_cast<float *>(s_idq + kAlphaThreads * stride), *s_lq = s_lp + kAlphaThreads * stride;
+    const int64_t pos0 = (int64_t)blockIdx.x * kAlphaThreads;
+    const int n_here = (int)min((int64_t)kAlphaThreads, n_pos - pos0);
     const int total = n_here * top_n;
-#pragma unroll
-    for (int k = 0; k < kP; ++k) s_idp[warp][k][lane] = -1;              // padding never matches a token id
-    __syncwarp();
     const int64_t g0 = pos0 * top_n;
-#pragma unroll
-    for (int e0 = 0; e0 < kP * 32; e0 += 32) {
-        const int e = e0 + lane;
-        if (e < total) {
-            const int k = e / top_n, i = e - k * top_n;
-            s_idp[warp][k][i] = ids_p[g0 + e];
-            s_idq[warp][k][i] = ids_q[g0 + e];
-            s_lp[warp][k][i] = logp_p[g0 + e];
-            s_lq[warp][k][i] = logp_q[g0 + e];
+    if (vec16) {                                                     // top_n a multiple of 4 and the four arrays 16-byte aligned (host)
+        // 16-byte loads: the CTA's slice starts on a 16-byte boundary (128 x top_n words) and a row is a whole number of
+        // quads, so a quad never straddles two positions; all four arrays' loads of a quad are issued before its stores
+        const int qpr = top_n >> 2;                                  // quads per row
+        for (int f = threadIdx.x; f < (total >> 2); f += kAlphaThreads) {
+            const int k = f / qpr, at = k * stride + ((f - k * qpr) << 2);
+            const int4 a = __ldg(reinterpret_cast<const int4 *>(ids_p + g0) + f), b = __ldg(reinterpret_cast<const int4 *>(ids_q + g0) + f);
+            const float4 c = __ldg(reinterpret_cast<const float4 *>(logp_p + g0) + f), d = __ldg(reinterpret_cast<const float4 *>(logp_q + g0) + f);
+            s_idp[at] = a.x; s_idp[at + 1] = a.y; s_idp[at + 2] = a.z; s_idp[at + 3] = a.w;
+            s_idq[at] = b.x; s_idq[at + 1] = b.y; s_idq[at + 2] = b.z; s_idq[at + 3] = b.w;
+            s_lp[at] = c.x; s_lp[at + 1] = c.y; s_lp[at + 2] = c.z; s_lp[at + 3] = c.w;
+            s_lq[at] = d.x; s_lq[at + 1] = d.y; s_lq[at + 2] = d.z; s_lq[at + 3] = d.w;
+        }
+    } else {
+        for (int e = threadIdx.x; e < total; e += kAlphaThreads) {   // coalesced: consecutive threads, consecutive words
+            const int k = e / top_n, at = k * stride + (e - k * top_n);
+            s_idp[at] = ids_p[g0 + e];
+            s_idq[at] = ids_q[g0 + e];
+            s_lp[at] = logp_p[g0 + e];
+            s_lq[at] = logp_q[g0 + e];
         }
     }
-    __syncwarp();
-    for (int k = 0; k < n_here; ++k) {
-        float acc = 0.f;
-        if (lane < top_n) {
-            const int idq = s_idq[warp][k][lane];
-            const int4 *row = reinterpret_cast<const int4 *>(s_idp[warp][k]);
-            int j = -1;
-            for (int i = 0; i < top_n; i += 4) {
-                const int4 v = row[i >> 2];
-                j = v.x == idq ? i : (v.y == idq ? i + 1 : (v.z == idq ? i + 2 : (v.w == idq ? i + 3 : j)));
-            }
-            if (j >= 0) acc = expf(fminf(s_lp[warp][k][j], s_lq[warp][k][lane]));
-        }
+    __syncthreads();
+    const int t = threadIdx.x;
+    if (t >= n_here) return;
+    int pid[kTop];
 #pragma unroll
-        for (int of = 16; of > 0; of >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, of);
-        if (lane == 0) alpha[pos0 + k] = acc;
+    for (int k = 0; k < kTop; ++k) pid[k] = k < top_n ? s_idp[t * stride + k] : -1;      // (token ids are >= 0)
+    float acc = 0.f;
+    for (int i = 0; i < top_n; ++i) {
+        const int idq = s_idq[t * stride + i];
+        int j = -1;
+#pragma unroll
+        for (int k = 0; k < kTop; ++k) j = pid[k] == idq ? k : j;
+        if (j >= 0) acc += expf(fminf(s_lp[t * stride + j], s_lq[t * stride + i]));
     }
+    alpha[pos0 + t] = acc;
 }
 
 // per-bin selection state: [0] prefix (key bits fixed so far), [1] mask, [2] remaining rank (1-based, from the
@@ -77,27 +85,42 @@ accept_alpha_kernel(const int32_t *__restrict__ ids_p, const float *__restrict__
 // One streaming pass over (alpha, position) per radix digit: every block keeps a private histogram of ALL bins in
 // shared memory ([n_bins_local][2048] ints; the host cuts the bins into groups of n_bins_local that fit, grid.y =
 // group) and flushes its non-zero counters with global atomics.
-__global__ void __launch_bounds__(kAccThreads)
+constexpr int kHistThreads = 1024;                // one CTA per SM (its histograms fill the shared memory): as many warps as fit
+__global__ void __launch_bounds__(kHistThreads)
 accept_hist_kernel(const float *__restrict__ alpha, const int32_t *__restrict__ positions, int64_t n_pos, int bin_tokens,
                    int n_bins, int bins_per_group, int shift, int digit_bits, const uint32_t *__restrict__ state,
                    int32_t *__restrict__ hist)
 {
     extern __shared__ int s_hist[];                                  // [bins_per_group][kAccDigits]
+    __shared__ uint32_t s_state[64][2];                              // (prefix, mask) of the group's bins (bins_per_group <= 64)
     const int bin0 = blockIdx.y * bins_per_group;
     const int nb = min(bins_per_group, n_bins - bin0);
-    for (int i = threadIdx.x; i < nb * kAccDigits; i += kAccThreads) s_hist[i] = 0;
+    for (int i = threadIdx.x; i < nb * kAccDigits; i += kHistThreads) s_hist[i] = 0;
+    if (threadIdx.x < 2 * nb) s_state[threadIdx.x >> 1][threadIdx.x & 1] = state[(bin0 + (threadIdx.x >> 1)) * 4 + (threadIdx.x & 1)];
     __syncthreads();
     const uint32_t dmask = (1u << digit_bits) - 1u;
-    for (int64_t i = (int64_t)blockIdx.x * kAccThreads + threadIdx.x; i < n_pos; i += (int64_t)gridDim.x * kAccThreads) {
-        int b = positions[i] / bin_tokens;
-        b = (b < 0 ? 0 : (b >= n_bins ? n_bins - 1 : b)) - bin0;
-        if (b < 0 || b >= nb) continue;
-        const uint32_t key = __float_as_uint(alpha[i]);
-        const uint32_t prefix = state[(bin0 + b) * 4 + 0], mask = state[(bin0 + b) * 4 + 1];
-        if ((key & mask) == prefix) atomicAdd(&s_hist[b * kAccDigits + ((key >> shift) & dmask)], 1);
+    const int64_t step = (int64_t)gridDim.x * kHistThreads;
+    constexpr int kU = 4;                                            // independent (position, alpha) loads in flight per thread
+    for (int64_t i0 = (int64_t)blockIdx.x * kHistThreads + threadIdx.x; i0 < n_pos; i0 += kU * step) {
+        int pos[kU];
+        uint32_t key[kU];
+#pragma unroll
+        for (int u = 0; u < kU; ++u) {
+            const int64_t i = i0 + u * step;
+            pos[u] = i < n_pos ? __ldg(positions + i) : -1;
+            key[u] = i < n_pos ? __float_as_uint(__ldg(alpha + i)) : 0u;
+        }
+#pragma unroll
+        for (int u = 0; u < kU; ++u) {
+            if (i0 + u * step >= n_pos) continue;
+            int b = pos[u] / bin_tokens;
+            b = (b < 0 ? 0 : (b >= n_bins ? n_bins - 1 : b)) - bin0;
+            if (b < 0 || b >= nb) continue;
+            if ((key[u] & s_state[b][1]) == s_state[b][0]) atomicAdd(&s_hist[b * kAccDigits + ((key[u] >> shift) & dmask)], 1);
+        }
     }
     __syncthreads();
-    for (int i = threadIdx.x; i < nb * kAccDigits; i += kAccThreads)
+    for (int i = threadIdx.x; i < nb * kAccDigits; i += kHistThreads)
         if (s_hist[i]) atomicAdd(&hist[bin0 * kAccDigits + i], s_hist[i]);
 }
 

@@ -26,7 +26,7 @@ constexpr int kNumSmsB200 = 148;
 struct DevState {
     bool init = false;
     int sms = 0;
-    size_t dyn_decode[2] = {0, 0}, dyn_select[2] = {0, 0}, dyn_hist = 0;
+    size_t dyn_decode[2] = {0, 0}, dyn_select[2] = {0, 0}, dyn_hist = 0, dyn_alpha[2] = {0, 0};
 };
 constexpr int kMaxDevices = 64;
 DevState g_dev[kMaxDevices];
@@ -536,10 +536,20 @@ int sparrow_acceptance(const int32_t *ids_p, const float *logp_p, const int32_t 
     cudaError_t e = cudaMemsetAsync(state, 0, (size_t)n_bins * 4 * sizeof(uint32_t), st);
     if (e != cudaSuccess) return cuda_fail(e, "memset(acceptance state)");
     if (n_pos > 0) {
-        const int64_t per_block = (int64_t)(kAccThreads / 32) * kAccPosPerWarp;
-        const int64_t blocks = (n_pos + per_block - 1) / per_block;
+        const int64_t blocks = (n_pos + kAlphaThreads - 1) / kAlphaThreads;
         if (blocks > 0x7fffffffLL) return SPARROW_ERR_UNSUPPORTED;
-        accept_alpha_kernel<<<(unsigned)blocks, kAccThreads, 0, st>>>(ids_p, logp_p, ids_q, logp_q, n_pos, top_n, alpha);
+        const size_t asmem = (size_t)4 * kAlphaThreads * (top_n | 1) * sizeof(int);
+        const int vec16 = (top_n & 3) == 0 && aligned16(ids_p) && aligned16(ids_q) && aligned16(logp_p) && aligned16(logp_q);
+        int rc_dev = SPARROW_OK;
+        DevState *ds = dev_state(&rc_dev);
+        if (!ds) return rc_dev;
+        if (top_n <= 20) {
+            if ((rc_dev = ensure_dyn_smem(accept_alpha_kernel<20>, asmem, &ds->dyn_alpha[0], "accept_alpha_kernel<20>"))) return rc_dev;
+            accept_alpha_kernel<20><<<(unsigned)blocks, kAlphaThreads, asmem, st>>>(ids_p, logp_p, ids_q, logp_q, n_pos, top_n, vec16, alpha);
+        } else {
+            if ((rc_dev = ensure_dyn_smem(accept_alpha_kernel<kAlphaMaxTop>, asmem, &ds->dyn_alpha[1], "accept_alpha_kernel<32>"))) return rc_dev;
+            accept_alpha_kernel<kAlphaMaxTop><<<(unsigned)blocks, kAlphaThreads, asmem, st>>>(ids_p, logp_p, ids_q, logp_q, n_pos, top_n, vec16, alpha);
+        }
         SPARROW_CHECK_LAUNCH("accept_alpha_kernel");
     }
     // 3-pass radix select per bin over the fp32 bit patterns: bits 31..21, 20..10, 9..0
@@ -555,11 +565,11 @@ int sparrow_acceptance(const int32_t *ids_p, const float *logp_p, const int32_t 
         rc_dev = ensure_dyn_smem(accept_hist_kernel, hsmem, &ds->dyn_hist, "accept_hist_kernel");
         if (rc_dev) return rc_dev;
     }
-    int64_t gx = (n_pos + kAccThreads * 8 - 1) / (kAccThreads * 8);
-    const int64_t gmax = (hsmem > 100 * 1024 ? 1 : 2) * kNumSmsB200;
+    int64_t gx = (n_pos + kHistThreads * 8 - 1) / (kHistThreads * 8);
+    const int64_t gmax = kNumSmsB200;                    // one 1024-thread CTA per SM
     gx = gx < 1 ? 1 : (gx > gmax ? gmax : gx);
     for (int pass = 0; pass < 3; ++pass) {
-        accept_hist_kernel<<<dim3((unsigned)gx, (unsigned)groups), kAccThreads, hsmem, st>>>(
+        accept_hist_kernel<<<dim3((unsigned)gx, (unsigned)groups), kHistThreads, hsmem, st>>>(
             alpha, positions, n_pos, bin_tokens, n_bins, bins_per_group, shifts[pass], bits[pass], state, hist);
         SPARROW_CHECK_LAUNCH("accept_hist_kernel");
         accept_scan_kernel<<<n_bins, kAccThreads, 0, st>>>(hist, state, shifts[pass], bits[pass], pass == 0, quantile, pass == 2,
