@@ -69,6 +69,21 @@ def test_ragged_lengths_all_group_sizes(Hq, Hkv):
     check_dense(eng, wl)
 
 
+@pytest.mark.parametrize("Hq,Hkv,lens,budget", [(8, 2, [33000], 9000), (5, 1, [20000, 17], 6000), (16, 8, [40000, 3, 25000], 20000)])
+def test_units_that_span_many_ctas(Hq, Hkv, lens, budget):
+    """Few, very long units: the decode stream of ONE (sequence, kv-head) unit is cut over tens of CTAs (up to all 148), so
+    the cross-piece merge (a7) folds tens of partials -- its multi-round loop, the last-arriver's register path and the
+    workspace slots unit + piece id -- where the full-size configs only ever see two or three pieces per unit."""
+    sched = W._sched("fixed", 64, 512, fixed_tokens=budget)
+    wl = W.make_workload(n_seq=len(lens), Hq=Hq, Hkv=Hkv, lengths=("list", lens), schedule=sched, seed=Hq * 7 + Hkv, device=DEV,
+                         poison_tail=True, plant=True)
+    eng = _run_sparse(wl, want_scores=True)
+    check_sparse_step(eng, wl)
+    eng.dense_decode()
+    torch.cuda.synchronize()
+    check_dense(eng, wl)
+
+
 @pytest.mark.parametrize("page", [16, 64])
 def test_non_finite_bits_in_unwritten_tails_never_reach_the_output(page):
     """A torch.empty pool or a recycled page leaves arbitrary bit patterns in the rows past L of a sequence's last page
