@@ -247,6 +247,10 @@ select_kernel(const uint16_t *__restrict__ q, const uint16_t *__restrict__ summa
     // Independent global loads first (sequence length, q, the first page-table entries), so that their latencies
     // overlap instead of chaining: only the summary gather depends on them.
     const int L = seq_lens[seq];
+    // A CTA whose slice lies past the sequence's last page has nothing to do (the grid is sized for the longest sequence the
+    // page table allows: at cfg4 half of the 8192 CTAs): it leaves here, after one load, before the query rows, the plan and
+    // the CTA barrier.  (L <= 0: no pages at all; slice 0 still runs on to write the empty list.)
+    if (slice > 0 && (int64_t)cta_page0 << sched.page_log2 >= (int64_t)L) return;
     int phys_cur = 0, phys_nxt = 0;                      // table entries of this warp's chunks i, i+1 (lane = page)
     {
         const int p0 = cta_page0 + warp * kSelPagesPerWarp + lane, p1 = p0 + kSelCtaPagesMin;
