@@ -295,7 +295,13 @@ def run_single(args, cfg, rank, local_rank, world, dev, headline=True) -> dict:
     from paper_2606_08446_b200.engine import SparrowEngine
     base_seed = 1000 * int("".join(ch for ch in cfg if ch.isdigit()) or 0)
     wl = W.make_config(cfg, seed=D.replica_seed(base_seed, rank), device=dev)
-    eng = SparrowEngine(wl, landmark=args.landmark)
+    wl_chk = wl                                          # the packed arrays: what the oracle checks and times against
+    if args.kv_layout == "nhd":                          # the same values in [page][token][kv-head][128] pools (sparrow_shape_t kv_stride_*)
+        import copy
+        wl = copy.copy(wl)
+        wl.k_cache = wl_chk.k_cache.permute(0, 2, 1, 3).contiguous()
+        wl.v_cache = wl_chk.v_cache.permute(0, 2, 1, 3).contiguous()
+    eng = SparrowEngine(wl, landmark=args.landmark, kv_layout=args.kv_layout)
     st = torch.cuda.Stream(device=dev)
     upd = tuple(t.to(dev) for t in W.just_filled_updates(wl))
     with torch.cuda.stream(st):
@@ -317,7 +323,7 @@ def run_single(args, cfg, rank, local_rank, world, dev, headline=True) -> dict:
         ext = [int(lens.argmin()), int(lens.argmax())]
         others = [i for i in np.random.default_rng(2).permutation(wl.n_seq).tolist() if i not in ext]
         idx = list(range(wl.n_seq)) if wl.n_seq <= 64 else ext + others[:16 - len(set(ext))]
-        chk, h = self_check(eng, wl, idx, dense_idx=ext)
+        chk, h = self_check(eng, wl_chk, idx, dense_idx=ext)
 
     def one_step():
         n = 0
@@ -451,6 +457,7 @@ def run_single(args, cfg, rank, local_rank, world, dev, headline=True) -> dict:
         "dtype": "bf16", "data": "synthetic",
         "config": {"workload": cfg, "n_seq": wl.n_seq, "Hq": wl.Hq, "Hkv": wl.Hkv, "head_dim": 128, "page_size": 16,
                    "len_min": int(lens.min()), "len_max": int(lens.max()), "schedule": wl.schedule["kind"], "landmark": args.landmark,
+                   "kv_layout": args.kv_layout,
                    "sink_tokens": wl.schedule["sink_tokens"], "local_tokens": wl.schedule["local_tokens"],
                    "selected_pages_per_seq_mean": float(cnt.mean()), "parallelism": f"replicas x{world} (no collective)",
                    "l2": "inputs larger than L2: %.0f MB touched per step vs 126 MB L2" % ((ab["decode"] + ab["select"]) / 1e6),
@@ -487,15 +494,15 @@ def run_single(args, cfg, rank, local_rank, world, dev, headline=True) -> dict:
     if chk is not None:
         res["self_check"] = chk
     if not args.no_cpu_baseline:
-        n_s = oracle_sample_size(wl, target_s=1.0)
+        n_s = oracle_sample_size(wl_chk, target_s=1.0)
         idx = list(range(n_s))
-        hh = h if (h is not None and set(idx) <= set(h["seq_index"].tolist())) else W.host_subset(wl, idx)
-        dt, dt_dense, cores = time_oracle(wl, hh, idx)
+        hh = h if (h is not None and set(idx) <= set(h["seq_index"].tolist())) else W.host_subset(wl_chk, idx)
+        dt, dt_dense, cores = time_oracle(wl_chk, hh, idx)
         res["cpu_baseline"] = {"value": n_s / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
                                "dense_value": n_s / dt_dense,
                                "sample": f"first {n_s} of {wl.n_seq} sequences of {cfg}: full select + sparse-attention steps, {dt:.3f} s each "
                                          f"(mean over ~6 s of CPU work when one step is short); dense attention on the same sequences {dt_dense:.3f} s"}
-    del eng, wl, scratch
+    del eng, wl, wl_chk, scratch
     torch.cuda.empty_cache()
     return res
 
@@ -895,6 +902,8 @@ def main():
     ap.add_argument("--acceptance", action="store_true", help="time sparrow_acceptance (SURVEY 8(f)-3) instead of the step benchmark")
     ap.add_argument("--landmark", default="minmax", choices=["minmax", "mean"],
                     help="page landmark: per-channel min/max (north_star's default, 512 B) or the mean key (the paper's cost model, 256 B)")
+    ap.add_argument("--kv-layout", default="hnd", choices=["hnd", "nhd"],
+                    help="single-layer configs: K/V pools packed [page][kv-head][token][128] (default) or [page][token][kv-head][128] through the stride fields")
     ap.add_argument("--launch-check", action="store_true", help="only bring up the N ranks, barrier, and print their count (CPU: gloo)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-check", action="store_true", help="skip the oracle self-check before timing")

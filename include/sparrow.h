@@ -61,6 +61,15 @@ typedef struct sparrow_shape {
     int32_t max_pages_per_seq;   /* row stride of page_table */
     int64_t n_phys_pages;        /* pages in the K/V pools */
     int32_t landmark;            /* SPARROW_LANDMARK_MINMAX (0, north_star's default) or SPARROW_LANDMARK_MEAN (1) */
+    /* Strides of the K and V pools in ELEMENTS (both pools share them; the head dim is contiguous): row t of kv-head g of
+     * physical page p starts at p * kv_stride_page + g * kv_stride_head + t * kv_stride_tok.  All three 0 (the default) =
+     * the packed "HND" layout [n_phys_pages][n_kv_heads][page_size][128] this library is tuned for (a (page, kv-head) tile
+     * is contiguous: one TMA box of 32 x 128 B).  "NHD" pools [n_phys_pages][page_size][n_kv_heads][128] (the default of
+     * vLLM / FlashInfer) are kv_stride_page = page_size * n_kv_heads * 128, kv_stride_tok = n_kv_heads * 128,
+     * kv_stride_head = 128.  Each stride must be a multiple of 8 elements (16 bytes), kv_stride_tok >= 128, and rows must
+     * not overlap; strided pools are fetched with one 5-D TMA box per tile instead of a 2-D one.  The summaries keep their
+     * own packed layout either way. */
+    int64_t kv_stride_page, kv_stride_head, kv_stride_tok;
 } sparrow_shape_t;
 
 /* Form of the page landmark (PAPER.md:147 leaves it open; reading R1):

@@ -30,7 +30,8 @@ class SparrowError(RuntimeError):
 
 class sparrow_shape_t(C.Structure):
     _fields_ = [("n_seq", C.c_int32), ("n_q_heads", C.c_int32), ("n_kv_heads", C.c_int32), ("head_dim", C.c_int32),
-                ("page_size", C.c_int32), ("max_pages_per_seq", C.c_int32), ("n_phys_pages", C.c_int64), ("landmark", C.c_int32)]
+                ("page_size", C.c_int32), ("max_pages_per_seq", C.c_int32), ("n_phys_pages", C.c_int64), ("landmark", C.c_int32),
+                ("kv_stride_page", C.c_int64), ("kv_stride_head", C.c_int64), ("kv_stride_tok", C.c_int64)]
 
 
 class sparrow_schedule_t(C.Structure):
@@ -53,8 +54,17 @@ class sparrow_cost_t(C.Structure):
 LANDMARK = {"minmax": 0, "mean": 1}
 
 
-def make_shape(n_seq, n_q_heads, n_kv_heads, max_pages_per_seq, n_phys_pages, head_dim=128, page_size=16, landmark="minmax"):
-    return sparrow_shape_t(n_seq, n_q_heads, n_kv_heads, head_dim, page_size, max_pages_per_seq, n_phys_pages, LANDMARK[landmark])
+def make_shape(n_seq, n_q_heads, n_kv_heads, max_pages_per_seq, n_phys_pages, head_dim=128, page_size=16, landmark="minmax",
+               kv_layout="hnd"):
+    """kv_layout: "hnd" (packed [page][kv-head][token][128], strides left 0), "nhd" ([page][token][kv-head][128]) or a tuple
+    (stride_page, stride_head, stride_tok) in elements."""
+    if kv_layout == "hnd":
+        st = (0, 0, 0)
+    elif kv_layout == "nhd":
+        st = (page_size * n_kv_heads * head_dim, head_dim, n_kv_heads * head_dim)
+    else:
+        st = tuple(int(x) for x in kv_layout)
+    return sparrow_shape_t(n_seq, n_q_heads, n_kv_heads, head_dim, page_size, max_pages_per_seq, n_phys_pages, LANDMARK[landmark], *st)
 
 
 def make_schedule(spec: dict, page_size: int = 0) -> sparrow_schedule_t:

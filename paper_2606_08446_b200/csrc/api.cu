@@ -117,7 +117,29 @@ int check_shape(const sparrow_shape_t *s)
     if (r < 1 || r > kMaxGroup) return SPARROW_ERR_UNSUPPORTED;
     if (s->n_kv_heads > 65535 || s->n_seq > 65535) return SPARROW_ERR_UNSUPPORTED;     // grid.y / grid.z
     if (s->landmark != SPARROW_LANDMARK_MINMAX && s->landmark != SPARROW_LANDMARK_MEAN) return SPARROW_ERR_INVALID_ARG;
+    if (s->kv_stride_page != 0 || s->kv_stride_head != 0 || s->kv_stride_tok != 0) {
+        const int64_t sp = s->kv_stride_page, sh = s->kv_stride_head, stt = s->kv_stride_tok;
+        if (sp <= 0 || sh <= 0 || stt < kDim || (sp & 7) || (sh & 7) || (stt & 7)) return SPARROW_ERR_INVALID_ARG;
+        // rows must not overlap: one of the two nestings token-inside-head (HND-like) or head-inside-token (NHD-like)
+        const bool hnd_like = sh >= stt * s->page_size && sp >= sh * s->n_kv_heads;
+        const bool nhd_like = sh >= kDim && stt >= sh * s->n_kv_heads && sp >= stt * s->page_size;
+        if (!hnd_like && !nhd_like) return SPARROW_ERR_INVALID_ARG;
+    }
     return SPARROW_OK;
+}
+
+// the pools' strides in elements; packed = the default HND layout, whose (page, kv-head) tiles are contiguous
+KvLayout kv_layout(const sparrow_shape_t *s, bool *packed)
+{
+    KvLayout kv;
+    const int64_t P = s->page_size;
+    if (s->kv_stride_page == 0 && s->kv_stride_head == 0 && s->kv_stride_tok == 0) {
+        kv.tok = kDim; kv.head = P * kDim; kv.page = (int64_t)s->n_kv_heads * P * kDim;
+    } else {
+        kv.tok = s->kv_stride_tok; kv.head = s->kv_stride_head; kv.page = s->kv_stride_page;
+    }
+    if (packed) *packed = kv.tok == kDim && kv.head == P * kDim && kv.page == (int64_t)s->n_kv_heads * P * kDim;
+    return kv;
 }
 
 // page_tokens: the shape's page size for the device entry points; 0 = take the schedule's own (host helpers), default 16
@@ -207,14 +229,30 @@ int make_pool_map(CUtensorMap *tm, const void *pool, const sparrow_shape_t *s)
             encode = reinterpret_cast<EncodeTiledFn>(fn);
         }
     }
-    const cuuint64_t rows = (cuuint64_t)s->n_phys_pages * s->n_kv_heads * s->page_size * 2;     // 128-byte rows: (token, half)
-    const cuuint64_t gdim[2] = {64, rows};
-    const cuuint64_t gstride[1] = {128};
-    const cuuint32_t box[2] = {64, (cuuint32_t)(2 * kPage)};
-    const cuuint32_t estr[2] = {1, 1};
-    const CUresult rc = encode(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void *>(pool), gdim, gstride, box, estr,
-                               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    bool packed = true;
+    const KvLayout kv = kv_layout(s, &packed);
+    CUresult rc;
+    if (packed) {
+        const cuuint64_t rows = (cuuint64_t)s->n_phys_pages * s->n_kv_heads * s->page_size * 2;     // 128-byte rows: (token, half)
+        const cuuint64_t gdim[2] = {64, rows};
+        const cuuint64_t gstride[1] = {128};
+        const cuuint32_t box[2] = {64, (cuuint32_t)(2 * kPage)};
+        const cuuint32_t estr[2] = {1, 1};
+        rc = encode(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void *>(pool), gdim, gstride, box, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    } else {
+        // strided pools (sparrow_shape_t kv_stride_*): [page][kv-head][token][half][64] as a 5-D tensor with the caller's
+        // strides; one box = (64 columns, 2 halves, 16 tokens) of one kv-head of one page -- it lands in shared memory in the
+        // same (token, half) row order and 128-byte swizzle as the packed layout's 32 x 64 box
+        const cuuint64_t gdim[5] = {64, 2, (cuuint64_t)s->page_size, (cuuint64_t)s->n_kv_heads, (cuuint64_t)s->n_phys_pages};
+        const cuuint64_t gstride[4] = {128, (cuuint64_t)kv.tok * 2, (cuuint64_t)kv.head * 2, (cuuint64_t)kv.page * 2};
+        const cuuint32_t box[5] = {64, 2, (cuuint32_t)kPage, 1, 1};
+        const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+        rc = encode(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 5, const_cast<void *>(pool), gdim, gstride, box, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    }
     if (rc != CUDA_SUCCESS) {
         snprintf(g_errbuf, sizeof(g_errbuf), "cuTensorMapEncodeTiled failed (CUresult %d)", (int)rc);
         return SPARROW_ERR_CUDA;
@@ -262,6 +300,11 @@ int launch_decode(const void *q, const void *k_cache, const void *v_cache, const
     A.out = (uint16_t *)out; A.lse = lse; A.scale_log2 = sm_scale * 1.4426950408889634f;
     A.n_seq = s->n_seq; A.n_q_heads = s->n_q_heads; A.n_kv_heads = s->n_kv_heads; A.max_pages = s->max_pages_per_seq;
     A.tpp_log2 = s->page_size == 16 ? 0 : (s->page_size == 32 ? 1 : (s->page_size == 64 ? 2 : 3));
+    {
+        bool packed = true;
+        kv_layout(s, &packed);
+        A.strided = packed ? 0 : 1;
+    }
     const int grid = ds->sms < kDecGrid ? ds->sms : kDecGrid;   // one CTA per SM (the partial slots are sized for 148)
     launch_chain(decode_kernel<kDense>, dim3(grid), dim3(kDecThreads), smem, st, A, tm_k, tm_v);
     SPARROW_CHECK_LAUNCH("decode_kernel");
@@ -277,10 +320,10 @@ int summarize_impl(const void *k_cache, void *summaries, const int32_t *page_ids
     if (blocks > 0x7fffffffLL) return SPARROW_ERR_UNSUPPORTED;
     if (s->landmark == SPARROW_LANDMARK_MEAN)
         launch_chain(summarize_mean_kernel, dim3((unsigned)blocks), dim3(kSumWarps * 32), 0, st, (const uint16_t *)k_cache,
-                     (uint16_t *)summaries, page_ids, n_valid, n_update, s->n_kv_heads, s->page_size);
+                     (uint16_t *)summaries, page_ids, n_valid, n_update, s->n_kv_heads, s->page_size, kv_layout(s, nullptr));
     else
         launch_chain(summarize_kernel, dim3((unsigned)blocks), dim3(kSumWarps * 32), 0, st, (const uint16_t *)k_cache,
-                     (uint16_t *)summaries, page_ids, n_valid, n_update, s->n_kv_heads, s->page_size);
+                     (uint16_t *)summaries, page_ids, n_valid, n_update, s->n_kv_heads, s->page_size, kv_layout(s, nullptr));
     SPARROW_CHECK_LAUNCH("summarize_kernel");
     return SPARROW_OK;
 }
@@ -507,7 +550,7 @@ int sparrow_append(const void *k_new, const void *v_new, void *k_cache, void *v_
     const int warps = shape->n_kv_heads < kAppendMaxWarps ? shape->n_kv_heads : kAppendMaxWarps;
     launch_chain(append_kernel, dim3(shape->n_seq), dim3(warps * 32), 0, (cudaStream_t)stream, (const uint16_t *)k_new,
                  (const uint16_t *)v_new, (uint16_t *)k_cache, (uint16_t *)v_cache, (uint16_t *)summaries, page_table, seq_lens,
-                 shape->n_kv_heads, shape->max_pages_per_seq, shape->page_size, shape->landmark);
+                 shape->n_kv_heads, shape->max_pages_per_seq, shape->page_size, shape->landmark, kv_layout(shape, nullptr));
     SPARROW_CHECK_LAUNCH("append_kernel");
     return SPARROW_OK;
 }

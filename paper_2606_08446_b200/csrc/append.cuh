@@ -15,7 +15,7 @@ constexpr int kAppendMaxWarps = 8;                 // warps per CTA; more kv-hea
 __global__ void __launch_bounds__(kAppendMaxWarps * 32)
 append_kernel(const uint16_t *__restrict__ k_new, const uint16_t *__restrict__ v_new, uint16_t *__restrict__ k_cache,
               uint16_t *__restrict__ v_cache, uint16_t *__restrict__ summaries, const int32_t *__restrict__ page_table,
-              int32_t *__restrict__ seq_lens, int n_kv_heads, int max_pages, int page_tokens, int landmark)
+              int32_t *__restrict__ seq_lens, int n_kv_heads, int max_pages, int page_tokens, int landmark, const KvLayout kv)
 {
     chain_entry();
     const int seq = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -26,16 +26,16 @@ append_kernel(const uint16_t *__restrict__ k_new, const uint16_t *__restrict__ v
     if (threadIdx.x == 0) seq_lens[seq] = L + 1;
     const int64_t page = page_table[(int64_t)seq * max_pages + page_l];
     for (int g = warp; g < n_kv_heads; g += blockDim.x >> 5) {
-        const int64_t tile = (page * n_kv_heads + g) * (int64_t)page_tokens * kDim;      // the page's rows, 256 B each
+        const int64_t tile = page * kv.page + g * kv.head;                               // the page's rows, 256 B each, kv.tok elements apart
         const int64_t src = ((int64_t)seq * n_kv_heads + g) * kDim;
         // 256-byte row = 16 lanes x 16 B: lanes 0-15 copy K, lanes 16-31 copy V
         const int c = lane & 15;
         const uint4 val = *reinterpret_cast<const uint4 *>((lane < 16 ? k_new : v_new) + src + c * 8);
-        *reinterpret_cast<uint4 *>((lane < 16 ? k_cache : v_cache) + tile + row * kDim + c * 8) = val;
+        *reinterpret_cast<uint4 *>((lane < 16 ? k_cache : v_cache) + tile + row * kv.tok + c * 8) = val;
         if (row != page_tokens - 1) continue;            // the page is not full yet
         __syncwarp();                                    // the new key row is visible to the whole warp
         if (landmark == SPARROW_LANDMARK_MEAN) {         // mean-key landmark: same device function as summarize_mean_kernel
-            mean_of_page(k_cache + tile, page_tokens, lane, summaries + (page * n_kv_heads + g) * (int64_t)kDim, true);
+            mean_of_page(k_cache + tile, kv.tok, page_tokens, lane, summaries + (page * n_kv_heads + g) * (int64_t)kDim, true);
             continue;
         }
         const int half = lane >> 4;
@@ -45,7 +45,7 @@ append_kernel(const uint16_t *__restrict__ k_new, const uint16_t *__restrict__ v
             uint4 v[8];
 #pragma unroll
             for (int i = 0; i < 8; ++i)                  // rows t0 + 2i + half; coherent loads (the last row was just written)
-                v[i] = __ldcg(reinterpret_cast<const uint4 *>(k_cache + tile + (t0 + 2 * i + half) * kDim + c * 8));
+                v[i] = __ldcg(reinterpret_cast<const uint4 *>(k_cache + tile + (t0 + 2 * i + half) * kv.tok + c * 8));
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
                 mn[0] = bf2_min(mn[0], v[i].x); mx[0] = bf2_max(mx[0], v[i].x);

@@ -17,6 +17,13 @@ constexpr int kTileElems = kPage * kDim;        // one (page, kv-head) K or V ti
 constexpr int kTileBytes = kTileElems * 2;
 constexpr int kSumElems = 2 * kDim;             // one (page, kv-head) summary: min[128] + max[128] = 512 B
 
+// Strides of the K and V pools in elements (sparrow_shape_t kv_stride_*; the head dim is always contiguous): row t of the
+// (page, kv-head) tile is at page * .page + head * .head + t * .tok.  Packed HND (the default): tok = 128, head = P * 128,
+// page = Hkv * P * 128 -- a tile is 4 KiB contiguous.  NHD (vLLM / FlashInfer's default): head = 128, tok = Hkv * 128.
+struct KvLayout {
+    int64_t page, head, tok;
+};
+
 // Schedule passed to kernels by value (no device memory, graph-capturable).
 struct SchedDev {
     int32_t kind, sink_tokens, local_tokens, table_len, bin_tokens;

@@ -132,6 +132,12 @@ __device__ __forceinline__ void tma_box(uint32_t dst, const CUtensorMap *tm, int
     asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
                  ::"r"(dst), "l"(reinterpret_cast<uint64_t>(tm)), "r"(col), "r"(row), "r"(bar) : "memory");
 }
+// The same tile out of a strided pool: box (64 columns, 2 halves, 16 tokens) at (0, 0, first token, kv-head, page) of the 5-D view.
+__device__ __forceinline__ void tma_box5(uint32_t dst, const CUtensorMap *tm, int tok, int head, int page, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %2, %3, %4, %5}], [%6];"
+                 ::"r"(dst), "l"(reinterpret_cast<uint64_t>(tm)), "r"(0), "r"(tok), "r"(head), "r"(page), "r"(bar) : "memory");
+}
 __device__ __forceinline__ int lds_volatile(const int32_t *p)
 {
     int v;
@@ -162,6 +168,7 @@ struct DecodeArgs {
     float scale_log2;
     int n_seq, n_q_heads, n_kv_heads, max_pages;
     int tpp_log2;                // log2 of the 16-token tiles per page (page size 16, 32, 64, 128 -> 0, 1, 2, 3)
+    int strided;                 // the pools are not the packed HND layout: tiles are fetched with 5-D boxes (sparrow_shape_t kv_stride_*)
 };
 
 // The CTA ranges: T tiles over G CTAs, the first `extra` CTAs one tile longer.
@@ -436,9 +443,16 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
         const uint32_t bar = full_u32 + 8 * stage, dst = ring_u32 + stage * kStageBytes;
         sts_volatile(s_issued + stage, it);
         mbar_arrive_expect_tx(bar, kStageBytes);
-        const int row = tile * 2 * kPage;
-        tma_box(dst, &tm_k, 0, row, bar);
-        tma_box(dst + kTileBytes, &tm_v, 0, row, bar);
+        if (!A.strided) {
+            const int row = tile * 2 * kPage;
+            tma_box(dst, &tm_k, 0, row, bar);
+            tma_box(dst + kTileBytes, &tm_v, 0, row, bar);
+        } else {                                                    // tile = ((page * Hkv + head) << tpp_log2) + sub
+            const int sub = tile & ((1 << A.tpp_log2) - 1), ph = tile >> A.tpp_log2;
+            const int page = ph / n_kv_heads, head = ph - page * n_kv_heads;
+            tma_box5(dst, &tm_k, sub * kPage, head, page, bar);
+            tma_box5(dst + kTileBytes, &tm_v, sub * kPage, head, page, bar);
+        }
     };
     for (int it = warp; it < kDecStages; it += kDecConsumers) {     // first fill of the ring: consumer w issues tiles w, w + 8, ...
         const bool ex = exists(it);

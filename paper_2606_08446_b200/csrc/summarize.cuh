@@ -23,7 +23,7 @@ __device__ __forceinline__ uint32_t bf2_max(uint32_t a, uint32_t b)
 __global__ void __launch_bounds__(kSumWarps * 32)
 summarize_kernel(const uint16_t *__restrict__ k_cache, uint16_t *__restrict__ summaries,
                  const int32_t *__restrict__ page_ids, const int32_t *__restrict__ n_valid,
-                 int64_t n_update, int n_kv_heads, int page_tokens)
+                 int64_t n_update, int n_kv_heads, int page_tokens, const KvLayout kv)
 {
     chain_entry();
     const int lane = threadIdx.x & 31;
@@ -35,7 +35,7 @@ summarize_kernel(const uint16_t *__restrict__ k_cache, uint16_t *__restrict__ su
     int valid = n_valid ? n_valid[u] : page_tokens;
     valid = valid < 0 ? 0 : (valid > page_tokens ? page_tokens : valid);
 
-    const uint16_t *src = k_cache + (page * n_kv_heads + g) * (int64_t)page_tokens * kDim;     // page_tokens rows of 256 B
+    const uint16_t *src = k_cache + page * kv.page + g * kv.head;     // page_tokens rows of 256 B, kv.tok elements apart
     const int half = lane >> 4;       // which of the two rows of this load
     const int c = lane & 15;          // 16-byte chunk (8 channels) of the row
 
@@ -47,7 +47,7 @@ summarize_kernel(const uint16_t *__restrict__ k_cache, uint16_t *__restrict__ su
 #pragma unroll
         for (int i = 0; i < 8; ++i) {     // all loads first (8 x 16 B in flight per lane)
             const int t = t0 + 2 * i + half;
-            if (t < valid) v[i] = ldg_stream16(src + t * kDim + c * 8);
+            if (t < valid) v[i] = ldg_stream16(src + t * kv.tok + c * 8);
         }
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
@@ -76,15 +76,15 @@ summarize_kernel(const uint16_t *__restrict__ k_cache, uint16_t *__restrict__ su
 // The definition is the exact mean rounded once (reading R24); the fp32 sum is within (valid + 1) 2^-24 mean|k| of it,
 // so the stored code is that one or, next to a rounding boundary, its neighbour -- the checker's validity band.
 // One warp per (page, kv-head); lane = 4 channels (8 bytes), so a row is one coalesced 256-byte load.
-__device__ __forceinline__ void mean_of_page(const uint16_t *__restrict__ src, int valid, int lane, uint16_t *__restrict__ dst,
-                                             bool coherent)
+__device__ __forceinline__ void mean_of_page(const uint16_t *__restrict__ src, int64_t row_stride, int valid, int lane,
+                                             uint16_t *__restrict__ dst, bool coherent)
 {
     float acc[4] = {0.f, 0.f, 0.f, 0.f};
     for (int t0 = 0; t0 < valid; t0 += kPage) {
         uint2 v[kPage];
 #pragma unroll
         for (int i = 0; i < kPage; ++i) {                // all loads of the tile first
-            const uint2 *p = reinterpret_cast<const uint2 *>(src + (t0 + i) * kDim + lane * 4);
+            const uint2 *p = reinterpret_cast<const uint2 *>(src + (t0 + i) * row_stride + lane * 4);
             if (t0 + i < valid) v[i] = coherent ? __ldcg(p) : __ldg(p);
         }
 #pragma unroll
@@ -106,7 +106,7 @@ __device__ __forceinline__ void mean_of_page(const uint16_t *__restrict__ src, i
 __global__ void __launch_bounds__(kSumWarps * 32)
 summarize_mean_kernel(const uint16_t *__restrict__ k_cache, uint16_t *__restrict__ summaries,
                       const int32_t *__restrict__ page_ids, const int32_t *__restrict__ n_valid,
-                      int64_t n_update, int n_kv_heads, int page_tokens)
+                      int64_t n_update, int n_kv_heads, int page_tokens, const KvLayout kv)
 {
     chain_entry();
     const int lane = threadIdx.x & 31;
@@ -117,8 +117,7 @@ summarize_mean_kernel(const uint16_t *__restrict__ k_cache, uint16_t *__restrict
     const int64_t page = page_ids ? (int64_t)page_ids[u] : u;
     int valid = n_valid ? n_valid[u] : page_tokens;
     valid = valid < 0 ? 0 : (valid > page_tokens ? page_tokens : valid);
-    mean_of_page(k_cache + (page * n_kv_heads + g) * (int64_t)page_tokens * kDim, valid, lane,
-                 summaries + (page * n_kv_heads + g) * (int64_t)kDim, false);
+    mean_of_page(k_cache + page * kv.page + g * kv.head, kv.tok, valid, lane, summaries + (page * n_kv_heads + g) * (int64_t)kDim, false);
 }
 
 }  // namespace sparrow

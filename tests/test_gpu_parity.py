@@ -84,6 +84,43 @@ def test_units_that_span_many_ctas(Hq, Hkv, lens, budget):
     check_dense(eng, wl)
 
 
+@pytest.mark.parametrize("Hq,Hkv,page,landmark", [(8, 2, 16, "minmax"), (5, 1, 16, "minmax"), (16, 8, 64, "minmax"), (8, 2, 32, "mean")])
+def test_strided_nhd_pools_match_the_oracle_and_the_packed_layout(Hq, Hkv, page, landmark):
+    """sparrow_shape_t kv_stride_*: the same K/V values in pools laid out [page][token][kv-head][128] (NHD, the default of
+    vLLM / FlashInfer) go through summarize, select, decode (5-D TMA boxes), the dense entry and append; everything is
+    checked against the oracle (which sees the packed arrays) and the appended caches against the packed run's, bit for bit."""
+    import copy
+    from paper_2606_08446_b200.engine import SparrowEngine
+    lens = [1, 16, 17, 250, 1000, 2049, 4099, 700]
+    sched = W._sched("fixed", 16, 64, fixed_tokens=300)
+    wl = W.make_workload(n_seq=len(lens), Hq=Hq, Hkv=Hkv, lengths=("list", lens), schedule=sched, seed=Hq * 31 + page, device=DEV,
+                         poison_tail=True, plant=True, page_size=page, reserve_tokens=8)
+    nhd = copy.copy(wl)
+    nhd.k_cache = wl.k_cache.permute(0, 2, 1, 3).contiguous()          # [n_phys][P][Hkv][128]
+    nhd.v_cache = wl.v_cache.permute(0, 2, 1, 3).contiguous()
+    nhd.seq_lens = wl.seq_lens.clone()
+    eng = SparrowEngine(nhd, want_scores=(landmark == "minmax"), landmark=landmark, kv_layout="nhd")
+    ref = SparrowEngine(wl, landmark=landmark)
+    for e in (eng, ref):
+        e.summarize_all(); e.step(); e.dense_decode()
+    torch.cuda.synchronize()
+    assert torch.equal(eng.summaries, ref.summaries) and torch.equal(eng.sel_pages, ref.sel_pages) and torch.equal(eng.sel_count, ref.sel_count)
+    if landmark == "minmax":
+        check_sparse_step(eng, wl)
+        check_dense(eng, wl)
+    assert_same_result(eng.out, ref.out, "NHD vs packed", eng.lse, ref.lse)
+    assert_same_result(eng.out_dense, ref.out_dense, "NHD vs packed, dense entry", eng.lse_dense, ref.lse_dense)
+    # rollout side: four appended tokens per sequence land in the same logical rows, and pages that fill get the same summaries
+    for e in (eng, ref):
+        e.reserve(4)
+    qs, ks, vs = W.make_rollout_inputs(wl, 4, seed=9)
+    for t in range(4):
+        eng.append(ks[t], vs[t]); ref.append(ks[t], vs[t])
+    torch.cuda.synchronize()
+    assert torch.equal(nhd.k_cache.permute(0, 2, 1, 3), wl.k_cache) and torch.equal(nhd.v_cache.permute(0, 2, 1, 3), wl.v_cache)
+    assert torch.equal(eng.summaries, ref.summaries) and torch.equal(nhd.seq_lens, wl.seq_lens)
+
+
 @pytest.mark.parametrize("page", [16, 64])
 def test_non_finite_bits_in_unwritten_tails_never_reach_the_output(page):
     """A torch.empty pool or a recycled page leaves arbitrary bit patterns in the rows past L of a sequence's last page

@@ -33,6 +33,14 @@ def test_library_exports_every_declared_symbol(B):
     assert declared == set(B.EXPORTS), "binding and header disagree"
 
 
+def test_stride_validation(B):
+    """sparrow_shape_t kv_stride_*: all zero = packed HND; otherwise 16-byte multiples whose rows do not overlap."""
+    shp = B.make_shape(2, 4, 2, 8, 16, kv_layout=(16 * 2 * 128, 128, 2 * 128))
+    assert B.sparrow_decode_workspace_bytes(shp, 4) > 0                     # a valid NHD description
+    for bad in [(16 * 2 * 128, 128, 128), (16 * 2 * 128 + 4, 128, 256), (0, 128, 256), (4096, 64, 256)]:   # rows overlap / misaligned / zero
+        assert B.sparrow_decode_workspace_bytes(B.make_shape(2, 4, 2, 8, 16, kv_layout=bad), 4) == 0
+
+
 def test_normal_build_carries_no_trace_stamps(B):
     """sparrow_trace_set is declared for every build; only the tracing build (build.py --trace) implements it."""
     lib = ctypes.CDLL(B.LIB_PATH)
