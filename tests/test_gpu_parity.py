@@ -84,6 +84,22 @@ def test_units_that_span_many_ctas(Hq, Hkv, lens, budget):
     check_dense(eng, wl)
 
 
+def test_many_short_sequences():
+    """700 sequences, most of them a few pages long: more sequences than the decode CTA has threads (its prefix table is then
+    built several sequences per thread), units far smaller than a CTA's piece (tens of parts per CTA), many empty slices in
+    the selector's grid, sequences that go dense inside the sparse batch."""
+    rng = np.random.default_rng(11)
+    lens = [int(x) for x in rng.integers(1, 700, size=700)]
+    lens[5], lens[77], lens[699] = 1, 16, 2500
+    sched = W._sched("fixed", 16, 32, fixed_tokens=96)
+    wl = W.make_workload(n_seq=len(lens), Hq=4, Hkv=2, lengths=("list", lens), schedule=sched, seed=4242, device=DEV, poison_tail=True, plant=True)
+    eng = _run_sparse(wl, want_scores=True)
+    check_sparse_step(eng, wl)
+    eng.dense_decode()
+    torch.cuda.synchronize()
+    check_dense(eng, wl)
+
+
 @pytest.mark.parametrize("Hq,Hkv,page,landmark", [(8, 2, 16, "minmax"), (5, 1, 16, "minmax"), (16, 8, 64, "minmax"), (8, 2, 32, "mean")])
 def test_strided_nhd_pools_match_the_oracle_and_the_packed_layout(Hq, Hkv, page, landmark):
     """sparrow_shape_t kv_stride_*: the same K/V values in pools laid out [page][token][kv-head][128] (NHD, the default of
