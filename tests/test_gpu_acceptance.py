@@ -28,7 +28,7 @@ def _run(inp, top_n, bin_tokens, n_bins, quantile):
     return alpha[:n_pos].cpu().numpy(), bq.cpu().numpy(), bc.cpu().numpy()
 
 
-@pytest.mark.parametrize("n_traj,max_len,top_n,bins", [(24, 9000, 20, 6), (3, 700, 20, 19), (40, 3000, 32, 2), (5, 100, 1, 3)])
+@pytest.mark.parametrize("n_traj,max_len,top_n,bins", [(24, 9000, 20, 6), (3, 700, 20, 19), (40, 3000, 32, 2), (5, 100, 1, 3), (7, 500, 18, 4), (9, 300, 27, 2)])
 def test_acceptance_matches_oracle(n_traj, max_len, top_n, bins):
     inp = W.make_acceptance_inputs(n_traj, max_len, top_n=top_n, seed=n_traj, device=DEV)
     a, bq, bc = _run(inp, top_n, 2048, bins, 0.05)
@@ -45,6 +45,25 @@ def test_acceptance_matches_oracle(n_traj, max_len, top_n, bins):
     # the statistic the paper tracks decays with length on this workload
     if bins == 6:
         assert bq[0] > bq[3] > 0
+
+
+def test_acceptance_with_lists_that_are_not_16_byte_aligned():
+    """The alpha kernel stages its lists with 16-byte loads only when top_n is a multiple of 4 AND the four arrays are 16-byte
+    aligned; copies that start 4 bytes into an allocation must take the scalar path and give the same values."""
+    def shifted(t):                          # same values, base pointer + one element (4 bytes)
+        buf = torch.empty((t.numel() + 1,), dtype=t.dtype, device=t.device)
+        v = buf[1:].view(t.shape)
+        v.copy_(t)
+        assert v.data_ptr() % 16 != 0 and v.is_contiguous()
+        return v
+    inp = W.make_acceptance_inputs(6, 400, top_n=20, seed=5, device=DEV)
+    ref, _, _ = _run(inp, 20, 2048, 2, 0.05)
+    mis = {k: (shifted(v) if k in ("ids_p", "logp_p", "ids_q", "logp_q") else v) for k, v in inp.items()}
+    got, _, _ = _run(mis, 20, 2048, 2, 0.05)
+    h = {k: v.cpu().numpy() for k, v in inp.items() if k != "lens"}
+    want = oracle.acceptance_rate(h["ids_p"], h["logp_p"].astype(np.float64), h["ids_q"], h["logp_q"].astype(np.float64))
+    assert np.abs(got - want).max() <= TOL and np.abs(ref - want).max() <= TOL
+    assert np.array_equal(got, ref)          # same arithmetic either way, only the staging differs
 
 
 def test_acceptance_exact_rank_on_the_gpu_values_and_edge_cases():
