@@ -49,7 +49,8 @@ typedef enum sparrow_status {
     SPARROW_ERR_INVALID_ARG = -1,        /* null / negative / misaligned argument */
     SPARROW_ERR_UNSUPPORTED = -2,        /* shape outside the supported set (see above) */
     SPARROW_ERR_WORKSPACE_TOO_SMALL = -3,
-    SPARROW_ERR_CUDA = -4                /* launch or runtime failure; text via sparrow_strerror */
+    SPARROW_ERR_CUDA = -4,               /* launch or runtime failure; text via sparrow_strerror */
+    SPARROW_ERR_STATIC_SCRATCH_TOO_SMALL = -5   /* sparrow_select_static only: the shape needs more than SPARROW_SELECT_STATIC_BYTES */
 } sparrow_status;
 
 typedef struct sparrow_shape {
@@ -133,6 +134,32 @@ int sparrow_select(const void *q, const void *summaries, const int32_t *page_tab
                    const sparrow_schedule_t *sched, int32_t *sel_pages, int32_t max_sel, int32_t *sel_count,
                    float *scores_dbg, void *workspace, size_t workspace_bytes,
                    const sparrow_shape_t *shape, void *stream);
+
+/* ---- a2..a5 for callers that cannot allocate device memory: sparrow_select with the scratch built into the library ----
+ * Same computation, same arguments and same results as sparrow_select, minus `workspace`: the selector's scratch (arrival
+ * counters + fp32 page scores, sparrow_select_workspace_bytes(shape) bytes) lives in a fixed array inside the library
+ * image instead of a buffer the caller allocates.  It is meant for code that is handed device pointers for its inputs
+ * and outputs but has no allocator of its own to call: a plug-in or custom op inside a serving process whose memory pool
+ * has already claimed the whole GPU (a cudaMalloc there fails, or takes memory the pool believes it owns), a step inside
+ * a latency-critical decode loop where cudaMalloc / cudaFree would stall the device, or a caller reaching this C ABI from
+ * a language runtime that has no CUDA allocation binding at all.  The call itself performs no cudaMalloc, no cudaFree and
+ * no library call that allocates.
+ *   Limit: sparrow_select_workspace_bytes(shape) <= SPARROW_SELECT_STATIC_BYTES (4 MiB: roughly
+ *     n_seq * n_kv_heads * max_pages_per_seq <= 1 000 000, e.g. 64 sequences x 8 kv-heads x 2 000 pages); a larger shape
+ *     returns SPARROW_ERR_STATIC_SCRATCH_TOO_SMALL before anything is launched -- use sparrow_select there.  The 4 MiB
+ *     are resident on every GPU the process uses this library on, from the moment the library is loaded there until the
+ *     process exits, whether or not this entry point is ever called.
+ *   First call on a device: looks up the array's address on that device (one synchronous runtime query, remembered per
+ *     device).  Make that first call during start-up, with the device current, before any stream capture begins.
+ *   Sharing: there is ONE array per GPU and every call on that GPU uses it, whatever the stream or host thread.  Calls
+ *     that may overlap on the GPU (two streams, two threads) race on it and give wrong selections; calls ordered one after
+ *     the other on a stream (or otherwise serialised) are fine.  The array keeps the previous call's contents; the
+ *     counters that must start at zero are cleared on `stream` at the head of each call. */
+#define SPARROW_SELECT_STATIC_BYTES (4u << 20)
+int sparrow_select_static(const void *q, const void *summaries, const int32_t *page_table, const int32_t *seq_lens,
+                          const sparrow_schedule_t *sched, int32_t *sel_pages, int32_t max_sel, int32_t *sel_count,
+                          float *scores_dbg, const sparrow_shape_t *shape, void *stream);
+size_t sparrow_select_static_bytes(void);   /* SPARROW_SELECT_STATIC_BYTES of the loaded build (host only) */
 
 /* ---- a6 + a7: split-K flash-decode over the selected pages, log-sum-exp merge ---------------------
  * out[i][h] = softmax_t(sm_scale * q[i][h].K_t) V_t over tokens t < L of the pages sel_pages[i][h/r][0..sel_count[i]),

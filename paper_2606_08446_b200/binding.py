@@ -84,6 +84,8 @@ _SHP, _SCH = C.POINTER(sparrow_shape_t), C.POINTER(sparrow_schedule_t)
 _SIGS = {
     "sparrow_summarize": (C.c_int, [_vp, _vp, _vp, _vp, _i64, _SHP, _vp]),
     "sparrow_select": (C.c_int, [_vp, _vp, _vp, _vp, _SCH, _vp, _i32, _vp, _vp, _vp, _sz, _SHP, _vp]),
+    "sparrow_select_static": (C.c_int, [_vp, _vp, _vp, _vp, _SCH, _vp, _i32, _vp, _vp, _SHP, _vp]),
+    "sparrow_select_static_bytes": (_sz, []),
     "sparrow_sparse_decode": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _i32, _vp, _vp, _vp, _f, _vp, _sz, _SHP, _vp]),
     "sparrow_dense_decode": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _f, _vp, _sz, _SHP, _vp]),
     "sparrow_append": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _SHP, _vp]),
@@ -224,6 +226,21 @@ def sparrow_select(q, summaries, page_table, seq_lens, sched, sel_pages, max_sel
                              0 if workspace is None else workspace.numel() * workspace.element_size(), _by(shape), _stream(stream))
     if check:
         _check(rc, "sparrow_select")
+    return rc
+
+
+def sparrow_select_static_bytes() -> int:
+    return _lib.sparrow_select_static_bytes()
+
+
+def sparrow_select_static(q, summaries, page_table, seq_lens, sched, sel_pages, max_sel: int, sel_count, scores_dbg,
+                          shape, stream=None, *, check=True):
+    """sparrow_select without a workspace argument: the scratch is a fixed 4 MiB array inside the library, for callers that
+    cannot allocate device memory themselves (see include/sparrow.h for the limit and the sharing rule)."""
+    rc = _lib.sparrow_select_static(_ptr(q), _ptr(summaries), _ptr(page_table), _ptr(seq_lens), _by(sched), _ptr(sel_pages),
+                                    max_sel, _ptr(sel_count), _ptr(scores_dbg), _by(shape), _stream(stream))
+    if check:
+        _check(rc, "sparrow_select_static")
     return rc
 
 

@@ -399,6 +399,10 @@ const char *sparrow_strerror(int status)
     case SPARROW_ERR_UNSUPPORTED: return "unsupported shape (need head_dim 128, page_size 16|32|64|128, 1 <= Hq/Hkv <= 8, bf16)";
     case SPARROW_ERR_WORKSPACE_TOO_SMALL: return "workspace too small";
     case SPARROW_ERR_CUDA: return g_errbuf[0] ? g_errbuf : "CUDA error";
+    case SPARROW_ERR_STATIC_SCRATCH_TOO_SMALL:
+        return "shape needs more selector scratch than the library's built-in array holds (sparrow_select_static is limited "
+               "to SPARROW_SELECT_STATIC_BYTES = 4 MiB, i.e. n_seq * n_kv_heads * max_pages_per_seq up to about one million): "
+               "use sparrow_select with a workspace of your own";
     default: return "unknown status";
     }
 }
@@ -505,6 +509,81 @@ int sparrow_select(const void *q, const void *summaries, const int32_t *page_tab
     if (!aligned16(q) || !aligned16(summaries) || !aligned16(workspace)) return SPARROW_ERR_INVALID_ARG;
     return select_impl(q, summaries, page_table, seq_lens, sd, sel_pages, max_sel, sel_count, scores_dbg, workspace,
                        workspace_bytes, shape, (cudaStream_t)stream);
+}
+
+}  // extern "C"
+
+// ---- sparrow_select_static: page selection for callers that have no way to hand the library a workspace ----------------
+// The selector needs scratch beyond its inputs and outputs (one arrival counter per (sequence, kv-head) unit and the fp32
+// page scores the unit's last CTA ranks).  sparrow_select takes that from the caller; this variant takes it from the
+// array below, which is part of the library image: the driver places it in every GPU's memory when the library is loaded
+// on that GPU and keeps it until the process exits.  Nothing here calls cudaMalloc / cudaFree or any routine that does.
+//
+// In HOST code the name g_select_static_scratch is only a handle for the symbol: it is not a device address, and a kernel
+// given it would read and write the wrong memory.  The address a kernel can use comes from cudaGetSymbolAddress, asked
+// once per device with that device current (each GPU has its own copy of the array at its own address).
+namespace {
+static __device__ __align__(256) unsigned char g_select_static_scratch[SPARROW_SELECT_STATIC_BYTES];
+
+void *g_select_static_ptr[kMaxDevices];             // per device: the array's device address (nullptr = not asked yet)
+std::mutex g_select_static_mutex;
+
+// The array's address on the calling thread's current device; first call per device does the look-up (a synchronous
+// runtime call, which is why the header asks for that first call to come before any stream capture).
+void *select_static_scratch(int *rc)
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess || dev < 0 || dev >= kMaxDevices) {
+        snprintf(g_errbuf, sizeof(g_errbuf), "cudaGetDevice failed or device ordinal >= %d", kMaxDevices);
+        *rc = SPARROW_ERR_CUDA;
+        return nullptr;
+    }
+    std::lock_guard<std::mutex> lock(g_select_static_mutex);
+    if (!g_select_static_ptr[dev]) {
+        void *p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_select_static_scratch);
+        if (e != cudaSuccess || !p) {
+            snprintf(g_errbuf, sizeof(g_errbuf), "cudaGetSymbolAddress(select static scratch) on device %d: %s", dev,
+                     cudaGetErrorString(e));
+            *rc = SPARROW_ERR_CUDA;
+            return nullptr;
+        }
+        g_select_static_ptr[dev] = p;
+    }
+    return g_select_static_ptr[dev];
+}
+}  // namespace
+
+extern "C" {
+
+size_t sparrow_select_static_bytes(void) { return SPARROW_SELECT_STATIC_BYTES; }
+
+int sparrow_select_static(const void *q, const void *summaries, const int32_t *page_table, const int32_t *seq_lens,
+                          const sparrow_schedule_t *sched, int32_t *sel_pages, int32_t max_sel, int32_t *sel_count,
+                          float *scores_dbg, const sparrow_shape_t *shape, void *stream)
+{
+    g_launches = 0;
+    int rc = check_shape(shape);
+    if (rc) return rc;
+    SchedDev sd;
+    rc = to_dev_sched(sched, &sd, shape->page_size);
+    if (rc) return rc;
+    if (!q || !summaries || !page_table || !seq_lens || !sel_pages || !sel_count || max_sel <= 0) return SPARROW_ERR_INVALID_ARG;
+    if (!aligned16(q) || !aligned16(summaries)) return SPARROW_ERR_INVALID_ARG;
+    const size_t need = sparrow_select_workspace_bytes(shape);
+    if (need > SPARROW_SELECT_STATIC_BYTES) return SPARROW_ERR_STATIC_SCRATCH_TOO_SMALL;   // before any CUDA call
+    if (shape->n_seq == 0) return SPARROW_OK;
+    void *ws = select_static_scratch(&rc);
+    if (!ws) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    // The array still holds whatever the previous call (possibly of another shape, possibly one that failed half-way)
+    // left in it.  Only the arrival counters must start at zero -- every score the ranking reads is written by this call
+    // first -- so they are cleared here, on the caller's stream, ahead of the kernel.
+    cudaError_t e = cudaMemsetAsync(ws, 0, select_ctr_bytes(shape), st);
+    if (e != cudaSuccess) return cuda_fail(e, "memset(select static scratch counters)");
+    return select_impl(q, summaries, page_table, seq_lens, sd, sel_pages, max_sel, sel_count, scores_dbg, ws,
+                       SPARROW_SELECT_STATIC_BYTES, shape, st);
 }
 
 int sparrow_sparse_decode(const void *q, const void *k_cache, const void *v_cache, const int32_t *page_table,
