@@ -44,6 +44,12 @@
 extern "C" {
 #endif
 
+/* ABI version of this header = what sparrow_version() of a matching library returns.  It changes whenever a struct layout or
+ * a signature does: 100 = the first layout; 300 = sparrow_shape_t with landmark + kv_stride_*, sparrow_step_host over one
+ * host block (sparrow_step / sparrow_step_workspace_bytes removed), sparrow_select_static.  A caller built against another
+ * header must not pass its structs to this library: compare SPARROW_ABI_VERSION with sparrow_version() at start-up. */
+#define SPARROW_ABI_VERSION 300
+
 typedef enum sparrow_status {
     SPARROW_OK = 0,
     SPARROW_ERR_INVALID_ARG = -1,        /* null / negative / misaligned argument */
@@ -62,6 +68,7 @@ typedef struct sparrow_shape {
     int32_t max_pages_per_seq;   /* row stride of page_table */
     int64_t n_phys_pages;        /* pages in the K/V pools */
     int32_t landmark;            /* SPARROW_LANDMARK_MINMAX (0, north_star's default) or SPARROW_LANDMARK_MEAN (1) */
+    int32_t flags;               /* 0 or SPARROW_FLAG_DETERMINISTIC (below); occupies what was padding: offsets and size unchanged */
     /* Strides of the K and V pools in ELEMENTS (both pools share them; the head dim is contiguous): row t of kv-head g of
      * physical page p starts at p * kv_stride_page + g * kv_stride_head + t * kv_stride_tok.  All three 0 (the default) =
      * the packed "HND" layout [n_phys_pages][n_kv_heads][page_size][128] this library is tuned for (a (page, kv-head) tile
@@ -72,6 +79,17 @@ typedef struct sparrow_shape {
      * own packed layout either way. */
     int64_t kv_stride_page, kv_stride_head, kv_stride_tok;
 } sparrow_shape_t;
+
+/* sparrow_shape_t.flags.
+ * SPARROW_FLAG_DETERMINISTIC: the decode entry points (sparse, dense, and the decode inside sparrow_step_host) hand their
+ *   page tiles to the CTA's warps in a fixed pattern (warp w takes tile pairs w, w + 8, ...) and merge the pieces of a unit
+ *   that spans CTAs in one fixed order, so `out` and `lse` are BIT-IDENTICAL from call to call on the same inputs, shape and
+ *   GPU model (the split of the tile stream over the SMs depends on the SM count).  Without it tiles go to whichever warp is
+ *   free, which balances the warps slightly better; results then agree only to the arithmetic's own error (see
+ *   sparrow_sparse_decode).  A rollout engine whose log-probabilities are compared with a trainer's (PAPER.md:76-79,
+ *   :409-414: the rollout / policy mismatch the paper measures) should set it.  Selection, summaries and append are
+ *   bit-reproducible either way.  Measured cost: DESIGN.md 6.3 / profiles/r3_deterministic.md. */
+enum { SPARROW_FLAG_DETERMINISTIC = 1 };
 
 /* Form of the page landmark (PAPER.md:147 leaves it open; reading R1):
  *   MINMAX  per-channel min and max of the page's keys, summaries [n_phys_pages][n_kv_heads][2][128] (512 B), score =

@@ -31,7 +31,7 @@ class SparrowError(RuntimeError):
 class sparrow_shape_t(C.Structure):
     _fields_ = [("n_seq", C.c_int32), ("n_q_heads", C.c_int32), ("n_kv_heads", C.c_int32), ("head_dim", C.c_int32),
                 ("page_size", C.c_int32), ("max_pages_per_seq", C.c_int32), ("n_phys_pages", C.c_int64), ("landmark", C.c_int32),
-                ("kv_stride_page", C.c_int64), ("kv_stride_head", C.c_int64), ("kv_stride_tok", C.c_int64)]
+                ("flags", C.c_int32), ("kv_stride_page", C.c_int64), ("kv_stride_head", C.c_int64), ("kv_stride_tok", C.c_int64)]
 
 
 class sparrow_schedule_t(C.Structure):
@@ -54,8 +54,11 @@ class sparrow_cost_t(C.Structure):
 LANDMARK = {"minmax": 0, "mean": 1}
 
 
+FLAG_DETERMINISTIC = 1
+
+
 def make_shape(n_seq, n_q_heads, n_kv_heads, max_pages_per_seq, n_phys_pages, head_dim=128, page_size=16, landmark="minmax",
-               kv_layout="hnd"):
+               kv_layout="hnd", deterministic=False):
     """kv_layout: "hnd" (packed [page][kv-head][token][128], strides left 0), "nhd" ([page][token][kv-head][128]) or a tuple
     (stride_page, stride_head, stride_tok) in elements."""
     if kv_layout == "hnd":
@@ -64,7 +67,8 @@ def make_shape(n_seq, n_q_heads, n_kv_heads, max_pages_per_seq, n_phys_pages, he
         st = (page_size * n_kv_heads * head_dim, head_dim, n_kv_heads * head_dim)
     else:
         st = tuple(int(x) for x in kv_layout)
-    return sparrow_shape_t(n_seq, n_q_heads, n_kv_heads, head_dim, page_size, max_pages_per_seq, n_phys_pages, LANDMARK[landmark], *st)
+    return sparrow_shape_t(n_seq, n_q_heads, n_kv_heads, head_dim, page_size, max_pages_per_seq, n_phys_pages, LANDMARK[landmark],
+                           FLAG_DETERMINISTIC if deterministic else 0, *st)
 
 
 def make_schedule(spec: dict, page_size: int = 0) -> sparrow_schedule_t:
@@ -111,6 +115,12 @@ for _name, (_res, _args) in _SIGS.items():
     _fn = getattr(_lib, _name)          # AttributeError here = the library does not export a declared symbol
     _fn.restype, _fn.argtypes = _res, _args
 EXPORTS = tuple(_SIGS)
+# the struct layouts above are those of ABI 300 (include/sparrow.h: SPARROW_ABI_VERSION); a library built from another header
+# would read garbage strides out of a shorter or longer sparrow_shape_t
+ABI_VERSION = 300
+if _lib.sparrow_version() != ABI_VERSION:
+    raise ImportError(f"{LIB_PATH} reports ABI {_lib.sparrow_version()}, this binding is written for {ABI_VERSION}: rebuild it "
+                      "(`python -m paper_2606_08446_b200.build --force`)")
 
 
 def _check(rc: int, what: str):

@@ -117,6 +117,7 @@ int check_shape(const sparrow_shape_t *s)
     if (r < 1 || r > kMaxGroup) return SPARROW_ERR_UNSUPPORTED;
     if (s->n_kv_heads > 65535 || s->n_seq > 65535) return SPARROW_ERR_UNSUPPORTED;     // grid.y / grid.z
     if (s->landmark != SPARROW_LANDMARK_MINMAX && s->landmark != SPARROW_LANDMARK_MEAN) return SPARROW_ERR_INVALID_ARG;
+    if (s->flags & ~SPARROW_FLAG_DETERMINISTIC) return SPARROW_ERR_INVALID_ARG;          // unknown bits (or a caller that left the old padding unset)
     if (s->kv_stride_page != 0 || s->kv_stride_head != 0 || s->kv_stride_tok != 0) {
         const int64_t sp = s->kv_stride_page, sh = s->kv_stride_head, stt = s->kv_stride_tok;
         if (sp <= 0 || sh <= 0 || stt < kDim || (sp & 7) || (sh & 7) || (stt & 7)) return SPARROW_ERR_INVALID_ARG;
@@ -271,10 +272,11 @@ int launch_decode(const void *q, const void *k_cache, const void *v_cache, const
     const DecodeGeom gm = decode_geom(s, kDense ? 0 : max_sel);
     if (workspace_bytes < gm.bytes_ctr + gm.bytes_o + gm.bytes_ml) return SPARROW_ERR_WORKSPACE_TOO_SMALL;
     if (s->n_seq > kDecMaxSeq) return SPARROW_ERR_UNSUPPORTED;
-    {   // flat tile positions and TMA row coordinates are 32-bit
+    {   // flat tile positions and TMA row coordinates are 32-bit: the packed map's row coordinate is tile * 32 (decode.cuh),
+        // so tile indices must stay below 2^26 (a 256 GiB pool -- beyond one B200, but the guard says what it protects)
         const int64_t max_cnt = kDense ? s->max_pages_per_seq : (max_sel < s->max_pages_per_seq ? max_sel : s->max_pages_per_seq);
         const int64_t tpp = s->page_size / kPage;
-        if ((int64_t)s->n_seq * max_cnt * s->n_kv_heads * tpp >= (1LL << 31) || s->n_phys_pages * s->n_kv_heads * tpp >= (1LL << 27))
+        if ((int64_t)s->n_seq * max_cnt * s->n_kv_heads * tpp >= (1LL << 31) || s->n_phys_pages * s->n_kv_heads * tpp >= (1LL << 26))
             return SPARROW_ERR_UNSUPPORTED;
     }
     if (s->n_seq == 0 || s->n_phys_pages == 0) return SPARROW_OK;
@@ -305,6 +307,7 @@ int launch_decode(const void *q, const void *k_cache, const void *v_cache, const
         kv_layout(s, &packed);
         A.strided = packed ? 0 : 1;
     }
+    A.deterministic = (s->flags & SPARROW_FLAG_DETERMINISTIC) ? 1 : 0;
     const int grid = ds->sms < kDecGrid ? ds->sms : kDecGrid;   // one CTA per SM (the partial slots are sized for 148)
     launch_chain(decode_kernel<kDense>, dim3(grid), dim3(kDecThreads), smem, st, A, tm_k, tm_v);
     SPARROW_CHECK_LAUNCH("decode_kernel");
@@ -377,7 +380,7 @@ int select_impl(const void *q, const void *summaries, const int32_t *page_table,
 
 extern "C" {
 
-int sparrow_version(void) { return 100; }
+int sparrow_version(void) { return SPARROW_ABI_VERSION; }
 
 int sparrow_trace_set(void *buffer)
 {
@@ -396,7 +399,9 @@ const char *sparrow_strerror(int status)
     switch (status) {
     case SPARROW_OK: return "ok";
     case SPARROW_ERR_INVALID_ARG: return "invalid argument (null, negative or misaligned)";
-    case SPARROW_ERR_UNSUPPORTED: return "unsupported shape (need head_dim 128, page_size 16|32|64|128, 1 <= Hq/Hkv <= 8, bf16)";
+    case SPARROW_ERR_UNSUPPORTED:
+        return "unsupported shape (need head_dim 128, page_size 16|32|64|128, 1 <= Hq/Hkv <= 8, bf16; decode: n_seq <= 4096, "
+               "pool below 2^26 16-token tiles; select: n_seq <= 65535, max_pages_per_seq <= 16384)";
     case SPARROW_ERR_WORKSPACE_TOO_SMALL: return "workspace too small";
     case SPARROW_ERR_CUDA: return g_errbuf[0] ? g_errbuf : "CUDA error";
     case SPARROW_ERR_STATIC_SCRATCH_TOO_SMALL:

@@ -135,7 +135,8 @@ __host__ __device__ inline SeqPlan make_plan(const SchedDev &s, int64_t L)
 // ---- tracing build (-DSPARROW_TRACE; `python -m paper_2606_08446_b200.build --trace`, read by paper_2606_08446_b200/trace.py):
 // the kernels drop %globaltimer stamps into a caller-provided buffer [65536 slots][8] of 64-bit words (sparrow_trace_set).
 // In the normal build SPARROW_TR() is empty and the kernels carry no trace of it.
-//   select_kernel:  slot = linear CTA index; 0 start, 1 prologue done, 2 summary stream done (warp 0), 3 CTA barrier passed,
+//   select_kernel:  slot = linear CTA index (CTAs past slot 55999 leave no stamps: the slots above belong to the decode, and
+//                   nothing is ever written past the buffer's 65536 slots); 0 start, 1 prologue done, 2 summary stream done (warp 0), 3 CTA barrier passed,
 //                   4 arrival atomic done, 5 top-k done (last CTA of a unit), 7 keys in shared memory, 6 radix select done
 //   decode_kernel:  slot = 60000 + CTA; 0 start, 1 dependency wait over, 2 prefix table built, 3 look-up warp finished,
 //                   4 first tile landed;   slot = 56000 + 9 x CTA + warp; 0 warp entry, 1 warp exit
@@ -151,7 +152,7 @@ __device__ __forceinline__ unsigned long long trace_now()
     do {                                                                          \
         const unsigned long long t__ = sparrow::trace_now();                      \
         unsigned long long *g__ = sparrow::g_trace;                               \
-        if (g__) g__[(size_t)(slot) * 8 + (k)] = t__;                             \
+        if (g__ && (unsigned)(slot) < (unsigned)sparrow::kTraceSlots) g__[(size_t)(slot) * 8 + (k)] = t__; \
     } while (0)
 #else
 #define SPARROW_TR(slot, k) do { } while (0)

@@ -85,6 +85,11 @@ constexpr int kTailChunk = 32;                                  // tiles of a se
 #ifndef SPARROW_DEC_STATIC_DEN
 #define SPARROW_DEC_STATIC_DEN 1
 #endif
+// deterministic mode (SPARROW_FLAG_DETERMINISTIC): rounds a consumer may run ahead of the slowest one (0 = no limit)
+#ifndef SPARROW_DEC_DET_WINDOW
+#define SPARROW_DEC_DET_WINDOW 1
+#endif
+constexpr int kDetWindow = SPARROW_DEC_DET_WINDOW;
 constexpr int kDecMetaBytes = kDecStages * 8 + kDecStages * 4 + 3 * kAccSlots * 4 + kDecConsumers * 4 + 64;   // (+ claim, ready, total)   // full barriers | issued tile per stage | area generation, tile count, consumer mask | consumer positions | claim, ready
 
 __device__ __forceinline__ void ldsm_x4(uint32_t &r0, uint32_t &r1, uint32_t &r2, uint32_t &r3, uint32_t addr)
@@ -169,6 +174,7 @@ struct DecodeArgs {
     int n_seq, n_q_heads, n_kv_heads, max_pages;
     int tpp_log2;                // log2 of the 16-token tiles per page (page size 16, 32, 64, 128 -> 0, 1, 2, 3)
     int strided;                 // the pools are not the packed HND layout: tiles are fetched with 5-D boxes (sparrow_shape_t kv_stride_*)
+    int deterministic;           // SPARROW_FLAG_DETERMINISTIC: fixed tile hand-out and merge order -- out / lse are bit-reproducible
 };
 
 // The CTA ranges: T tiles over G CTAs, the first `extra` CTAs one tile longer.
@@ -561,12 +567,17 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
         // store -> release atomic -> load -> store (four dependent trips, all at the very end of a CTA's stream, where they
         // are the launch's tail: the piece that ends a CTA's range is usually the LAST of its unit to finish, its neighbour
         // having started with it).
+        // (The fold below starts from this part's registers and takes the other pieces in stream order; the slow path folds
+        // every piece in stream order.  Which of the two runs, and for which piece, is a matter of timing -- two summation
+        // orders for one unit.  Deterministic mode therefore has a fast path of its own, after this one.)
+        bool completes = false;
         {
             int cur = 0;
             if (lane == 0) asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(cur) : "l"(A.counters + unit) : "memory");
             cur = __shfl_sync(kFull, cur, 0);
             __syncwarp();                                           // orders lane 0's acquire before the other lanes' loads
-            if (cur + part_len == c) {
+            completes = cur + part_len == c;
+            if (completes && !A.deterministic) {
                 float m_f = m_new, l_f = l_new;
                 for (int s2 = 0; s2 < nseg; ++s2) {
                     const int pid = piece_of(s2);
@@ -603,6 +614,84 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
                 if (lane == 0) A.counters[unit] = 0;                // restore the zero for the next call (nobody else is left to touch it)
                 return;
             }
+        }
+        if (completes) {
+            // DETERMINISTIC FAST PATH: the same saving (no store / atomic / re-load of this part), but the fold is the slow
+            // path's, operation for operation: pieces in stream order from an empty state, this part's registers taking
+            // their place in that order.  Pieces before it are folded into a temporary, a half row at a time (register
+            // budget); the (m, l) recurrence is recomputed for each half, so both halves see identical weights.
+            int own = 0;
+            while (piece_of(own) != piece.x) ++own;
+            const int64_t row_of0 = (int64_t)unit * r + (hrow < r ? hrow : 0);
+            float m_f = -INFINITY, l_f = 0.f;
+#pragma unroll
+            for (int half = 0; half < 2; ++half) {
+                float2 acc[8];
+#pragma unroll
+                for (int nt = 0; nt < 8; ++nt) acc[nt] = make_float2(0.f, 0.f);
+                float m_a = -INFINITY, l_a = 0.f;
+                for (int s2 = 0; s2 < own; ++s2) {                  // pieces before this one
+                    const int64_t row = row_of0 + (int64_t)piece_of(s2) * r;
+                    float2 ml2 = make_float2(-INFINITY, 0.f);
+                    if (hrow < r) ml2 = __ldcg(reinterpret_cast<const float2 *>(A.ws_ml + row * 2));
+                    if (!(ml2.y > 0.f)) continue;                   // empty partial: contributes nothing (as in the slow path)
+                    float2 v[8];
+#pragma unroll
+                    for (int nt = 0; nt < 8; ++nt) v[nt] = __ldcg(reinterpret_cast<const float2 *>(A.ws_o + row * kDim + col + (half * 8 + nt) * 8));
+                    const float m2 = fmaxf(m_a, ml2.x);
+                    const float w_old = fast_exp2(m_a - m2), w_new = fast_exp2(ml2.x - m2);
+                    l_a = fmaf(ml2.y, w_new, l_a * w_old);
+#pragma unroll
+                    for (int nt = 0; nt < 8; ++nt) {
+                        acc[nt].x = fmaf(v[nt].x, w_new, acc[nt].x * w_old);
+                        acc[nt].y = fmaf(v[nt].y, w_new, acc[nt].y * w_old);
+                    }
+                    m_a = m2;
+                }
+                if (l_new > 0.f) {                                  // this part, from the registers
+                    const float m2 = fmaxf(m_a, m_new);
+                    const float w_old = fast_exp2(m_a - m2), w_new = fast_exp2(m_new - m2);
+                    l_a = fmaf(l_new, w_new, l_a * w_old);
+#pragma unroll
+                    for (int nt = 0; nt < 8; ++nt) {
+                        o[half * 8 + nt][0] = fmaf(o[half * 8 + nt][0], w_new, acc[nt].x * w_old);
+                        o[half * 8 + nt][1] = fmaf(o[half * 8 + nt][1], w_new, acc[nt].y * w_old);
+                    }
+                    m_a = m2;
+                } else {
+#pragma unroll
+                    for (int nt = 0; nt < 8; ++nt) { o[half * 8 + nt][0] = acc[nt].x; o[half * 8 + nt][1] = acc[nt].y; }
+                }
+                for (int s2 = own + 1; s2 < nseg; ++s2) {           // pieces after this one
+                    const int64_t row = row_of0 + (int64_t)piece_of(s2) * r;
+                    float2 ml2 = make_float2(-INFINITY, 0.f);
+                    if (hrow < r) ml2 = __ldcg(reinterpret_cast<const float2 *>(A.ws_ml + row * 2));
+                    if (!(ml2.y > 0.f)) continue;
+                    float2 v[8];
+#pragma unroll
+                    for (int nt = 0; nt < 8; ++nt) v[nt] = __ldcg(reinterpret_cast<const float2 *>(A.ws_o + row * kDim + col + (half * 8 + nt) * 8));
+                    const float m2 = fmaxf(m_a, ml2.x);
+                    const float w_old = fast_exp2(m_a - m2), w_new = fast_exp2(ml2.x - m2);
+                    l_a = fmaf(ml2.y, w_new, l_a * w_old);
+#pragma unroll
+                    for (int nt = 0; nt < 8; ++nt) {
+                        o[half * 8 + nt][0] = fmaf(v[nt].x, w_new, o[half * 8 + nt][0] * w_old);
+                        o[half * 8 + nt][1] = fmaf(v[nt].y, w_new, o[half * 8 + nt][1] * w_old);
+                    }
+                    m_a = m2;
+                }
+                m_f = m_a; l_f = l_a;
+            }
+            if (hrow < r) {
+                const float inv = l_f > 0.f ? 1.f / l_f : 0.f;
+                uint32_t *dst = reinterpret_cast<uint32_t *>(A.out + ((int64_t)unit * r + hrow) * kDim + col);
+#pragma unroll
+                for (int nt = 0; nt < 16; ++nt) dst[nt * 4] = pack_bf16(o[nt][0] * inv, o[nt][1] * inv);
+                if (A.lse && (lane & 3) == 0)
+                    A.lse[(int64_t)unit * r + hrow] = l_f > 0.f ? (m_f + log2f(l_f)) * kLn2 : -INFINITY;
+            }
+            if (lane == 0) A.counters[unit] = 0;                    // restore the zero for the next call
+            return;
         }
         // SLOW PATH: park the partial in slot unit + piece id and add this part's tiles to the unit's counter.  Release /
         // acquire through ONE atomic of lane 0: the warp barrier orders the lanes' partial stores before the acq_rel atomic
@@ -682,11 +771,39 @@ decode_kernel(const DecodeArgs A, const __grid_constant__ CUtensorMap tm_k, cons
 
     int part = -1, unit = 0, n_mine = 0, part_len = 0;              // the part this consumer is accumulating
     int4 piece = make_int4(0, 0, 0, 0);                             // ... and the piece it belongs to (id, begin, end)
+    int n_claims = 0;                                               // deterministic mode: chunks this consumer has taken
 #pragma unroll 1
     while (true) {
         int cidx = 0;
-        if (lane == 0) cidx = atomicAdd(s_claim, 1);
-        cidx = __shfl_sync(kFull, cidx, 0);
+        if (A.deterministic) {
+            // Fixed hand-out: consumer w takes chunks w, w + 8, w + 16 ... of the CTA's stream -- which tiles a consumer
+            // sums, and in which order, is then a function of the inputs alone.  (Chunk c lives in stages 2c % 16 and
+            // 2c % 16 + 1, so every consumer refills its own two stages; the ring, the descriptors and the parking
+            // protocol are unchanged.)
+            cidx = warp + n_claims * kDecConsumers;
+#if SPARROW_DEC_DET_WINDOW > 0
+            // Drift throttle.  With private tile sequences the consumers drift apart like random walks (each waits out its
+            // own memory latencies), and the CTA ends with its slowest warp running alone at two tiles in flight.  A
+            // consumer therefore starts round k only once every consumer has started round k - kDetWindow: the leaders'
+            // landed tiles wait a little, the bandwidth they would have drawn goes to the laggards.  The slowest consumer
+            // never waits here, so the order in which parts complete (park) is unaffected.
+            if (n_claims > kDetWindow) {
+                const int need = (n_claims - kDetWindow) * kDecConsumers * kDecChunk;      // first tile of round k - window
+                for (uint32_t n = 0;; ++n) {
+                    int lo = lane < kDecConsumers ? lds_volatile(s_pos + lane) : 0x7fffffff;
+#pragma unroll
+                    for (int of = 4; of > 0; of >>= 1) lo = min(lo, __shfl_xor_sync(kFull, lo, of));
+                    lo = __shfl_sync(kFull, lo, 0);
+                    if (lo >= need) break;
+                    if (n > (1u << 27)) __trap();
+                }
+            }
+#endif
+            ++n_claims;
+        } else {
+            if (lane == 0) cidx = atomicAdd(s_claim, 1);
+            cidx = __shfl_sync(kFull, cidx, 0);
+        }
         const int it0 = cidx * kDecChunk;
         if (lane == 0) sts_volatile(s_pos + warp, it0);
         const int n_it = exists(it0) ? (exists(it0 + 1) ? 2 : 1) : 0;   // tiles of this claim that exist

@@ -227,7 +227,9 @@ select_kernel(const uint16_t *__restrict__ q, const uint16_t *__restrict__ summa
               int n_q_heads, int n_kv_heads, int max_pages, int pages_per_cta)
 {
     chain_entry();
-    const int tr_slot = (blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;   // tracing build only
+    // tracing build only: the linear CTA index while it stays below the decode's slot ranges, else "no slot"
+    const long long tr_lin = ((long long)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
+    const int tr_slot = tr_lin < kTraceDecodeWarp ? (int)tr_lin : kTraceSlots;
     (void)tr_slot;
     if (threadIdx.x == 0) SPARROW_TR(tr_slot, 0);
     extern __shared__ uint32_t s_keys[];                 // [n_pages] (phase B only)

@@ -15,14 +15,14 @@ from .workloads import PAGE, Workload, full_page_updates
 
 class SparrowEngine:
     def __init__(self, wl: Workload, schedule: Optional[dict] = None, want_scores: bool = False, landmark: str = "minmax",
-                 kv_layout="hnd"):
+                 kv_layout="hnd", deterministic=False):
         assert wl.q.is_cuda, "the engine needs the workload on a CUDA device (no CPU fallback)"
         self.wl = wl
         dev = wl.q.device
         self.landmark = landmark      # "minmax" (north_star's default, 512 B per page and head) or "mean" (the cost model's single vector, 256 B)
         # kv_layout: how wl.k_cache / wl.v_cache are laid out -- "hnd" (packed, the default), "nhd" or explicit element strides
         self.shape = B.make_shape(wl.n_seq, wl.Hq, wl.Hkv, wl.max_pages, wl.n_phys, page_size=wl.page_size, landmark=landmark,
-                                  kv_layout=kv_layout)
+                                  kv_layout=kv_layout, deterministic=deterministic)
         self.set_schedule(schedule or wl.schedule)
         self.summaries = torch.zeros((wl.n_phys, wl.Hkv, 2, 128) if landmark == "minmax" else (wl.n_phys, wl.Hkv, 128),
                                      dtype=torch.bfloat16, device=dev)

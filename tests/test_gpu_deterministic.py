@@ -1,0 +1,126 @@
+"""SPARROW_FLAG_DETERMINISTIC (``-m gpu``): with the flag the decode's tile hand-out and merge orders are fixed, so two
+calls on the same inputs must agree BIT FOR BIT -- out, lse, and of course the page lists -- and the result must still pass
+the oracle's gates.  This is the bitwise guard the run-time hand-out of the default mode cannot give (tests there use
+parity_util.assert_same_result, a tolerance); the protocol that could drop or double-count a small partial -- parking areas,
+cross-piece partials, the completing part's fast path -- is the same code in both modes, so an intermittent slip in it shows
+here as a differing bit instead of hiding inside a tolerance.  PAPER.md:76-79, :409-414: the paper's subject is the
+log-prob mismatch between rollout and trainer; a rollout kernel should not add a source of its own."""
+import pytest
+import torch
+
+from paper_2606_08446_b200 import workloads as W
+
+from parity_util import check_dense, check_sparse_step
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+
+
+def _engine(wl, **kw):
+    from paper_2606_08446_b200.engine import SparrowEngine
+    eng = SparrowEngine(wl, deterministic=True, **kw)
+    eng.summarize_all()
+    return eng
+
+
+def _repeat_bitwise(eng, n_runs, dense_runs=0):
+    eng.step()
+    torch.cuda.synchronize()
+    sel0, cnt0, out0, lse0 = eng.sel_pages.clone(), eng.sel_count.clone(), eng.out.clone(), eng.lse.clone()
+    for i in range(n_runs):
+        eng.sel_pages.fill_(-1); eng.sel_count.zero_(); eng.out.zero_(); eng.lse.zero_()
+        eng.step()
+        torch.cuda.synchronize()
+        assert torch.equal(eng.sel_pages, sel0) and torch.equal(eng.sel_count, cnt0), f"run {i}: selection differs"
+        assert torch.equal(eng.out, out0), f"run {i}: out differs in {(eng.out != out0).sum().item()} elements"
+        assert torch.equal(eng.lse, lse0), f"run {i}: lse differs"
+    if dense_runs:
+        eng.dense_decode()
+        torch.cuda.synchronize()
+        d0, l0 = eng.out_dense.clone(), eng.lse_dense.clone()
+        for i in range(dense_runs):
+            eng.out_dense.zero_(); eng.lse_dense.zero_()
+            eng.dense_decode()
+            torch.cuda.synchronize()
+            assert torch.equal(eng.out_dense, d0) and torch.equal(eng.lse_dense, l0), f"dense run {i} differs"
+
+
+@pytest.mark.parametrize("cfg", ["cfg2", "cfg5"])
+def test_full_size_step_is_bit_reproducible(cfg):
+    """The launch configuration bench.py times, 20 times over: every unit spans parts of several consumers, most CTAs end
+    inside a unit (cross-piece partials, both the completing part's fast path and the slow path occur)."""
+    wl = W.make_config(cfg, device=DEV)
+    eng = _engine(wl)
+    _repeat_bitwise(eng, 20, dense_runs=3)
+    check_sparse_step(eng, wl, check_summ=False, out_idx=list(range(0, wl.n_seq, 4)))      # and it is still the right answer
+
+
+@pytest.mark.parametrize("Hq,Hkv,page,lens,budget", [
+    (8, 2, 16, [33000], 9000),                      # one unit per kv-head over tens of CTAs: up to 74 partials per unit
+    (5, 1, 16, [20000, 17, 3, 9000], 6000),         # r = 5, tiny units between long ones
+    (16, 8, 64, [40000, 300, 25000], 20000),        # page 64: four tiles per page
+    (2, 2, 16, [1, 15, 16, 17, 33, 250, 256, 257, 1000, 2049, 4099], 200),   # r = 1, ragged
+])
+def test_bit_reproducible_and_oracle_exact_on_awkward_shapes(Hq, Hkv, page, lens, budget):
+    sched = W._sched("fixed", 16, 64, fixed_tokens=budget)
+    wl = W.make_workload(n_seq=len(lens), Hq=Hq, Hkv=Hkv, lengths=("list", lens), schedule=sched, seed=Hq * 7 + Hkv, device=DEV,
+                         plant=True, poison_tail=True, page_size=page)
+    eng = _engine(wl, want_scores=True)
+    _repeat_bitwise(eng, 10, dense_runs=5)
+    check_sparse_step(eng, wl)
+    check_dense(eng, wl)
+
+
+def test_many_short_sequences_bit_reproducible():
+    """The workload of test_gpu_parity.test_many_short_sequences: tens of parts per CTA, more sequences than decode threads."""
+    import numpy as np
+    rng = np.random.default_rng(11)
+    lens = [int(x) for x in rng.integers(1, 700, size=700)]
+    lens[5], lens[77], lens[699] = 1, 16, 2500
+    wl = W.make_workload(n_seq=len(lens), Hq=4, Hkv=2, lengths=("list", lens), schedule=W._sched("fixed", 16, 32, fixed_tokens=96),
+                         seed=4242, device=DEV, poison_tail=True, plant=True)
+    eng = _engine(wl, want_scores=True)
+    _repeat_bitwise(eng, 10, dense_runs=5)
+    check_sparse_step(eng, wl)
+    check_dense(eng, wl)
+
+
+def test_graph_replay_and_host_entry_are_bitwise_equal_to_the_eager_device_path():
+    from paper_2606_08446_b200 import binding as B
+    wl = W.make_workload(n_seq=6, Hq=8, Hkv=4, lengths=("list", [3000, 4000, 513, 9000, 77, 2500]),
+                         schedule=W._sched("fixed", 64, 256, fixed_tokens=1024), seed=3, device=DEV, plant=True)
+    eng = _engine(wl)
+    eng.step()
+    torch.cuda.synchronize()
+    ref_sel, ref_out, ref_lse = eng.sel_pages.clone(), eng.out.clone(), eng.lse.clone()
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        eng.step(stream=st)
+        st.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=st):
+            eng.step(stream=st)
+        for _ in range(5):
+            eng.sel_pages.fill_(-1); eng.out.zero_(); eng.lse.zero_()
+            g.replay()
+            st.synchronize()
+            assert torch.equal(eng.sel_pages, ref_sel) and torch.equal(eng.out, ref_out) and torch.equal(eng.lse, ref_lse)
+    torch.cuda.synchronize()
+    # the host-buffer entry runs the same kernels on its own scratch: same bits
+    scratch = torch.zeros((B.sparrow_step_scratch_bytes(eng.shape, eng.max_sel),), dtype=torch.uint8, device=DEV)
+    hb = B.HostBlock(eng.shape)
+    hb.q.copy_(wl.q.cpu()); hb.seq_lens.copy_(wl.seq_lens.cpu())
+    out_h = torch.zeros_like(hb.q).pin_memory()
+    B.sparrow_step_host(hb.block, 0, False, wl.k_cache, wl.v_cache, eng.summaries, wl.page_table, eng.sched, eng.max_sel,
+                        wl.sm_scale, out_h, scratch, eng.shape)
+    assert torch.equal(out_h, ref_out.cpu())
+
+
+def test_unknown_flag_bits_are_refused():
+    from paper_2606_08446_b200 import binding as B
+    shp = B.make_shape(2, 4, 2, 8, 16)
+    assert B.sparrow_decode_workspace_bytes(shp, 4) > 0
+    shp.flags = 2
+    assert B.sparrow_decode_workspace_bytes(shp, 4) == 0      # check_shape: INVALID_ARG
+    shp.flags = B.FLAG_DETERMINISTIC
+    assert B.sparrow_decode_workspace_bytes(shp, 4) > 0

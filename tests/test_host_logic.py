@@ -33,6 +33,17 @@ def test_library_exports_every_declared_symbol(B):
     assert declared == set(B.EXPORTS), "binding and header disagree"
 
 
+def test_abi_version_matches_header_and_struct_layout(B):
+    """the ABI changed without a version bump.  sparrow_version() == SPARROW_ABI_VERSION of the header == the
+    binding's ABI_VERSION (binding.py refuses to import otherwise), and `flags` sits in what used to be padding."""
+    hdr = open(os.path.join(ROOT, "include", "sparrow.h")).read()
+    ver = int(re.search(r"#define\s+SPARROW_ABI_VERSION\s+(\d+)", hdr).group(1))
+    assert B.sparrow_version() == ver == B.ABI_VERSION
+    T = B.sparrow_shape_t
+    assert ctypes.sizeof(T) == 64 and T.landmark.offset == 32 and T.flags.offset == 36 and T.kv_stride_page.offset == 40
+    assert B.sparrow_select_static_bytes() == int(re.search(r"#define\s+SPARROW_SELECT_STATIC_BYTES\s+\((\d+)u << 20\)", hdr).group(1)) << 20
+
+
 def test_stride_validation(B):
     """sparrow_shape_t kv_stride_*: all zero = packed HND; otherwise 16-byte multiples whose rows do not overlap."""
     shp = B.make_shape(2, 4, 2, 8, 16, kv_layout=(16 * 2 * 128, 128, 2 * 128))
