@@ -1,7 +1,7 @@
 """GPU parity tests (``-m gpu``): the CUDA library, called through the C ABI binding, against the fp64 oracle,
 element by element on the same seeded inputs.  Sizes span several tiles / chunks and ragged tails; the
 full-size BASELINE.json configs (2, 3, 4, 5) are checked in the launch configuration bench.py times: selection on
-every sequence, outputs on every sequence (cfg2, cfg5) or 32 of them (cfg3, cfg4)."""
+every sequence, outputs on every sequence (cfg4: every sequence of one K/V pool)."""
 import numpy as np
 import pytest
 import torch
@@ -170,6 +170,45 @@ def test_schedules_medium_batch(sched):
     check_sparse_step(eng, wl)
 
 
+def test_near_tie_across_the_threshold_takes_the_band_and_r11_path():
+    """R10 / R11 on GPU data.  Per unit, the page at the top-k threshold (A) is copied onto an unselected candidate with a
+    HIGHER index (B), and one key of B is raised by one bf16 step in a channel where the group's queries are 2^-20: in
+    fp64 B now outscores A by ~1e-8 (relative 1e-11, far inside the 1e-4 band) and the oracle picks B; in fp32 the two
+    scores round to the same number and the kernel's tie rule keeps A.  Both are valid results: the checker must accept the
+    list through the band rule and compare the attention on the GPU's own sets -- branches no other test has reached."""
+    lens = [3000, 4100, 2500, 5000]
+    wl = W.make_workload(n_seq=len(lens), Hq=8, Hkv=2, lengths=("list", lens), schedule=W._sched("fixed", 64, 256, fixed_tokens=1024),
+                         seed=91, device=DEV, plant=True)
+    d0 = 5
+    wl.q[:, :, d0] = 2.0 ** -20
+    h = wl.host()
+    sched = oracle.Schedule.from_spec(wl.schedule)
+    res = oracle.sparse_step(h["q"], h["k_cache"], h["v_cache"], h["page_table"], h["seq_lens"], sched, wl.sm_scale, do_attention=False)
+    made = 0
+    for i, L in enumerate(lens):
+        n_pages = -(-L // 16)
+        F = set(np.flatnonzero(res["forced"][i, :n_pages]).tolist())
+        cnt = int(res["sel_count"][i])
+        for g in range(wl.Hkv):
+            row = set(res["sel"][i, g, :cnt].tolist())
+            top = sorted(row - F, key=lambda p: res["scores"][i, g, p])
+            a = top[0]                                                # the page at the threshold
+            assert res["scores"][i, g, a] == res["tau"][i, g] and res["scores"][i, g, top[1]] > res["tau"][i, g]
+            b = max(p for p in range(n_pages) if p not in row and p > a)
+            pa, pb = int(wl.page_table[i, a]), int(wl.page_table[i, b])
+            wl.k_cache[pb, g] = wl.k_cache[pa, g]
+            col = wl.k_cache[pb, g, :, d0]
+            t = int(col.float().argmax())
+            bits = col.view(torch.int16)
+            assert float(col[t]) != 0.0
+            bits[t] += 1 if float(col[t]) > 0 else -1                # one bf16 step up: the page's max in channel d0 rises
+            made += 1
+    eng = _run_sparse(wl, want_scores=True)
+    st = check_sparse_step(eng, wl)
+    print(f"near ties planted in {made} units: {st}")
+    assert st["differing_units"] >= made // 2 and st["band_pages"] >= 2 * (made // 2)
+
+
 def test_all_ties_zero_query_picks_lowest_pages():
     lens = [1200, 640, 5000]
     sched = W._sched("fixed", 16, 32, fixed_tokens=320)
@@ -259,9 +298,10 @@ def test_error_statuses_on_device_calls():
 
 # ------------------------------------------------------------------ full-size BASELINE.json configs ----
 # The launch configuration bench.py times.  Selection (count, order, range, F, band rule, fp32 scores) and the summaries
-# are checked on EVERY sequence of the batch; out / lse on every sequence of cfg2 / cfg5 and on 32 of cfg3 / cfg4 (the
-# shortest, the longest, every sequence of cfg4 that goes dense inside the sparse batch, and seeded others).
-@pytest.mark.parametrize("cfg,n_out", [("cfg2", None), ("cfg5", None), ("cfg3", 32), ("cfg4", 32)])
+# are checked on EVERY sequence of the batch, and so are out / lse (the oracle needs about a second per config on the box's
+# cores; the n_out parameter remains for sampling, unused).  The dense entry is compared on the shortest and the longest
+# sequence and on sequences of cfg4 that go dense inside the sparse batch.
+@pytest.mark.parametrize("cfg,n_out", [("cfg2", None), ("cfg5", None), ("cfg3", None), ("cfg4", None)])
 def test_full_size_config_against_oracle(cfg, n_out):
     wl = W.make_config(cfg, device=DEV)
     eng = _run_sparse(wl, want_scores=True)
