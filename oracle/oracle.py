@@ -330,7 +330,9 @@ def cost_model(P, B, N, L_in, L_out, D, r, I, K, pagesize, c=1.0) -> dict:
     L_out^2 / 2 terms).  The paper charges one D-vector read (memory D) and r D multiply-adds (compute r D) per landmark
     vector visited -- its clean terms at :142 are memory I N D L_out^2 / (2 pagesize), compute r N D L_out^2 / (2 pagesize),
     the same r : 1 ratio as the attention terms -- so with c landmark vectors per page:
-    memory c B N D S;  compute r c B N D S.   C = C_comp + I C_mem."""
+    memory c B N D S;  compute r c B N D S.   C = C_comp + I C_mem.
+    "parity unpinned": the L_in part of S.  PAPER.md:142 prints its L_in scoring terms without the 1 / pagesize factor; R21
+    reads that as garbled, and the only pin of these terms is a per-step sum written from the same reading."""
     L_dense = min(L_out, max(K - L_in, 0.0))
     H = (2 * L_in + L_dense) * L_dense + 2 * K * max(L_out - L_dense, 0.0)
     H_dense = (2 * L_in + L_out) * L_out
