@@ -669,10 +669,12 @@ def run_cfg4(args, rank, local_rank, world, dev) -> dict:
             p = l % n_pools
             e, wl, (hb, n_upd) = engs[p], wls[p], hbs[p]
             B.sparrow_step_host(hb.block, n_upd, False, wl.k_cache, wl.v_cache, e.summaries, wl.page_table,
-                                dense_spec if l < n_dense else e.sched, e.max_sel, wl.sm_scale, out_h, scr[p], e.shape, st)
+                                dense_spec if l < n_dense else e.sched, e.max_sel, wl.sm_scale, out_h, scr[p], e.shape, st,
+                                wait=False)          # 36 layers enqueued (each with its H2D and D2H) ...
+        st.synchronize()                                 # ... and ONE wait per step, where the caller reads the result
     host_full_step()
     D.barrier(); torch.cuda.synchronize()
-    Ke = max(1, min(K, 5))
+    Ke = K                                               # the same K steps as the device-resident value
     h0e, h1e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     h0e.record(st)
     for _ in range(Ke):

@@ -228,6 +228,16 @@ int sparrow_step_host(const void *in_block_host, int64_t n_update, int has_n_val
                       const sparrow_schedule_t *sched, int32_t max_sel, float sm_scale,
                       void *out_host, void *scratch, size_t scratch_bytes,
                       const sparrow_shape_t *shape, void *stream);
+/* The same step, left ENQUEUED: returns once the copies and kernels are on `stream`, without waiting for them.  A model
+ * step is many layers; waiting after each costs a host round trip per layer (36 per step at config 4) during which the GPU
+ * idles.  The caller waits once (cudaStreamSynchronize / an event) before it reads out_host, and must leave in_block_host
+ * and out_host untouched until then; pinned memory is needed for the copies to be asynchronous at all.  Calls on the
+ * same stream may share `scratch` (they run in stream order). */
+int sparrow_step_host_async(const void *in_block_host, int64_t n_update, int has_n_valid,
+                            const void *k_cache, const void *v_cache, void *summaries, const int32_t *page_table,
+                            const sparrow_schedule_t *sched, int32_t max_sel, float sm_scale,
+                            void *out_host, void *scratch, size_t scratch_bytes,
+                            const sparrow_shape_t *shape, void *stream);
 /* Size of the host block and (optional out-parameters) the offsets of its seq_lens / page_ids / n_valid parts. */
 size_t sparrow_step_host_block_bytes(const sparrow_shape_t *shape, size_t *off_seq_lens, size_t *off_page_ids,
                                      size_t *off_n_valid);

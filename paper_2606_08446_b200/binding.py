@@ -94,6 +94,7 @@ _SIGS = {
     "sparrow_dense_decode": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _f, _vp, _sz, _SHP, _vp]),
     "sparrow_append": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _SHP, _vp]),
     "sparrow_step_host": (C.c_int, [_vp, _i64, C.c_int, _vp, _vp, _vp, _vp, _SCH, _i32, _f, _vp, _vp, _sz, _SHP, _vp]),
+    "sparrow_step_host_async": (C.c_int, [_vp, _i64, C.c_int, _vp, _vp, _vp, _vp, _SCH, _i32, _f, _vp, _vp, _sz, _SHP, _vp]),
     "sparrow_step_host_block_bytes": (_sz, [_SHP, C.POINTER(_sz), C.POINTER(_sz), C.POINTER(_sz)]),
     "sparrow_select_workspace_bytes": (_sz, [_SHP]),
     "sparrow_decode_workspace_bytes": (_sz, [_SHP, _i32]),
@@ -304,8 +305,10 @@ class HostBlock:
 
 
 def sparrow_step_host(in_block, n_update: int, has_n_valid: bool, k_cache, v_cache, summaries,
-                      page_table, sched, max_sel: int, sm_scale: float, out_host, scratch, shape, stream=None, *, check=True):
-    rc = _lib.sparrow_step_host(_ptr(in_block, cuda=False), n_update, 1 if has_n_valid else 0, _ptr(k_cache), _ptr(v_cache),
+                      page_table, sched, max_sel: int, sm_scale: float, out_host, scratch, shape, stream=None, *, check=True,
+                      wait=True):
+    """wait=False: sparrow_step_host_async -- the step stays enqueued on the stream; synchronise before reading out_host."""
+    rc = (_lib.sparrow_step_host if wait else _lib.sparrow_step_host_async)(_ptr(in_block, cuda=False), n_update, 1 if has_n_valid else 0, _ptr(k_cache), _ptr(v_cache),
                                 _ptr(summaries), _ptr(page_table), _by(sched), max_sel, sm_scale, _ptr(out_host, cuda=False),
                                 _ptr(scratch), scratch.numel() * scratch.element_size(), _by(shape), _stream(stream))
     if check:

@@ -351,9 +351,14 @@ int select_impl(const void *q, const void *summaries, const int32_t *page_table,
     // Pages per CTA: as large as keeps >= 4 CTAs per resident slot (4 per SM) so the tail stays short, because the
     // per-CTA fixed costs (loads of L / table entries / query rows, arrival) are amortised over the pages a CTA streams.
     const int64_t units = (int64_t)s->n_seq * s->n_kv_heads;
+    // The mean landmark streams half the bytes per page, so its per-CTA fixed costs weigh twice as much: there the largest
+    // slice that still leaves two CTAs per SM wins (measured, round 3: cfg2 27.6 -> 24.2 us, cfg5 37.8 -> 34.5 us, cfg3
+    // unchanged; most units are then ONE CTA, which also skips the cross-CTA arrival before the top-k).
+    const bool mean_lm = s->landmark == SPARROW_LANDMARK_MEAN;
+    const int64_t ctas_wanted = mean_lm ? 2 * (int64_t)ds->sms : 4 * (int64_t)kSelMinBlocks * ds->sms;
     int pages_per_cta = kSelCtaPagesMin;
     for (int p = 4 * kSelCtaPagesMin; p > kSelCtaPagesMin; p >>= 1) {
-        if (units * ((s->max_pages_per_seq + p - 1) / p) >= 4 * kSelMinBlocks * ds->sms) { pages_per_cta = p; break; }
+        if (units * ((s->max_pages_per_seq + p - 1) / p) >= ctas_wanted) { pages_per_cta = p; break; }
     }
 #ifdef SPARROW_SEL_PPC_FIXED
     pages_per_cta = SPARROW_SEL_PPC_FIXED;
@@ -752,10 +757,11 @@ size_t sparrow_step_host_block_bytes(const sparrow_shape_t *s, size_t *off_seq_l
     return c.in_end;
 }
 
-int sparrow_step_host(const void *in_block_host, int64_t n_update, int has_n_valid, const void *k_cache, const void *v_cache,
-                      void *summaries, const int32_t *page_table, const sparrow_schedule_t *sched, int32_t max_sel,
-                      float sm_scale, void *out_host, void *scratch, size_t scratch_bytes, const sparrow_shape_t *s,
-                      void *stream)
+namespace {
+int step_host_impl(const void *in_block_host, int64_t n_update, int has_n_valid, const void *k_cache, const void *v_cache,
+                   void *summaries, const int32_t *page_table, const sparrow_schedule_t *sched, int32_t max_sel,
+                   float sm_scale, void *out_host, void *scratch, size_t scratch_bytes, const sparrow_shape_t *s,
+                   void *stream, bool wait)
 {
     g_launches = 0;
     int rc = check_shape(s);
@@ -796,8 +802,27 @@ int sparrow_step_host(const void *in_block_host, int64_t n_update, int has_n_val
     }
     if (rc) return rc;
     if ((e = cudaMemcpyAsync(out_host, base + c.out, qbytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e, "D2H out");
-    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e, "stream sync");
+    if (wait && (e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e, "stream sync");
     return SPARROW_OK;
+}
+}  // namespace
+
+int sparrow_step_host(const void *in_block_host, int64_t n_update, int has_n_valid, const void *k_cache, const void *v_cache,
+                      void *summaries, const int32_t *page_table, const sparrow_schedule_t *sched, int32_t max_sel,
+                      float sm_scale, void *out_host, void *scratch, size_t scratch_bytes, const sparrow_shape_t *s,
+                      void *stream)
+{
+    return step_host_impl(in_block_host, n_update, has_n_valid, k_cache, v_cache, summaries, page_table, sched, max_sel, sm_scale,
+                          out_host, scratch, scratch_bytes, s, stream, true);
+}
+
+int sparrow_step_host_async(const void *in_block_host, int64_t n_update, int has_n_valid, const void *k_cache, const void *v_cache,
+                            void *summaries, const int32_t *page_table, const sparrow_schedule_t *sched, int32_t max_sel,
+                            float sm_scale, void *out_host, void *scratch, size_t scratch_bytes, const sparrow_shape_t *s,
+                            void *stream)
+{
+    return step_host_impl(in_block_host, n_update, has_n_valid, k_cache, v_cache, summaries, page_table, sched, max_sel, sm_scale,
+                          out_host, scratch, scratch_bytes, s, stream, false);
 }
 
 }  // extern "C"

@@ -114,6 +114,14 @@ def test_graph_replay_and_host_entry_are_bitwise_equal_to_the_eager_device_path(
     B.sparrow_step_host(hb.block, 0, False, wl.k_cache, wl.v_cache, eng.summaries, wl.page_table, eng.sched, eng.max_sel,
                         wl.sm_scale, out_h, scratch, eng.shape)
     assert torch.equal(out_h, ref_out.cpu())
+    # ... and so does the enqueue-only form, several steps in flight on one stream sharing the scratch, one wait at the end
+    outs = [torch.zeros_like(hb.q).pin_memory() for _ in range(4)]
+    for o in outs:
+        B.sparrow_step_host(hb.block, 0, False, wl.k_cache, wl.v_cache, eng.summaries, wl.page_table, eng.sched, eng.max_sel,
+                            wl.sm_scale, o, scratch, eng.shape, wait=False)
+    torch.cuda.current_stream().synchronize()
+    for o in outs:
+        assert torch.equal(o, ref_out.cpu())
 
 
 def test_unknown_flag_bits_are_refused():
