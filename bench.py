@@ -461,7 +461,7 @@ def run_single(args, cfg, rank, local_rank, world, dev, headline=True) -> dict:
     roof_kernel = "decode_kernel<sparse> (one sparrow_sparse_decode call; LSE merge fused in the same launch)"
     gbs = lambda b, ms: b / (ms * 1e-3) / 1e9
     dec_gbs, sel_gbs, dense_gbs = gbs(roof_bytes, k_dec["ms"]), gbs(ab["select"], k_sel["ms"]), gbs(ab["dense"], dense_ms)
-    traffic, traffic_note = ncu_traffic(cfg, "decode_kernel")
+    traffic, traffic_note = ncu_traffic(cfg, "decode_kernel" + ("@deterministic" if args.deterministic else ""))
     ms_step = t_max * 1e3 / K
     res = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
