@@ -246,7 +246,8 @@ size_t sparrow_step_host_block_bytes(const sparrow_shape_t *shape, size_t *off_s
  * Per token position i < n_pos the dense policy P and the sparse policy Q each give their top_n (<= 32) tokens and
  * natural-log probabilities: ids_p, logp_p, ids_q, logp_q are [n_pos][top_n].  alpha[i] = sum over the tokens present
  * in BOTH lists of min(p, q) -- Eq. 1's sum_x min(p(x), q(x)) restricted to what the engine returns (reading R23; a
- * token missing from one list adds nothing; ids are assumed distinct within a list).  Positions are grouped in bins
+ * token missing from one list adds nothing; ids must be >= 0 -- the kernel pads short lists with -1 -- and distinct within a
+ * list).  Positions are grouped in bins
  * b = min(positions[i] / bin_tokens, n_bins - 1) (2K-token bins in the paper); bin_count[b] = tokens in the bin and
  * bin_quantile[b] = the nearest-rank `quantile` (0.05 in the paper) of alpha over the bin: the value of rank
  * max(1, ceil(quantile * count)) in ascending order, NaN for an empty bin.  fp32 throughout; exact selection.
@@ -292,7 +293,7 @@ const char *sparrow_strerror(int status);   /* static string; for SPARROW_ERR_CU
 int sparrow_version(void);
 /* Kernels launched by the most recent entry-point call on this thread (for gpu_launches accounting). */
 int sparrow_last_launch_count(void);
-/* Tracing build only (compiled with -DSPARROW_TRACE: `python -m paper_2606_08446_b200.build --trace`): the select and
+/* Profiling plumbing, not one of the method's calls.  Tracing build only (compiled with -DSPARROW_TRACE: `python -m paper_2606_08446_b200.build --trace`): the select and
  * decode kernels drop %globaltimer stamps per CTA / warp into `buffer`, a DEVICE array of 65536 x 8 64-bit words the
  * caller zeroes (layout: csrc/common.cuh); NULL switches the stamps off.  Synchronous (a symbol copy).  The normal build
  * carries no stamps and returns SPARROW_ERR_UNSUPPORTED.  Used by paper_2606_08446_b200/trace.py for the timelines under

@@ -18,12 +18,17 @@ def sources():
 
 
 def source_hash() -> str:
-    """Short hash of the kernel sources + the C header: names the build a measurement (e.g. an ncu capture) was taken on."""
+    """Short hash of the kernel sources + the C header: names the build a measurement (e.g. an ncu capture) was taken on.
+    Comments and whitespace are left out of it, so a documentation edit does not orphan the captures under profiles/."""
     import hashlib
+    import re
     h = hashlib.sha256()
     for f in sources():
         h.update(os.path.basename(f).encode())
-        h.update(open(f, "rb").read())
+        text = open(f, "r", encoding="utf-8").read()
+        text = re.sub(r"/\*.*?\*/", " ", text, flags=re.S)          # block comments
+        text = re.sub(r"(?<![:\"'])//[^\n]*", " ", text)            # line comments (not the // of a string or URL)
+        h.update(" ".join(text.split()).encode())
     return h.hexdigest()[:12]
 
 
