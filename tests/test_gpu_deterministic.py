@@ -132,3 +132,63 @@ def test_unknown_flag_bits_are_refused():
     assert B.sparrow_decode_workspace_bytes(shp, 4) == 0      # check_shape: INVALID_ARG
     shp.flags = B.FLAG_DETERMINISTIC
     assert B.sparrow_decode_workspace_bytes(shp, 4) > 0
+
+
+def test_rollout_as_one_graph_is_bitwise_equal_to_step_by_step():
+    """The rollout chain append -> select -> decode, T steps: run step by step and as ONE CUDA graph on a fresh copy of the
+    batch.  With the flag the two must agree in every bit of every step's out and lse (the default mode's version of this
+    check, tests/test_gpu_rollout.py, can only assert a tolerance)."""
+    from paper_2606_08446_b200.engine import SparrowEngine
+    T, lens = 20, [250, 1023, 15, 2040, 4090]
+    sched = W._sched("table", 16, 48, table_pages=(6, 9, 14, 20, 20, 24, 24, 30, 40), bin_tokens=512)
+
+    def setup():
+        wl = W.make_workload(n_seq=len(lens), Hq=8, Hkv=2, lengths=("list", lens), schedule=sched, seed=21, device=DEV,
+                             reserve_tokens=T + 3, plant=True)
+        eng = SparrowEngine(wl, deterministic=True)
+        eng.summarize_all()
+        eng.reserve(T)
+        return (wl, eng) + tuple(W.make_rollout_inputs(wl, T, seed=5))
+
+    wl, eng, qs, ks, vs = setup()
+    out = torch.zeros((T, wl.n_seq, wl.Hq, 128), dtype=torch.bfloat16, device=DEV)
+    lse = torch.zeros((T, wl.n_seq, wl.Hq), dtype=torch.float32, device=DEV)
+    for t in range(T):
+        eng.append(ks[t], vs[t]); eng.select(qs[t]); eng.sparse_decode(qs[t], out=out[t], lse=lse[t])
+        torch.cuda.synchronize()
+    wl2, eng2, qs2, ks2, vs2 = setup()
+    out2, lse2 = torch.zeros_like(out), torch.zeros_like(lse)
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=st):
+            eng2.rollout(qs2, ks2, vs2, out2, lse2, stream=st)
+        g.replay()
+    st.synchronize()
+    torch.cuda.synchronize()
+    assert wl2.seq_lens.cpu().tolist() == [L + T for L in lens]
+    assert torch.equal(out2, out) and torch.equal(lse2, lse)
+    assert torch.equal(wl2.k_cache, wl.k_cache) and torch.equal(eng2.summaries, eng.summaries)
+
+
+@pytest.mark.parametrize("Hq,Hkv,page", [(8, 2, 16), (5, 1, 16), (16, 8, 64)])
+def test_nhd_pools_give_the_same_bits_as_packed_pools(Hq, Hkv, page):
+    """Strided pools are fetched with 5-D TMA boxes that land in shared memory exactly as the packed layout's 2-D boxes do:
+    same tiles, same hand-out, so -- with the flag -- the same bits out of the sparse and the dense entry."""
+    import copy
+    from paper_2606_08446_b200.engine import SparrowEngine
+    lens = [1, 16, 17, 250, 1000, 2049, 4099, 700]
+    wl = W.make_workload(n_seq=len(lens), Hq=Hq, Hkv=Hkv, lengths=("list", lens), schedule=W._sched("fixed", 16, 64, fixed_tokens=300),
+                         seed=Hq * 31 + page, device=DEV, poison_tail=True, plant=True, page_size=page)
+    nhd = copy.copy(wl)
+    nhd.k_cache = wl.k_cache.permute(0, 2, 1, 3).contiguous()
+    nhd.v_cache = wl.v_cache.permute(0, 2, 1, 3).contiguous()
+    eng = SparrowEngine(nhd, kv_layout="nhd", deterministic=True)
+    ref = SparrowEngine(wl, deterministic=True)
+    for e in (eng, ref):
+        e.summarize_all(); e.step(); e.dense_decode()
+    torch.cuda.synchronize()
+    assert torch.equal(eng.sel_pages, ref.sel_pages) and torch.equal(eng.sel_count, ref.sel_count)
+    assert torch.equal(eng.out, ref.out) and torch.equal(eng.lse, ref.lse)
+    assert torch.equal(eng.out_dense, ref.out_dense) and torch.equal(eng.lse_dense, ref.lse_dense)
+    check_sparse_step(ref, wl, check_summ=False)
