@@ -693,7 +693,7 @@ def run_cfg4(args, rank, local_rank, world, dev) -> dict:
     dec_gbs, sel_gbs = gbs(ab["decode"], k_dec["ms"]), gbs(ab["select"], k_sel["ms"])
     hb0 = hbs[0][0]
     qbytes = int(hb0.q.numel() * 2)
-    traffic, traffic_note = ncu_traffic("cfg4", "decode_kernel")
+    traffic, traffic_note = ncu_traffic("cfg4", "decode_kernel" + ("@deterministic" if args.deterministic else ""))
     ms_step = t_max * 1e3 / K
     step_bytes = (n_layers - n_dense) * (ab["decode"] + ab["select"]) + n_dense * ab["dense"]
     res = {
